@@ -1,0 +1,197 @@
+/*
+ * stag.h -- C ABI of libstag: the single-GPU hot path of the mixed-precision
+ * staggered-fermion CG inverter of arXiv:1111.0125 (Jang, Kim, Lee, Lattice
+ * 2011), written for NVIDIA B200 (sm_100a).
+ *
+ * Citations "P:Lnn" are lines of the paper text; "Qn" are the
+ * readings listed in DESIGN.md where the paper is silent.
+ *
+ * What the library computes
+ *   D chi(x) = sum_mu [ W_mu(x) chi(x+mu) - W_mu(x-mu)^dag chi(x-mu) ]   eq. 2.5
+ *   A        = -D^2 + m^2 on the even sites = m^2 - D_eo D_oe             eq. 2.3
+ *   A x = b  by conjugate gradient (Fig. 1), in fp64, in fp32, by
+ *            iterative refinement (Fig. 2) or with the corrected
+ *            restart + reliable + group-wise updates of section 3.2
+ * W_mu(x) = eta_mu(x) * bc_mu(x) * U_mu(x): the staggered phases (and the
+ * antiperiodic time boundary) are folded into the links by the caller before
+ * the solver is entered, as the paper does.
+ *
+ * Geometry (all entry points)
+ *   dims = (X0,X1,X2,X3), every extent even and >= 2; mu = 3 is time.
+ *   site index   idx = x0 + X0*(x1 + X1*(x2 + X2*x3))
+ *   parity       p = (x0+x1+x2+x3) & 1   (0 = even)
+ *   checkerboard cb = idx >> 1,  Vh = X0*X1*X2*X3/2 sites per parity
+ *
+ * Canonical (interchange) layouts, fp64, C order -- what the caller hands in:
+ *   links   W[mu][p][cb][i][j][re,im]   4*2*Vh*18 doubles
+ *   spinor  chi[cb][i][re,im]           Vh*6 doubles, one parity
+ *
+ * Device (working) layouts -- what the kernels read and write:
+ *   spinor, one parity, precision fp64 or fp32: three colour planes of
+ *     complex numbers,  v[c][cb],  c = 0..2, cb = 0..Vh_pad-1, where
+ *     Vh_pad = Vh rounded up to a multiple of 32.  Pad entries are zero and
+ *     every kernel keeps them zero.  stag_spinor_bytes() gives the size.
+ *   links: owned by the opaque handle, see stag_links_create().
+ *
+ * Pointers: every `void *` / `const void *` spinor argument is DEVICE memory
+ * in the device layout unless the name ends in `_host`.  The caller owns all
+ * spinor buffers; the library owns only what hangs off a stag_links_t.
+ * All calls are asynchronous on the stream set by stag_set_stream() except
+ * where stated.  No call throws or aborts; every `int` return is a
+ * stag_status (0 = OK, < 0 = failure, > 0 = solver outcome that still wrote
+ * its results).
+ */
+#ifndef STAG_H
+#define STAG_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- status codes ------------------------------------------------------- */
+enum {
+    STAG_OK         = 0,
+    STAG_EINVAL     = -1,  /* null pointer, odd or < 2 extent, dims != handle's, bad enum,
+                              tol <= 0, maxiter < 0, out aliases in, 12-real unavailable     */
+    STAG_ECUDA      = -2,  /* a CUDA call failed; text via stag_strerror(STAG_ECUDA)         */
+    STAG_ENOMEM     = -3,  /* device or host allocation failed                               */
+    STAG_ENOCONV    = 1,   /* maxiter reached; x, iters and the true residual ARE written    */
+    STAG_EBREAKDOWN = 2    /* NaN or <d,Ad> <= 0; x, iters and the true residual ARE written */
+};
+
+/* ---- precision / storage of one Dslash ------------------------------------
+ * 18-real: all nine complex entries of each link are stored.
+ * 12-real: rows 0 and 1 are stored; row 2 = s * conj(row0 x row1) is rebuilt
+ *          in registers, s = +-1 recomputed from the site coordinates (Q12). */
+enum {
+    STAG_PREC_F64    = 0,
+    STAG_PREC_F32    = 1,
+    STAG_PREC_F64_R12 = 2,
+    STAG_PREC_F32_R12 = 3
+};
+
+/* ---- CG modes ---------------------------------------------------------- */
+enum {
+    STAG_CG_F64      = 0,  /* Fig. 1 in fp64                                                 */
+    STAG_CG_F32      = 1,  /* Fig. 1 in fp32 (diagnostic: stalls above 1e-10)                */
+    STAG_CG_DEFECT   = 2,  /* Fig. 2: fp64 outer loop, fresh fp32 inner solve of A y = r_k   */
+    STAG_CG_RELIABLE = 3   /* section 3.2: fp32 iteration, direction kept across restarts
+                              (eq. 3.1), reliable + group-wise update on the trigger of P:L97 */
+};
+
+typedef struct stag_links stag_links_t;
+
+/* ---- global state ------------------------------------------------------ */
+
+/* Stream (a cudaStream_t cast to void*) every later call enqueues on; NULL = the legacy
+ * default stream.  Per host thread. */
+int stag_set_stream(void *cuda_stream);
+
+/* Text for a status; for STAG_ECUDA, the text of the last CUDA error seen by this thread.
+ * The pointer stays valid until the next failing call on this thread. */
+const char *stag_strerror(int status);
+
+/* Number of kernel launches (graph-replayed launches included) issued by this library since
+ * the process started or since the last stag_reset_launch_count(). */
+unsigned long long stag_launch_count(void);
+void stag_reset_launch_count(void);
+
+/* ---- links: setup step S0 (P:L60 eta folding is the caller's; "rearranging data
+ * for the coalesced access" is this call) --------------------------------------------
+ *
+ * W: canonical fp64 links (layout above), with eta*bc already folded in; host memory when
+ * on_device == 0, device memory otherwise.  The call reads W before it returns only when W
+ * is host memory (it synchronises the stream in that case); a device W must stay valid until
+ * the stream has passed this call.  antiperiodic_t says whether the caller folded a -1 into
+ * the mu=3 links leaving x3 = X3-1; it is needed only to rebuild 12-real links (Q12).
+ *
+ * The handle keeps, per output parity p and per precision, the EIGHT matrices each output
+ * site needs in one place ("gathered" form):
+ *   M_d(x) = W_d(x)                      d = 0..3   (forward hop)
+ *   M_d(x) = -W_{d-4}(x - (d-4)^)^dag    d = 4..7   (backward hop, sign folded)
+ * so that D chi(x) = sum_d M_d(x) chi(nbr_d(x)), stored in tiles of 32 sites:
+ *   L[p][tile][d][k][lane]  complex,  k = 3*row+col (18-real: 9 entries, 12-real: 6)
+ * The fp64/18 form is built by this call; the other three are built on first use. */
+int stag_links_create(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
+                      const double *W, int on_device);
+void stag_links_destroy(stag_links_t *links);
+
+/* Largest | row2 - s conj(row0 x row1) | over all links, measured when the handle was made.
+ * 12-real precisions are refused (STAG_EINVAL) when it exceeds 1e-10. */
+int stag_links_recon_error(const stag_links_t *links, double *err_out);
+
+/* ---- spinors ----------------------------------------------------------- */
+
+/* Bytes of one single-parity spinor in the device layout (prec: F64 or F32; the _R12
+ * values are accepted and mean the same as their 18-real partner).  0 on bad arguments. */
+size_t stag_spinor_bytes(const int dims[4], int prec);
+
+/* canonical fp64 chi[cb][3][re,im] (device) -> device layout of precision prec, pads zeroed */
+int stag_spinor_pack(void *dst, const double *src_canonical, const int dims[4], int prec);
+/* device layout -> canonical fp64 (device) */
+int stag_spinor_unpack(double *dst_canonical, const void *src, const int dims[4], int prec);
+
+/* ---- the operator ------------------------------------------------------ */
+
+/* One parity hop of eq. 2.5: out (sites of parity `parity`, 0 = even, 1 = odd)
+ * = D in (sites of the other parity).  parity = 1 is D_oe, parity = 0 is D_eo.  576 flop per
+ * output site.  dims must equal the handle's.  out must not alias in. */
+int stag_dslash(void *out, const void *in, const stag_links_t *links, int parity,
+                const int dims[4], int prec);
+
+/* A = -D^2 + m^2 on the even sites (eq. 2.3):
+ *   out_even = mass^2 * in_even - D_eo ( D_oe in_even ).
+ * The odd-parity intermediate lives in scratch owned by the handle.  out must not alias in. */
+int stag_apply_A(void *out_even, const void *in_even, const stag_links_t *links, double mass,
+                 int prec);
+
+/* ---- the solver -------------------------------------------------------- */
+
+/* Optional knobs for stag_cg_solve_ex; zero-initialise, then set what you need
+ * (a zero field means "library default"). */
+typedef struct stag_cg_params {
+    double eps_in;        /* inner tolerance eps^in of P:L82 / P:L97 (Q8).  Default 0.1 for
+                             STAG_CG_RELIABLE, 1e-2 for STAG_CG_DEFECT.                       */
+    int    recon12;       /* 1: the fp32 (and, in mode 0, fp64) Dslash uses 12-real links     */
+    int    graph_chunk;   /* CG iterations per CUDA-graph replay between host checks
+                             (default 32); < 0 disables graphs (plain launches)               */
+    int    recon12_f64;   /* 1: the fp64 correction steps use 12-real links too               */
+} stag_cg_params_t;
+
+typedef struct stag_cg_stats {
+    int    iters;         /* loop passes of Fig. 1 = applications of A to d (Q7)              */
+    int    n_updates;     /* reliable/group-wise updates (mode 3) or outer steps (mode 2)     */
+    int    n_restarts;    /* mode 0: restarts after the true residual missed tol (Q6b)        */
+    int    iters_f32;     /* of iters, how many ran in fp32 (P:L84's "99.8 %")                */
+    int    applies_f64;   /* fp64 applications of A (initial, updates, final residual)        */
+    double true_resid;    /* |b - A x| / |b| in fp64 on exit                                  */
+    double iter_resid;    /* the iterated residual norm / |b| on exit                         */
+    double seconds;       /* device time of the solve (CUDA events around it)                 */
+} stag_cg_stats_t;
+
+/* Solve A x = b on the even sites (eq. 2.1 with A of eq. 2.3).  x (fp64 device layout) holds
+ * the initial guess on entry and the solution on exit; b is fp64 device layout.  Convergence:
+ * |r| <= tol * |b| (Q6), checked on the fp64 true residual before returning.  Synchronises
+ * the stream before returning iterations and true residual.  b = 0 gives x = 0, 0 iterations,
+ * residual 0.  Returns STAG_OK, STAG_ENOCONV, STAG_EBREAKDOWN or an error < 0. */
+int stag_cg_solve(void *x_even, const void *b_even, const stag_links_t *links, double mass,
+                  double tol, int maxiter, int mode, int *iters_out, double *true_resid_out);
+
+int stag_cg_solve_ex(void *x_even, const void *b_even, const stag_links_t *links, double mass,
+                     double tol, int maxiter, int mode, const stag_cg_params_t *params,
+                     stag_cg_stats_t *stats_out);
+
+/* The same solve from and to HOST memory in the canonical fp64 layout (Vh*6 doubles each):
+ * copies b (and x as the initial guess) to the device, packs, solves, unpacks, copies x back.
+ * This is the end-to-end entry bench.py times.  Pinned host memory makes the copies faster
+ * but is not required. */
+int stag_cg_solve_host(double *x_host, const double *b_host, const stag_links_t *links,
+                       double mass, double tol, int maxiter, int mode,
+                       const stag_cg_params_t *params, stag_cg_stats_t *stats_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STAG_H */

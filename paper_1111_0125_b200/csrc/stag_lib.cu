@@ -1,0 +1,754 @@
+// stag_lib.cu -- host side of libstag: the C ABI of include/stag.h, the link handle and its
+// setup kernels (step S0), kernel launchers, and the CG drivers (Fig. 1, Fig. 2, section 3.2).
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "stag_blas.cuh"
+#include "stag_common.cuh"
+#include "stag_dslash.cuh"
+
+using namespace stag;
+
+// ------------------------------------------------------------------------------------
+// per-thread state, errors, launch counting
+// ------------------------------------------------------------------------------------
+namespace {
+
+thread_local cudaStream_t t_stream = nullptr;
+thread_local char t_errbuf[256] = "no error recorded";
+thread_local int t_errbuf_status = 0;   // which status t_errbuf describes
+std::atomic<unsigned long long> g_launches{0};
+thread_local bool t_capturing = false;
+thread_local unsigned long long t_captured_nodes = 0;
+
+inline void count_launch(unsigned long long n = 1)
+{
+    if (t_capturing) t_captured_nodes += n;
+    else g_launches.fetch_add(n, std::memory_order_relaxed);
+}
+
+int cuda_fail(cudaError_t e, const char *what, int line)
+{
+    snprintf(t_errbuf, sizeof(t_errbuf), "%s (line %d): %s", what, line, cudaGetErrorString(e));
+    (void)cudaGetLastError();
+    t_errbuf_status = (e == cudaErrorMemoryAllocation) ? STAG_ENOMEM : STAG_ECUDA;
+    return t_errbuf_status;
+}
+
+#define CU(call)                                                     \
+    do {                                                             \
+        cudaError_t e_ = (call);                                     \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call, __LINE__); \
+    } while (0)
+
+#define KCHECK() CU(cudaGetLastError())
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+inline bool prec_ok(int prec) { return prec >= 0 && prec <= 3; }
+inline bool prec_is_f32(int prec) { return prec == STAG_PREC_F32 || prec == STAG_PREC_F32_R12; }
+inline int prec_rows(int prec) { return (prec == STAG_PREC_F64_R12 || prec == STAG_PREC_F32_R12) ? 2 : 3; }
+
+// Grid of the streaming vector kernels: 4 resident blocks of 256 threads per SM (a multiple of
+// the SM count), fewer when the vector is too short to feed them.
+int blas_grid(long n_reals)
+{
+    static int full = 0;
+    if (full == 0) {
+        int dev = 0, sms = 148;
+        if (cudaGetDevice(&dev) == cudaSuccess)
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        full = sms * 4;
+    }
+    const long need = (n_reals / 2 + BLAS_BLOCK - 1) / BLAS_BLOCK;
+    return (int)(need < full ? (need < 1 ? 1 : need) : full);
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------
+// the link handle
+// ------------------------------------------------------------------------------------
+struct stag_links {
+    Geom g;
+    int dims[4];
+    int ntiles;            // Vh_pad / TILE
+    void *L[4];            // gathered link fields by precision enum; L[STAG_PREC_F64] always set
+    double recon_err;
+    void *tmp_odd[2];      // scratch odd-parity spinor for stag_apply_A: [0] fp64, [1] fp32
+    // CG workspace (lazy)
+    char *ws;
+    size_t ws_bytes;
+    CgCtrl *h_ctrl;        // pinned mirror
+    cudaStream_t cap_stream;
+    // staging for stag_cg_solve_host (lazy)
+    double *stage_dev;     // 2 canonical spinors + 2 device-layout fp64 spinors
+    cudaEvent_t ev0, ev1;
+};
+
+namespace {
+
+size_t links_elems(const stag_links *L, int rows)   // complex numbers in one gathered field
+{
+    return (size_t)2 * L->ntiles * 8 * (3 * rows) * TILE;
+}
+
+// ---- S0 kernels ----------------------------------------------------------------------
+
+// canonical W[mu][p][cb][3][3] (fp64, eta*bc folded) -> gathered fp64/18 field
+// L[p][tile][d][k][lane]; also measures how well row 2 is rebuilt from rows 0,1 (Q12).
+__global__ void __launch_bounds__(128)
+gather_links_kernel(double2 *__restrict__ L, const double *__restrict__ W, const Geom g,
+                    unsigned long long *__restrict__ err_bits)
+{
+    const long idx = blockIdx.x * 128L + threadIdx.x;
+    if (idx >= 2L * g.Vh_pad) return;
+    const int p = (int)(idx / g.Vh_pad);
+    const int cb = (int)(idx % g.Vh_pad);
+    double2 *dst = L + ((size_t)p * (g.Vh_pad / TILE) + (cb >> 5)) * (size_t)(8 * 9 * TILE) + (cb & 31);
+    if (cb >= g.Vh) {
+        for (int k = 0; k < 72; ++k) dst[k * TILE] = make_double2(0.0, 0.0);
+        return;
+    }
+    Site s;
+    decode_site(g, p, cb, s);
+    const unsigned neg = det_sign_mask(g, s);
+    double worst = 0.0;
+    for (int d = 0; d < 8; ++d) {
+        double2 m[9];
+        if (d < 4) {
+            const double *src = W + (((size_t)d * 2 + p) * g.Vh + cb) * 18;
+            for (int k = 0; k < 9; ++k) m[k] = make_double2(src[2 * k], src[2 * k + 1]);
+        } else {
+            const double *src = W + (((size_t)(d - 4) * 2 + (1 - p)) * g.Vh + s.nbr[d]) * 18;
+            for (int i = 0; i < 3; ++i)
+                for (int j = 0; j < 3; ++j)   // M = -W^dag : M_ij = -conj(W_ji)
+                    m[3 * i + j] = make_double2(-src[2 * (3 * j + i)], src[2 * (3 * j + i) + 1]);
+        }
+        for (int k = 0; k < 9; ++k) dst[(d * 9 + k) * TILE] = m[k];
+        double2 t[9];
+        for (int k = 0; k < 6; ++k) t[k] = m[k];
+        rebuild_row2<double>(t, (neg >> d) & 1u);
+        for (int j = 0; j < 3; ++j)
+            worst = fmax(worst, fmax(fabs(t[6 + j].x - m[6 + j].x), fabs(t[6 + j].y - m[6 + j].y)));
+    }
+    if (!(worst == worst)) worst = 1e300;
+    atomicMax(err_bits, (unsigned long long)__double_as_longlong(worst));   // worst >= 0
+}
+
+// fp64/18 gathered field -> another precision / row count
+template <typename TD, int ROWS>
+__global__ void __launch_bounds__(256)
+derive_links_kernel(cplx_t<TD> *__restrict__ dst, const double2 *__restrict__ src, long n_dst)
+{
+    constexpr int K = 3 * ROWS;
+    const long i = blockIdx.x * 256L + threadIdx.x;
+    if (i >= n_dst) return;
+    const int lane = (int)(i % TILE);
+    const long r = i / TILE;
+    const int k = (int)(r % K);
+    const long td = r / K;                     // (p*ntiles + tile)*8 + d
+    const double2 v = src[(td * 9 + k) * TILE + lane];
+    dst[i] = mk<TD>((TD)v.x, (TD)v.y);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128)
+spinor_pack_kernel(cplx_t<T> *__restrict__ dst, const double *__restrict__ src, int Vh, int Vh_pad)
+{
+    const int cb = blockIdx.x * 128 + threadIdx.x;
+    if (cb >= Vh_pad) return;
+    for (int c = 0; c < 3; ++c) {
+        cplx_t<T> v = mk<T>(0, 0);
+        if (cb < Vh) v = mk<T>((T)src[(size_t)cb * 6 + 2 * c], (T)src[(size_t)cb * 6 + 2 * c + 1]);
+        dst[(size_t)c * Vh_pad + cb] = v;
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128)
+spinor_unpack_kernel(double *__restrict__ dst, const cplx_t<T> *__restrict__ src, int Vh, int Vh_pad)
+{
+    const int cb = blockIdx.x * 128 + threadIdx.x;
+    if (cb >= Vh) return;
+    for (int c = 0; c < 3; ++c) {
+        const cplx_t<T> v = src[(size_t)c * Vh_pad + cb];
+        dst[(size_t)cb * 6 + 2 * c] = (double)v.x;
+        dst[(size_t)cb * 6 + 2 * c + 1] = (double)v.y;
+    }
+}
+
+// Build (once) the gathered field of precision `prec` from the fp64/18 one.
+int ensure_links(stag_links *L, int prec)
+{
+    if (L->L[prec]) return STAG_OK;
+    const int rows = prec_rows(prec);
+    if (rows == 2 && !(L->recon_err <= 1e-10)) {
+        snprintf(t_errbuf, sizeof(t_errbuf),
+                 "12-real links refused: row 2 is not s*conj(row0 x row1) (max error %.3g)", L->recon_err);
+        t_errbuf_status = STAG_EINVAL;
+        return STAG_EINVAL;
+    }
+    const size_t n = links_elems(L, rows);
+    const size_t bytes = n * (prec_is_f32(prec) ? sizeof(float2) : sizeof(double2));
+    void *dst = nullptr;
+    CU(cudaMalloc(&dst, bytes));
+    const unsigned grid = (unsigned)((n + 255) / 256);
+    const double2 *src = (const double2 *)L->L[STAG_PREC_F64];
+    switch (prec) {
+    case STAG_PREC_F32:     derive_links_kernel<float, 3><<<grid, 256, 0, t_stream>>>((float2 *)dst, src, (long)n); break;
+    case STAG_PREC_F64_R12: derive_links_kernel<double, 2><<<grid, 256, 0, t_stream>>>((double2 *)dst, src, (long)n); break;
+    case STAG_PREC_F32_R12: derive_links_kernel<float, 2><<<grid, 256, 0, t_stream>>>((float2 *)dst, src, (long)n); break;
+    default: cudaFree(dst); return STAG_EINVAL;
+    }
+    count_launch();
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { cudaFree(dst); return cuda_fail(e, "derive_links_kernel", __LINE__); }
+    L->L[prec] = dst;
+    return STAG_OK;
+}
+
+int ensure_tmp(stag_links *L, int f32)
+{
+    if (L->tmp_odd[f32]) return STAG_OK;
+    CU(cudaMalloc(&L->tmp_odd[f32], (size_t)3 * L->g.Vh_pad * (f32 ? sizeof(float2) : sizeof(double2))));
+    return STAG_OK;
+}
+
+// ---- Dslash launcher ---------------------------------------------------------------------
+template <typename T, int NR>
+int launch_hop_t(const stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx_t<T> *in,
+                 int parity, double m2, const cplx_t<T> *own, double *partials, CgCtrl *ctrl,
+                 cudaStream_t s)
+{
+    const Geom &g = L->g;
+    const cplx_t<T> *field = (const cplx_t<T> *)L->L[prec] + (size_t)parity * L->ntiles * 8 * (3 * NR) * TILE;
+    const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
+    switch (hop) {
+    case HOP_PLAIN:
+        dslash_kernel<T, NR, HOP_PLAIN><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)m2, own, partials, ctrl);
+        break;
+    case HOP_XPAY:
+        dslash_kernel<T, NR, HOP_XPAY><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)m2, own, partials, ctrl);
+        break;
+    default:
+        dslash_kernel<T, NR, HOP_XPAY_DOT><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)m2, own, partials, ctrl);
+        break;
+    }
+    count_launch();
+    KCHECK();
+    return STAG_OK;
+}
+
+int launch_hop(const stag_links *L, int prec, int hop, void *out, const void *in, int parity,
+               double m2, const void *own, double *partials, CgCtrl *ctrl, cudaStream_t s)
+{
+    switch (prec) {
+    case STAG_PREC_F64:
+        return launch_hop_t<double, 3>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, m2, (const double2 *)own, partials, ctrl, s);
+    case STAG_PREC_F32:
+        return launch_hop_t<float, 3>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, m2, (const float2 *)own, partials, ctrl, s);
+    case STAG_PREC_F64_R12:
+        return launch_hop_t<double, 2>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, m2, (const double2 *)own, partials, ctrl, s);
+    case STAG_PREC_F32_R12:
+        return launch_hop_t<float, 2>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, m2, (const float2 *)own, partials, ctrl, s);
+    }
+    return STAG_EINVAL;
+}
+
+bool same_dims(const stag_links *L, const int dims[4])
+{
+    return dims && dims[0] == L->dims[0] && dims[1] == L->dims[1] && dims[2] == L->dims[2] &&
+           dims[3] == L->dims[3];
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------
+// C ABI: state
+// ------------------------------------------------------------------------------------
+extern "C" int stag_set_stream(void *cuda_stream)
+{
+    t_stream = (cudaStream_t)cuda_stream;
+    return STAG_OK;
+}
+
+extern "C" const char *stag_strerror(int status)
+{
+    switch (status) {
+    case STAG_OK: return "ok";
+    case STAG_EINVAL: return (t_errbuf_status == STAG_EINVAL) ? t_errbuf : "invalid argument";
+    case STAG_ECUDA: return t_errbuf;
+    case STAG_ENOMEM: return (t_errbuf_status == STAG_ENOMEM) ? t_errbuf : "out of memory";
+    case STAG_ENOCONV: return "maxiter reached before the true residual met tol";
+    case STAG_EBREAKDOWN: return "CG breakdown (NaN or <d,Ad> <= 0)";
+    }
+    return "unknown status";
+}
+
+extern "C" unsigned long long stag_launch_count(void) { return g_launches.load(); }
+extern "C" void stag_reset_launch_count(void) { g_launches.store(0); }
+
+// ------------------------------------------------------------------------------------
+// C ABI: links
+// ------------------------------------------------------------------------------------
+extern "C" int stag_links_create(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
+                                 const double *W, int on_device)
+{
+    if (!links_out || !W) return STAG_EINVAL;
+    *links_out = nullptr;
+    Geom g;
+    if (!make_geom(g, dims, antiperiodic_t)) return STAG_EINVAL;
+    stag_links *L = new (std::nothrow) stag_links();
+    if (!L) return STAG_ENOMEM;
+    memset(L, 0, sizeof(*L));
+    L->g = g;
+    for (int m = 0; m < 4; ++m) L->dims[m] = dims[m];
+    L->ntiles = g.Vh_pad / TILE;
+
+    const size_t canon_bytes = (size_t)4 * 2 * g.Vh * 18 * sizeof(double);
+    double *Wd = nullptr;
+    unsigned long long *err = nullptr;
+    int rc = STAG_OK;
+    cudaError_t e;
+    do {
+        if (!on_device) {
+            if ((e = cudaMalloc(&Wd, canon_bytes)) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(staging)", __LINE__); break; }
+            if ((e = cudaMemcpyAsync(Wd, W, canon_bytes, cudaMemcpyHostToDevice, t_stream)) != cudaSuccess) { rc = cuda_fail(e, "cudaMemcpyAsync(W)", __LINE__); break; }
+        }
+        if ((e = cudaMalloc(&L->L[STAG_PREC_F64], links_elems(L, 3) * sizeof(double2))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(links)", __LINE__); break; }
+        if ((e = cudaMalloc(&err, sizeof(*err))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(err)", __LINE__); break; }
+        if ((e = cudaMemsetAsync(err, 0, sizeof(*err), t_stream)) != cudaSuccess) { rc = cuda_fail(e, "cudaMemsetAsync", __LINE__); break; }
+        const unsigned grid = (unsigned)((2L * g.Vh_pad + 127) / 128);
+        gather_links_kernel<<<grid, 128, 0, t_stream>>>((double2 *)L->L[STAG_PREC_F64], on_device ? W : Wd, g, err);
+        count_launch();
+        if ((e = cudaGetLastError()) != cudaSuccess) { rc = cuda_fail(e, "gather_links_kernel", __LINE__); break; }
+        unsigned long long bits = 0;
+        if ((e = cudaMemcpyAsync(&bits, err, sizeof(bits), cudaMemcpyDeviceToHost, t_stream)) != cudaSuccess) { rc = cuda_fail(e, "cudaMemcpyAsync(err)", __LINE__); break; }
+        if ((e = cudaStreamSynchronize(t_stream)) != cudaSuccess) { rc = cuda_fail(e, "cudaStreamSynchronize", __LINE__); break; }
+        memcpy(&L->recon_err, &bits, sizeof(double));
+        if ((e = cudaStreamCreateWithFlags(&L->cap_stream, cudaStreamNonBlocking)) != cudaSuccess) { rc = cuda_fail(e, "cudaStreamCreate", __LINE__); break; }
+        if ((e = cudaEventCreate(&L->ev0)) != cudaSuccess || (e = cudaEventCreate(&L->ev1)) != cudaSuccess) { rc = cuda_fail(e, "cudaEventCreate", __LINE__); break; }
+    } while (0);
+    if (Wd) cudaFree(Wd);
+    if (err) cudaFree(err);
+    if (rc != STAG_OK) { stag_links_destroy(L); return rc; }
+    *links_out = L;
+    return STAG_OK;
+}
+
+extern "C" void stag_links_destroy(stag_links_t *L)
+{
+    if (!L) return;
+    for (int i = 0; i < 4; ++i) if (L->L[i]) cudaFree(L->L[i]);
+    for (int i = 0; i < 2; ++i) if (L->tmp_odd[i]) cudaFree(L->tmp_odd[i]);
+    if (L->ws) cudaFree(L->ws);
+    if (L->h_ctrl) cudaFreeHost(L->h_ctrl);
+    if (L->stage_dev) cudaFree(L->stage_dev);
+    if (L->cap_stream) cudaStreamDestroy(L->cap_stream);
+    if (L->ev0) cudaEventDestroy(L->ev0);
+    if (L->ev1) cudaEventDestroy(L->ev1);
+    delete L;
+}
+
+extern "C" int stag_links_recon_error(const stag_links_t *L, double *err_out)
+{
+    if (!L || !err_out) return STAG_EINVAL;
+    *err_out = L->recon_err;
+    return STAG_OK;
+}
+
+// ------------------------------------------------------------------------------------
+// C ABI: spinors
+// ------------------------------------------------------------------------------------
+extern "C" size_t stag_spinor_bytes(const int dims[4], int prec)
+{
+    Geom g;
+    if (!prec_ok(prec) || !make_geom(g, dims, 0)) return 0;
+    return (size_t)3 * g.Vh_pad * (prec_is_f32(prec) ? sizeof(float2) : sizeof(double2));
+}
+
+extern "C" int stag_spinor_pack(void *dst, const double *src, const int dims[4], int prec)
+{
+    Geom g;
+    if (!dst || !src || !prec_ok(prec) || !make_geom(g, dims, 0)) return STAG_EINVAL;
+    const unsigned grid = (unsigned)((g.Vh_pad + 127) / 128);
+    if (prec_is_f32(prec)) spinor_pack_kernel<float><<<grid, 128, 0, t_stream>>>((float2 *)dst, src, g.Vh, g.Vh_pad);
+    else spinor_pack_kernel<double><<<grid, 128, 0, t_stream>>>((double2 *)dst, src, g.Vh, g.Vh_pad);
+    count_launch();
+    KCHECK();
+    return STAG_OK;
+}
+
+extern "C" int stag_spinor_unpack(double *dst, const void *src, const int dims[4], int prec)
+{
+    Geom g;
+    if (!dst || !src || !prec_ok(prec) || !make_geom(g, dims, 0)) return STAG_EINVAL;
+    const unsigned grid = (unsigned)((g.Vh + 127) / 128);
+    if (prec_is_f32(prec)) spinor_unpack_kernel<float><<<grid, 128, 0, t_stream>>>(dst, (const float2 *)src, g.Vh, g.Vh_pad);
+    else spinor_unpack_kernel<double><<<grid, 128, 0, t_stream>>>(dst, (const double2 *)src, g.Vh, g.Vh_pad);
+    count_launch();
+    KCHECK();
+    return STAG_OK;
+}
+
+// ------------------------------------------------------------------------------------
+// C ABI: the operator
+// ------------------------------------------------------------------------------------
+extern "C" int stag_dslash(void *out, const void *in, const stag_links_t *links, int parity,
+                           const int dims[4], int prec)
+{
+    stag_links *L = const_cast<stag_links *>(links);
+    if (!out || !in || !L || out == in || (parity & ~1) || !prec_ok(prec) || !same_dims(L, dims))
+        return STAG_EINVAL;
+    int rc = ensure_links(L, prec);
+    if (rc) return rc;
+    return launch_hop(L, prec, HOP_PLAIN, out, in, parity, 0.0, nullptr, nullptr, nullptr, t_stream);
+}
+
+extern "C" int stag_apply_A(void *out_even, const void *in_even, const stag_links_t *links,
+                            double mass, int prec)
+{
+    stag_links *L = const_cast<stag_links *>(links);
+    if (!out_even || !in_even || !L || out_even == in_even || !prec_ok(prec)) return STAG_EINVAL;
+    int rc = ensure_links(L, prec);
+    if (rc) return rc;
+    const int f32 = prec_is_f32(prec) ? 1 : 0;
+    if ((rc = ensure_tmp(L, f32))) return rc;
+    // tmp_o = D_oe in_e ;  out_e = m^2 in_e - D_eo tmp_o      (eq. 2.3)
+    if ((rc = launch_hop(L, prec, HOP_PLAIN, L->tmp_odd[f32], in_even, 1, 0.0, nullptr, nullptr, nullptr, t_stream))) return rc;
+    return launch_hop(L, prec, HOP_XPAY, out_even, L->tmp_odd[f32], 0, mass * mass, in_even, nullptr, nullptr, t_stream);
+}
+
+// ------------------------------------------------------------------------------------
+// the CG drivers
+// ------------------------------------------------------------------------------------
+namespace {
+
+struct Workspace {
+    CgCtrl *ctrl;
+    double *partials;
+    double *r64, *q64, *tmp64, *d64;
+    float *y32, *r32, *d32, *q32, *tmp32;
+};
+
+int ensure_workspace(stag_links *L, Workspace &w)
+{
+    const size_t n = (size_t)6 * L->g.Vh_pad;
+    const size_t nb64 = align_up(n * sizeof(double), 256), nb32 = align_up(n * sizeof(float), 256);
+    const size_t npart = (size_t)L->g.Vh_pad / DSLASH_BLOCK + 1 + (size_t)blas_grid((long)n);
+    const size_t pb = align_up(npart * sizeof(double), 256);
+    const size_t total = 256 + pb + 4 * nb64 + 5 * nb32;
+    if (!L->ws) {
+        CU(cudaMalloc((void **)&L->ws, total));
+        L->ws_bytes = total;
+        CU(cudaMallocHost((void **)&L->h_ctrl, sizeof(CgCtrl)));
+    }
+    char *p = L->ws;
+    w.ctrl = (CgCtrl *)p; p += 256;
+    w.partials = (double *)p; p += pb;
+    w.r64 = (double *)p; p += nb64;
+    w.q64 = (double *)p; p += nb64;
+    w.tmp64 = (double *)p; p += nb64;
+    w.d64 = (double *)p; p += nb64;
+    w.y32 = (float *)p; p += nb32;
+    w.r32 = (float *)p; p += nb32;
+    w.d32 = (float *)p; p += nb32;
+    w.q32 = (float *)p; p += nb32;
+    w.tmp32 = (float *)p; p += nb32;
+    return STAG_OK;
+}
+
+static_assert(sizeof(CgCtrl) <= 256, "CgCtrl must fit its workspace slot");
+
+struct Solver {
+    stag_links *L;
+    Workspace w;
+    cudaStream_t s;
+    double m2;
+    int mode;
+    int prec_lo;     // precision enum of the iteration's Dslash
+    int prec_hi;     // precision enum of the fp64 corrections
+    long n;          // reals per spinor
+    int gb;          // blas grid
+    int applies_f64;
+
+    // q64 = A x  in fp64 (two hops), outside the iteration
+    int apply_A64(const double *x)
+    {
+        int rc = launch_hop(L, prec_hi, HOP_PLAIN, w.tmp64, x, 1, 0.0, nullptr, nullptr, nullptr, s);
+        if (rc) return rc;
+        ++applies_f64;
+        return launch_hop(L, prec_hi, HOP_XPAY, w.q64, w.tmp64, 0, m2, x, nullptr, nullptr, s);
+    }
+
+    template <int WHAT>
+    int residual(const double *b, bool lo_copy)
+    {
+        residual_kernel<float, WHAT><<<gb, BLAS_BLOCK, 0, s>>>(w.r64, b, w.q64, lo_copy ? w.r32 : nullptr, n, w.partials, w.ctrl);
+        count_launch();
+        KCHECK();
+        return STAG_OK;
+    }
+
+    int accumulate(double *x)
+    {
+        accumulate_kernel<float><<<gb, BLAS_BLOCK, 0, s>>>(x, w.y32, n);
+        count_launch();
+        KCHECK();
+        return STAG_OK;
+    }
+
+    // one pass of the loop body of Fig. 1, four launches
+    template <typename T>
+    int iteration(T *y, T *r, T *d, T *q, T *tmp, cudaStream_t st)
+    {
+        xpay_kernel<T><<<gb, BLAS_BLOCK, 0, st>>>(d, r, n, w.ctrl);                          // d = r + beta d
+        count_launch();
+        KCHECK();
+        int rc = launch_hop(L, prec_lo, HOP_PLAIN, tmp, d, 1, 0.0, nullptr, nullptr, w.ctrl, st);   // D_oe d
+        if (rc) return rc;
+        rc = launch_hop(L, prec_lo, HOP_XPAY_DOT, q, tmp, 0, m2, d, w.partials, w.ctrl, st);  // q = A d, alpha
+        if (rc) return rc;
+        update_kernel<T><<<gb, BLAS_BLOCK, 0, st>>>(y, r, d, q, n, w.partials, w.ctrl);      // y, r, delta, beta
+        count_launch();
+        KCHECK();
+        return STAG_OK;
+    }
+
+    int iteration_mode(double *x, cudaStream_t st)
+    {
+        if (mode == STAG_CG_F64) return iteration<double>(x, w.r64, w.d64, w.q64, w.tmp64, st);
+        return iteration<float>(w.y32, w.r32, w.d32, w.q32, w.tmp32, st);
+    }
+
+    int read_ctrl()
+    {
+        CU(cudaMemcpyAsync(L->h_ctrl, w.ctrl, sizeof(CgCtrl), cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+        return STAG_OK;
+    }
+};
+
+int cg_solve_device(double *x, const double *b, stag_links *L, double mass, double tol, int maxiter,
+                    int mode, const stag_cg_params_t *prm, stag_cg_stats_t *stats)
+{
+    stag_cg_params_t P;
+    memset(&P, 0, sizeof(P));
+    if (prm) P = *prm;
+    if (!(P.eps_in > 0.0)) P.eps_in = (mode == STAG_CG_DEFECT) ? 1e-2 : 0.1;
+    if (P.graph_chunk == 0) P.graph_chunk = 32;
+
+    Solver S;
+    S.L = L;
+    S.s = t_stream;
+    S.m2 = mass * mass;
+    S.mode = mode;
+    S.prec_lo = (mode == STAG_CG_F64) ? (P.recon12 ? STAG_PREC_F64_R12 : STAG_PREC_F64)
+                                       : (P.recon12 ? STAG_PREC_F32_R12 : STAG_PREC_F32);
+    S.prec_hi = P.recon12_f64 ? STAG_PREC_F64_R12 : STAG_PREC_F64;
+    S.n = (long)6 * L->g.Vh_pad;
+    S.gb = blas_grid(S.n);
+    S.applies_f64 = 0;
+    int rc;
+    if ((rc = ensure_links(L, S.prec_lo))) return rc;
+    if ((rc = ensure_links(L, S.prec_hi))) return rc;
+    if ((rc = ensure_workspace(L, S.w))) return rc;
+    Workspace &w = S.w;
+    cudaStream_t s = S.s;
+    const bool lo = (mode != STAG_CG_F64);
+
+    CU(cudaEventRecord(L->ev0, s));
+
+    // ---- |b|^2 and the solver scalars ---------------------------------------------------
+    CgCtrl *h = L->h_ctrl;
+    memset(h, 0, sizeof(*h));
+    h->mode = mode;
+    h->maxiter = maxiter;
+    h->eps_in = P.eps_in;
+    CU(cudaMemcpyAsync(w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, s));
+    residual_kernel<float, RES_NORM><<<S.gb, BLAS_BLOCK, 0, s>>>(nullptr, b, nullptr, nullptr, S.n, w.partials, w.ctrl);
+    count_launch();
+    KCHECK();
+    if ((rc = S.read_ctrl())) return rc;
+    const double bnorm2 = h->bnorm2;
+
+    stag_cg_stats_t st;
+    memset(&st, 0, sizeof(st));
+    if (bnorm2 == 0.0) {   // b = 0  =>  x = 0, nothing to iterate
+        CU(cudaMemsetAsync(x, 0, (size_t)S.n * sizeof(double), s));
+        CU(cudaEventRecord(L->ev1, s));
+        CU(cudaStreamSynchronize(s));
+        if (stats) *stats = st;
+        return STAG_OK;
+    }
+    if (!(bnorm2 == bnorm2) || std::isinf(bnorm2)) {
+        if (stats) { st.true_resid = NAN; *stats = st; }
+        return STAG_EBREAKDOWN;
+    }
+    h->tol2b = tol * tol * bnorm2;
+    CU(cudaMemcpyAsync(w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, s));
+
+    // ---- r = b - A x0 (P:L46 / Fig. 2), in fp64 -------------------------------------
+    if ((rc = S.apply_A64(x))) return rc;
+    if ((rc = S.residual<RES_INIT>(b, lo))) return rc;
+    if (lo) CU(cudaMemsetAsync(w.y32, 0, (size_t)S.n * sizeof(float), s));
+    // beta = 0 makes the first xpay d = r without reading d, so d needs no initial value
+
+    // ---- the iteration as a CUDA graph of `chunk` passes ----------------------------------
+    const int chunk = P.graph_chunk;
+    cudaGraphExec_t gexec = nullptr;
+    unsigned long long graph_nodes = 0;
+    if (chunk > 0) {
+        cudaGraph_t graph = nullptr;
+        cudaError_t e = cudaStreamBeginCapture(L->cap_stream, cudaStreamCaptureModeThreadLocal);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaStreamBeginCapture", __LINE__);
+        t_capturing = true;
+        t_captured_nodes = 0;
+        rc = STAG_OK;
+        for (int i = 0; i < chunk && rc == STAG_OK; ++i) rc = S.iteration_mode(x, L->cap_stream);
+        t_capturing = false;
+        graph_nodes = t_captured_nodes;
+        e = cudaStreamEndCapture(L->cap_stream, &graph);
+        if (rc != STAG_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture", __LINE__);
+        e = cudaGraphInstantiate(&gexec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaGraphInstantiate", __LINE__);
+    }
+    struct GraphGuard { cudaGraphExec_t g; ~GraphGuard() { if (g) cudaGraphExecDestroy(g); } } guard{gexec};
+
+    int n_restarts = 0, n_outer = 0;
+    int final_state = CG_RUN;
+    bool have_true = true;      // ctrl->sum0 holds |b - A x|^2 for the current x
+    bool verifying = false;     // mode 0: the last launch was the true-residual check of Q6b
+    for (;;) {
+        if ((rc = S.read_ctrl())) return rc;
+        const int state = h->state;
+        if (state == CG_RUN) {
+            if (verifying) ++n_restarts;
+            verifying = false;
+            if (gexec) {
+                CU(cudaGraphLaunch(gexec, s));
+                count_launch(graph_nodes);
+            } else {
+                for (int i = 0; i < 8; ++i) if ((rc = S.iteration_mode(x, s))) return rc;
+            }
+            have_true = false;
+            continue;
+        }
+        if (state == CG_UPDATE) {                      // section 3.2: mode 3 only
+            if ((rc = S.accumulate(x))) return rc;                 // x += y ; y = 0
+            if ((rc = S.apply_A64(x))) return rc;
+            if ((rc = S.residual<RES_UPDATE>(b, true))) return rc; // r = b - A x -> r32, beta
+            have_true = true;
+            continue;
+        }
+        if (state == CG_CONVERGED && !have_true) {
+            if (mode == STAG_CG_F64) {                 // Q6b: verify on the true residual
+                if ((rc = S.apply_A64(x))) return rc;
+                if ((rc = S.residual<RES_INIT>(b, false))) return rc;
+                have_true = true;
+                verifying = true;
+                continue;
+            }
+            if (mode == STAG_CG_DEFECT) {              // Fig. 2 outer step
+                if ((rc = S.accumulate(x))) return rc;
+                if ((rc = S.apply_A64(x))) return rc;
+                if ((rc = S.residual<RES_INIT>(b, true))) return rc;
+                have_true = true;
+                ++n_outer;
+                continue;
+            }
+            if (mode == STAG_CG_F32) {
+                if ((rc = S.accumulate(x))) return rc;
+                if ((rc = S.apply_A64(x))) return rc;
+                if ((rc = S.residual<RES_FINAL>(b, false))) return rc;
+                have_true = true;
+                final_state = CG_CONVERGED;
+                if ((rc = S.read_ctrl())) return rc;
+                break;
+            }
+        }
+        if (state == CG_CONVERGED) { final_state = CG_CONVERGED; break; }
+        // CG_MAXITER or CG_BREAKDOWN: fold y into x, report the true residual
+        final_state = state;
+        if (!have_true) {
+            if (lo && (rc = S.accumulate(x))) return rc;
+            if ((rc = S.apply_A64(x))) return rc;
+            if ((rc = S.residual<RES_FINAL>(b, false))) return rc;
+            if ((rc = S.read_ctrl())) return rc;
+        }
+        break;
+    }
+    CU(cudaEventRecord(L->ev1, s));
+    CU(cudaStreamSynchronize(s));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, L->ev0, L->ev1));
+
+    st.iters = h->iter;
+    st.n_updates = (mode == STAG_CG_DEFECT) ? n_outer : h->n_updates;
+    st.n_restarts = n_restarts;
+    st.iters_f32 = lo ? h->iter : 0;
+    st.applies_f64 = S.applies_f64;
+    st.true_resid = sqrt(h->sum0 / bnorm2);
+    st.iter_resid = sqrt(h->sum1 / bnorm2);
+    st.seconds = ms * 1e-3;
+    if (stats) *stats = st;
+    if (final_state == CG_BREAKDOWN) return STAG_EBREAKDOWN;
+    if (!(st.true_resid <= tol)) return STAG_ENOCONV;
+    return STAG_OK;
+}
+
+}  // namespace
+
+extern "C" int stag_cg_solve_ex(void *x_even, const void *b_even, const stag_links_t *links,
+                                double mass, double tol, int maxiter, int mode,
+                                const stag_cg_params_t *params, stag_cg_stats_t *stats_out)
+{
+    stag_links *L = const_cast<stag_links *>(links);
+    if (!x_even || !b_even || !L || x_even == b_even || !(tol > 0.0) || maxiter < 0 || mode < 0 ||
+        mode > 3)
+        return STAG_EINVAL;
+    return cg_solve_device((double *)x_even, (const double *)b_even, L, mass, tol, maxiter, mode,
+                           params, stats_out);
+}
+
+extern "C" int stag_cg_solve(void *x_even, const void *b_even, const stag_links_t *links,
+                             double mass, double tol, int maxiter, int mode, int *iters_out,
+                             double *true_resid_out)
+{
+    stag_cg_stats_t st;
+    memset(&st, 0, sizeof(st));
+    int rc = stag_cg_solve_ex(x_even, b_even, links, mass, tol, maxiter, mode, nullptr, &st);
+    if (rc < 0) return rc;
+    if (iters_out) *iters_out = st.iters;
+    if (true_resid_out) *true_resid_out = st.true_resid;
+    return rc;
+}
+
+extern "C" int stag_cg_solve_host(double *x_host, const double *b_host, const stag_links_t *links,
+                                  double mass, double tol, int maxiter, int mode,
+                                  const stag_cg_params_t *params, stag_cg_stats_t *stats_out)
+{
+    stag_links *L = const_cast<stag_links *>(links);
+    if (!x_host || !b_host || !L || x_host == b_host) return STAG_EINVAL;
+    const size_t nc = (size_t)L->g.Vh * 6;         // canonical doubles
+    const size_t nd = (size_t)L->g.Vh_pad * 6;     // device-layout doubles
+    if (!L->stage_dev) CU(cudaMalloc((void **)&L->stage_dev, (2 * nc + 2 * nd) * sizeof(double)));
+    double *cx = L->stage_dev, *cb = cx + nc, *dx = cb + nc, *db = dx + nd;
+    CU(cudaMemcpyAsync(cb, b_host, nc * sizeof(double), cudaMemcpyHostToDevice, t_stream));
+    CU(cudaMemcpyAsync(cx, x_host, nc * sizeof(double), cudaMemcpyHostToDevice, t_stream));
+    int rc;
+    if ((rc = stag_spinor_pack(db, cb, L->dims, STAG_PREC_F64))) return rc;
+    if ((rc = stag_spinor_pack(dx, cx, L->dims, STAG_PREC_F64))) return rc;
+    const int solve_rc = stag_cg_solve_ex(dx, db, L, mass, tol, maxiter, mode, params, stats_out);
+    if (solve_rc < 0) return solve_rc;
+    if ((rc = stag_spinor_unpack(cx, dx, L->dims, STAG_PREC_F64))) return rc;
+    CU(cudaMemcpyAsync(x_host, cx, nc * sizeof(double), cudaMemcpyDeviceToHost, t_stream));
+    CU(cudaStreamSynchronize(t_stream));
+    return solve_rc;
+}

@@ -1,0 +1,164 @@
+"""GPU parity of the Dslash hop and of A against the CPU oracle, element by element, through
+the C ABI (include/stag.h).  Tolerances are BASELINE.json's: relative L2 error <= 1e-13 in
+fp64 and <= 2e-6 in fp32 (the same bars for the 12-real variants)."""
+import numpy as np
+import pytest
+
+import fieldgen
+import oracle
+import paper_1111_0125_b200 as stag
+
+pytestmark = pytest.mark.gpu
+
+TOL = {stag.PREC_F64: 1e-13, stag.PREC_F64_R12: 1e-13, stag.PREC_F32: 2e-6, stag.PREC_F32_R12: 2e-6}
+ALL_PREC = [stag.PREC_F64, stag.PREC_F32, stag.PREC_F64_R12, stag.PREC_F32_R12]
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
+
+
+# several tiles + ragged tails (Vh not a multiple of 32 or of the 128-thread block), extents of
+# 2 (forward and backward neighbour coincide), and the small BASELINE configs
+DIMS = [(4, 4, 4, 4), (2, 2, 2, 2), (6, 4, 2, 10), (2, 6, 6, 4), (8, 8, 8, 8), (10, 6, 4, 6), (4, 2, 2, 2)]
+
+
+@pytest.mark.parametrize("dims", DIMS)
+@pytest.mark.parametrize("prec", ALL_PREC)
+@pytest.mark.parametrize("parity", [0, 1])
+def test_dslash_matches_oracle(dims, prec, parity):
+    W = fieldgen.links(dims, "random", seed=11)
+    chi = fieldgen.spinor_gaussian(dims, 1 - parity, seed=12)
+    ref = oracle.dslash(chi, W, dims, parity)
+    L = stag.Links(dims, W)
+    out = stag.spinor_unpack(stag.dslash(stag.spinor_pack(chi, dims, prec), L, parity, prec), dims, prec)
+    assert rel_l2(out, ref) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ALL_PREC)
+def test_dslash_periodic_time_boundary(prec):
+    """antiperiodic_t = 0: the 12-real sign rebuild must not assume a boundary sign."""
+    dims = (4, 4, 2, 6)
+    W = fieldgen.links(dims, "random", seed=5, antiperiodic_t=False)
+    chi = fieldgen.spinor_gaussian(dims, 0, seed=6)
+    L = stag.Links(dims, W, antiperiodic_t=False)
+    out = stag.spinor_unpack(stag.dslash(stag.spinor_pack(chi, dims, prec), L, 1, prec), dims, prec)
+    assert rel_l2(out, oracle.dslash(chi, W, dims, 1)) <= TOL[prec]
+
+
+def test_pack_unpack_roundtrip_and_pad_is_zero():
+    dims = (6, 4, 2, 10)          # Vh = 240, Vh_pad = 256
+    chi = fieldgen.spinor_gaussian(dims, 0, seed=3)
+    v = stag.spinor_pack(chi, dims, stag.PREC_F64)
+    assert v.numel() == 6 * 256
+    planes = v.view(3, 256, 2)
+    assert float(planes[:, 240:, :].abs().max()) == 0.0
+    assert np.array_equal(stag.spinor_unpack(v, dims, stag.PREC_F64), chi)
+    v32 = stag.spinor_pack(chi, dims, stag.PREC_F32)
+    assert np.array_equal(stag.spinor_unpack(v32, dims, stag.PREC_F32), chi.astype(np.complex64).astype(np.complex128))
+
+
+def test_dslash_keeps_pad_lanes_zero():
+    dims = (6, 4, 2, 10)
+    W = fieldgen.links(dims, "random", seed=1)
+    chi = fieldgen.spinor_gaussian(dims, 0, seed=2)
+    L = stag.Links(dims, W)
+    for prec in ALL_PREC:
+        out = stag.empty_spinor(dims, prec)
+        out.fill_(float("nan"))
+        stag.dslash(stag.spinor_pack(chi, dims, prec), L, 1, prec, out=out)
+        assert float(out.view(3, 256, 2)[:, 240:, :].abs().max()) == 0.0
+
+
+def test_twelve_real_links_refused_when_not_special_unitary():
+    dims = (4, 4, 4, 4)
+    rng = np.random.default_rng(0)
+    W = rng.normal(size=(4, 2, 128, 3, 3)) + 1j * rng.normal(size=(4, 2, 128, 3, 3))
+    chi = fieldgen.spinor_gaussian(dims, 0, seed=2)
+    L = stag.Links(dims, W)
+    assert L.recon_error() > 1e-3
+    out = stag.spinor_unpack(stag.dslash(stag.spinor_pack(chi, dims, stag.PREC_F64), L, 1, stag.PREC_F64), dims, stag.PREC_F64)
+    assert rel_l2(out, oracle.dslash(chi, W, dims, 1)) <= 1e-13   # 18-real works for any W
+    with pytest.raises(stag.StagError) as e:
+        stag.dslash(stag.spinor_pack(chi, dims, stag.PREC_F32_R12), L, 1, stag.PREC_F32_R12)
+    assert e.value.status == stag.EINVAL
+
+
+def test_recon_error_is_rounding_for_folded_su3_links():
+    dims = (4, 6, 4, 8)
+    for kind, eps in (("random", 0.0), ("smooth", 0.5), ("unit", 0.0)):
+        L = stag.Links(dims, fieldgen.links(dims, kind, seed=9, eps=eps))
+        assert L.recon_error() < 1e-14
+
+
+def test_links_from_device_memory_match_links_from_host():
+    import torch
+    dims = (4, 4, 6, 4)
+    W = fieldgen.links(dims, "random", seed=21)
+    chi = fieldgen.spinor_gaussian(dims, 0, seed=22)
+    Wd = torch.from_numpy(W.view(np.float64).reshape(-1)).cuda()
+    a = stag.dslash(stag.spinor_pack(chi, dims, stag.PREC_F64), stag.Links(dims, W), 1, stag.PREC_F64)
+    b = stag.dslash(stag.spinor_pack(chi, dims, stag.PREC_F64), stag.Links(dims, Wd), 1, stag.PREC_F64)
+    assert torch.equal(a, b)
+
+
+def test_argument_errors_on_device():
+    dims = (4, 4, 4, 4)
+    L = stag.Links(dims, fieldgen.links(dims, "random", seed=1))
+    v = stag.spinor_pack(fieldgen.spinor_gaussian(dims, 0, seed=2), dims, stag.PREC_F64)
+    with pytest.raises(stag.StagError):
+        stag.dslash(v, L, 1, stag.PREC_F64, out=v)            # out aliases in
+    with pytest.raises(stag.StagError):
+        stag.dslash(v, L, 2, stag.PREC_F64)                   # bad parity
+    with pytest.raises(stag.StagError):
+        stag.dslash(v, L, 1, 9)                               # bad precision
+    L2 = stag.Links((4, 4, 4, 6), fieldgen.links((4, 4, 4, 6), "random", seed=1))
+    import ctypes
+    out = stag.empty_spinor(dims, stag.PREC_F64)
+    rc = stag.lib().stag_dslash(ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(v.data_ptr()),
+                                L2.handle, 1, (ctypes.c_int * 4)(*dims), 0)
+    assert rc == stag.EINVAL                                  # dims != the handle's
+
+
+@pytest.mark.parametrize("name", ["c1_4^4", "c2_8^4_free", "c2_8^4", "c3_16^3x32"])
+@pytest.mark.parametrize("prec", ALL_PREC)
+def test_apply_A_matches_oracle_on_baseline_configs(name, prec):
+    cfg = fieldgen.CONFIGS[name]
+    W, b = cfg.links(), cfg.source()
+    ref = oracle.apply_A(b, W, cfg.dims, cfg.mass)
+    L = stag.Links(cfg.dims, W)
+    out = stag.spinor_unpack(stag.apply_A(stag.spinor_pack(b, cfg.dims, prec), L, cfg.mass, prec), cfg.dims, prec)
+    assert rel_l2(out, ref) <= TOL[prec]
+
+
+def test_free_field_plane_wave_eigenvalue_on_gpu():
+    """BASELINE configs[1]: A chi = (m^2 + 4 sum sin^2 p_mu) chi for plane waves on U = 1."""
+    dims, m = (8, 8, 8, 8), 0.05
+    W = fieldgen.links(dims, "unit")
+    L = stag.Links(dims, W)
+    for n in [(0, 0, 0, 0), (1, 2, 3, 0), (3, 1, 0, 5)]:
+        chi = fieldgen.spinor_planewave(dims, n)
+        p = [2 * np.pi * (n[mu] + (0.5 if mu == 3 else 0.0)) / dims[mu] for mu in range(4)]
+        lam = m * m + 4 * sum(np.sin(pm) ** 2 for pm in p)
+        out = stag.spinor_unpack(stag.apply_A(stag.spinor_pack(chi, dims, 0), L, m, 0), dims, 0)
+        assert rel_l2(out, lam * chi) <= 1e-13
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("name", ["c4_28^3x96", "c5_48^3x96"])
+def test_dslash_full_size_matches_oracle(name):
+    """The bench configuration (and the largest one): all four precisions, both hops, every
+    output site compared with the oracle's hop on the same seeded field."""
+    cfg = fieldgen.CONFIGS[name]
+    W = cfg.links()
+    chi = cfg.source()
+    L = stag.Links(cfg.dims, W)
+    ref1 = oracle.dslash(chi, W, cfg.dims, 1)
+    ref0 = oracle.dslash(ref1, W, cfg.dims, 0)
+    del W
+    for prec in ALL_PREC:
+        o1 = stag.spinor_unpack(stag.dslash(stag.spinor_pack(chi, cfg.dims, prec), L, 1, prec), cfg.dims, prec)
+        assert rel_l2(o1, ref1) <= TOL[prec]
+        o0 = stag.spinor_unpack(stag.dslash(stag.spinor_pack(ref1, cfg.dims, prec), L, 0, prec), cfg.dims, prec)
+        assert rel_l2(o0, ref0) <= TOL[prec]
+    L.close()
