@@ -111,7 +111,7 @@ def test_argument_errors_on_device():
     with pytest.raises(stag.StagError):
         stag.dslash(v, L, 2, stag.PREC_F64)                   # bad parity
     with pytest.raises(stag.StagError):
-        stag.dslash(v, L, 1, 9)                               # bad precision
+        stag.dslash(v, L, 1, 9, out=stag.empty_spinor(dims, 0))  # bad precision
     L2 = stag.Links((4, 4, 4, 6), fieldgen.links((4, 4, 4, 6), "random", seed=1))
     import ctypes
     out = stag.empty_spinor(dims, stag.PREC_F64)
