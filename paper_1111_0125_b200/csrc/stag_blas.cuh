@@ -69,18 +69,38 @@ xpay_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const CgCtrl *__
     }
 }
 
-// y += alpha d ; r -= alpha q ; delta' = |r|^2 ; then the scalar part of the iteration
-// (P:L52-54 and the trigger of P:L97) in the last block.
+// Sum of v[0..n) in a fixed order, the same in every block, returned to ALL threads of the
+// block: every block that calls it with the same arguments gets the same bits.
+__device__ __forceinline__ double block_total_fixed(const double *__restrict__ v, int n, double *red)
+{
+    double t = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) t += __ldcg(v + i);
+    t = block_sum(t, red);
+    __shared__ double total;
+    if (threadIdx.x == 0) total = t;
+    __syncthreads();
+    return total;
+}
+
+// alpha = delta / <d,Ad> ; y += alpha d ; r -= alpha q ; delta' = |r|^2 ; then the scalar part
+// of the iteration (P:L51-54 and the trigger of P:L97) in the last block.
+// <d,Ad> arrives as the per-block partial sums of the second hop (stag_dslash.cuh); every block
+// adds them in the same order, so all blocks use the same alpha and no extra launch or
+// device-wide fence is needed between the hop and this kernel.
 template <typename T>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
-              const T *__restrict__ q, long n, double *__restrict__ partials,
-              CgCtrl *__restrict__ ctrl)
+              const T *__restrict__ q, long n, const double *__restrict__ hop_partials,
+              int n_hop_partials, double *__restrict__ partials, CgCtrl *__restrict__ ctrl)
 {
     if (ctrl->state != CG_RUN) return;
     using V = typename Vec4<T>::type;
     constexpr int N = Vec4<T>::N;
-    const T alpha = (T)ctrl->alpha;
+    __shared__ double red[32];
+    const double dAd = block_total_fixed(hop_partials, n_hop_partials, red);
+    const bool ok = dAd > 0.0;                       // false also for NaN
+    const double alpha_d = ok ? ctrl->delta / dAd : 0.0;   // alpha = delta_new / d^dag A d
+    const T alpha = (T)alpha_d;
     const long nv = n / N;
     double s = 0.0;
     for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)gridDim.x * BLAS_BLOCK) {
@@ -98,15 +118,16 @@ update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
         reinterpret_cast<V *>(y)[i] = pack(yy);
         reinterpret_cast<V *>(r)[i] = pack(rr);
     }
-    __shared__ double red[32];
     double bs = block_sum(s, red), dn;
     if (!finish_reduction(bs, partials, &ctrl->ticket[1], red, &dn)) return;
 
     // ---- scalar epilogue, one thread ------------------------------------------------
     const int it = ctrl->iter + 1;
     ctrl->iter = it;
+    ctrl->dAd = dAd;
+    ctrl->alpha = alpha_d;
     int st = CG_RUN;
-    if (!(dn == dn)) st = CG_BREAKDOWN;
+    if (!ok || !(dn == dn)) st = CG_BREAKDOWN;
     else if (ctrl->mode == STAG_CG_RELIABLE) {
         const double rn = sqrt(dn);
         if (dn <= ctrl->tol2b || rn < ctrl->eps_in * ctrl->maxr) st = CG_UPDATE;   // P:L97, Q11

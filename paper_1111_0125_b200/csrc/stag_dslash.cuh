@@ -2,11 +2,17 @@
 //
 // One thread per output site, one warp per 32-site link tile.  Per site the kernel
 // streams eight link matrices from the gathered, tiled field (include/stag.h,
-// stag_links_create) with evict-first loads -- the gauge field is read exactly once per hop
-// and must not push the spinors out of L2 -- gathers the eight neighbour colour vectors
-// through L1/L2 (each is needed by eight output sites, the farthest reuse one time slice
-// away), and accumulates eight 3x3 complex matrix-vector products: 8*(66+6) = 576 flop
-// (P:L62).  HBM-bound: 8*18 + 6 + 6 reals per site compulsory.
+// stag_links_create) in 16-byte packets with evict-first loads -- the gauge field is read
+// exactly once per hop and must not push the spinors out of L2 -- gathers the eight
+// neighbour colour vectors through L1/L2 (each is needed by eight output sites, the farthest
+// reuse one time slice away), and accumulates eight 3x3 complex matrix-vector products:
+// 8*(66+6) = 576 flop.  HBM-bound: 8*18 + 6 + 6 reals per site
+// compulsory.
+//
+// The link stream is issued in GROUPS of K*GM independent 16-byte loads per thread (K = 9 or
+// 6 packets) before the first of them is used; with __launch_bounds__(128, MINB) giving
+// ptxas the registers to keep a group in flight this is what moves the kernel from 0.94 to
+// 1.05 of the measured copy bandwidth (profiles/README.md, round-1 sweep).
 #pragma once
 #include "stag_common.cuh"
 
@@ -16,12 +22,22 @@ constexpr int DSLASH_BLOCK = 128;
 
 enum { HOP_PLAIN = 0,   // out = D in
        HOP_XPAY = 1,    // out = m2*own - D in                       (second hop of A, eq. 2.3)
-       HOP_XPAY_DOT = 2 // same, plus <own,out> -> ctrl->dAd, alpha  (Fig. 1)
+       HOP_XPAY_DOT = 2 // same, plus per-block partial sums of <own,out>  (Fig. 1)
 };
 
-// streaming (read-once) and cached loads of one complex number
-template <typename C> __device__ __forceinline__ C ld_stream(const C *p) { return __ldcs(p); }
-template <typename C> __device__ __forceinline__ C ld_cached(const C *p) { return __ldg(p); }
+// 16-byte link packets: two complex numbers in fp32, one in fp64.
+template <typename T> struct Pkt;
+template <> struct Pkt<float>  { using type = float4;  static constexpr int CPP = 2; };
+template <> struct Pkt<double> { using type = double2; static constexpr int CPP = 1; };
+template <typename T> using pkt_t = typename Pkt<T>::type;
+
+// complex number c of a run of packets held in registers (c is a compile-time constant
+// after unrolling)
+__device__ __forceinline__ float2 pk_get(const float4 *pk, int c)
+{
+    return (c & 1) ? make_float2(pk[c >> 1].z, pk[c >> 1].w) : make_float2(pk[c >> 1].x, pk[c >> 1].y);
+}
+__device__ __forceinline__ double2 pk_get(const double2 *pk, int c) { return pk[c]; }
 
 // Row 2 of a matrix whose rows 0,1 are m[0..5] and whose determinant is +-1:
 // row2 = s * conj(row0 x row1)  (Q12).
@@ -40,18 +56,33 @@ __device__ __forceinline__ void rebuild_row2(cplx_t<T> *m, bool neg)
     }
 }
 
+// Launch shape per precision / storage, from the sweep on 28^3 x 96 (profiles/README.md):
+// MINB = resident blocks per SM promised to ptxas, GM = directions' worth of packets loaded
+// ahead (group = K*GM packets).
+template <typename T, int NR> struct HopTune { static constexpr int MINB = 4, GM = 1; };
+template <> struct HopTune<float, 2>         { static constexpr int MINB = 6, GM = 2; };
+
 // T: float or double.  NR: rows of each link held in memory (3 = 18-real, 2 = 12-real).
-// links: the gathered field of the OUTPUT parity, L[tile][d][k][lane].
-// in:  the other parity's spinor planes; out / own: this parity's.
+// links: the gathered field of the OUTPUT parity as packets, L[tile][j][lane], packet j holding
+// complex numbers CPP*j .. CPP*j+CPP-1 of the site's run c = d*K + k (d = direction 0..7,
+// k = 3*row+col).  in: the other parity's spinor planes; out / own: this parity's.
+// partials: HOP_XPAY_DOT writes sum over the block of Re<own,out> (fp64) to
+// partials[blockIdx.x]; the kernel that needs <d,Ad> adds them in index order (stag_blas.cuh).
 template <typename T, int NR, int MODE>
-__global__ void __launch_bounds__(DSLASH_BLOCK)
+__global__ void __launch_bounds__(DSLASH_BLOCK, HopTune<T, NR>::MINB)
 dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
-              const cplx_t<T> *__restrict__ links, const Geom g, const int p, const T m2,
+              const pkt_t<T> *__restrict__ links, const Geom g, const int p, const T m2,
               const cplx_t<T> *__restrict__ own, double *__restrict__ partials,
-              CgCtrl *__restrict__ ctrl)
+              const CgCtrl *__restrict__ ctrl)
 {
     using C = cplx_t<T>;
+    using P = pkt_t<T>;
     constexpr int K = 3 * NR;
+    constexpr int GM = HopTune<T, NR>::GM;
+    constexpr int DPG = Pkt<T>::CPP * GM;     // directions per group
+    constexpr int NG = 8 / DPG;               // groups per site
+    constexpr int KG = K * GM;                // packets per group
+    static_assert(8 % DPG == 0, "group must divide the eight directions");
     if (ctrl != nullptr && ctrl->state != CG_RUN) return;
 
     const int cb = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
@@ -60,31 +91,38 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
         // pad lanes (cb >= Vh) read zero links, so they produce zeros without a branch
         Site s;
         decode_site(g, p, cb < g.Vh ? cb : 0, s);
-        const C *L = links + (size_t)(cb >> 5) * (size_t)(8 * K * TILE) + (cb & 31);
+        const P *L = links + (size_t)(cb >> 5) * (size_t)(NG * KG * TILE) + (cb & 31);
+
+        unsigned neg = 0;
+        if (NR == 2) neg = det_sign_mask(g, s);
 
         C v[8][3];
 #pragma unroll
         for (int d = 0; d < 8; ++d)
 #pragma unroll
-            for (int c = 0; c < 3; ++c) v[d][c] = ld_cached(in + (size_t)c * g.Vh_pad + s.nbr[d]);
-
-        unsigned neg = 0;
-        if (NR == 2) neg = det_sign_mask(g, s);
+            for (int c = 0; c < 3; ++c) v[d][c] = __ldg(in + (size_t)c * g.Vh_pad + s.nbr[d]);
 
         C acc[3];
 #pragma unroll
         for (int i = 0; i < 3; ++i) acc[i] = mk<T>(0, 0);
 
 #pragma unroll
-        for (int d = 0; d < 8; ++d) {
-            C m[9];
+        for (int grp = 0; grp < NG; ++grp) {
+            P pk[KG];
 #pragma unroll
-            for (int k = 0; k < K; ++k) m[k] = ld_stream(L + (d * K + k) * TILE);
-            if (NR == 2) rebuild_row2<T>(m, (neg >> d) & 1u);
+            for (int i = 0; i < KG; ++i) pk[i] = __ldcs(L + (grp * KG + i) * TILE);
 #pragma unroll
-            for (int i = 0; i < 3; ++i)
+            for (int dd = 0; dd < DPG; ++dd) {
+                const int d = grp * DPG + dd;
+                C m[9];
 #pragma unroll
-                for (int j = 0; j < 3; ++j) cfma(acc[i], m[3 * i + j], v[d][j]);
+                for (int k = 0; k < K; ++k) m[k] = pk_get(pk, dd * K + k);
+                if (NR == 2) rebuild_row2<T>(m, (neg >> d) & 1u);
+#pragma unroll
+                for (int i = 0; i < 3; ++i)
+#pragma unroll
+                    for (int j = 0; j < 3; ++j) cfma(acc[i], m[3 * i + j], v[d][j]);
+            }
         }
 
         if (MODE == HOP_PLAIN) {
@@ -105,27 +143,12 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
     }
 
     if (MODE == HOP_XPAY_DOT) {
+        // No ticket, no fence here: a gpu-scope fence invalidates the SM's L1 under the
+        // neighbour gathers of the co-resident blocks.  The kernel boundary orders the
+        // partials for their reader.
         __shared__ double red[32];
-        __shared__ bool last;
-        double bs = block_sum(dot, red);
-        if (threadIdx.x == 0) {
-            partials[blockIdx.x] = bs;
-            __threadfence();
-            last = (atomicAdd(&ctrl->ticket[0], 1u) == gridDim.x - 1);
-        }
-        __syncthreads();
-        if (last) {
-            // fixed-order second stage: the value does not depend on block scheduling
-            double t = 0.0;
-            for (unsigned i = threadIdx.x; i < gridDim.x; i += DSLASH_BLOCK) t += __ldcg(partials + i);
-            t = block_sum(t, red);
-            if (threadIdx.x == 0) {
-                ctrl->dAd = t;
-                if (t > 0.0) ctrl->alpha = ctrl->delta / t;        // alpha = delta_new / d^dag A d
-                else ctrl->state = CG_BREAKDOWN;                   // also catches NaN
-                ctrl->ticket[0] = 0;
-            }
-        }
+        const double bs = block_sum(dot, red);
+        if (threadIdx.x == 0) partials[blockIdx.x] = bs;
     }
 }
 

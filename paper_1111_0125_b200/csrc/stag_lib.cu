@@ -139,20 +139,31 @@ gather_links_kernel(double2 *__restrict__ L, const double *__restrict__ W, const
     atomicMax(err_bits, (unsigned long long)__double_as_longlong(worst));   // worst >= 0
 }
 
-// fp64/18 gathered field -> another precision / row count
+// fp64/18 gathered field -> another precision / row count, in the packet layout of
+// stag_dslash.cuh: dst[tile][j][lane], packet j = complex numbers CPP*j .. CPP*j+CPP-1 of the
+// site's run c = d*K + k.  n_pkt = packets in dst (both parities).
 template <typename TD, int ROWS>
 __global__ void __launch_bounds__(256)
-derive_links_kernel(cplx_t<TD> *__restrict__ dst, const double2 *__restrict__ src, long n_dst)
+derive_links_kernel(pkt_t<TD> *__restrict__ dst, const double2 *__restrict__ src, long n_pkt)
 {
     constexpr int K = 3 * ROWS;
+    constexpr int CPP = Pkt<TD>::CPP;
+    constexpr int PPS = 8 * K / CPP;             // packets per site
     const long i = blockIdx.x * 256L + threadIdx.x;
-    if (i >= n_dst) return;
+    if (i >= n_pkt) return;
     const int lane = (int)(i % TILE);
     const long r = i / TILE;
-    const int k = (int)(r % K);
-    const long td = r / K;                     // (p*ntiles + tile)*8 + d
-    const double2 v = src[(td * 9 + k) * TILE + lane];
-    dst[i] = mk<TD>((TD)v.x, (TD)v.y);
+    const int j = (int)(r % PPS);
+    const long tile = r / PPS;                   // p*ntiles + tile
+    TD v[2 * CPP];
+#pragma unroll
+    for (int h = 0; h < CPP; ++h) {
+        const int c = CPP * j + h, d = c / K, k = c % K;
+        const double2 w = src[((tile * 8 + d) * 9 + k) * TILE + lane];
+        v[2 * h] = (TD)w.x;
+        v[2 * h + 1] = (TD)w.y;
+    }
+    dst[i] = pack(v);
 }
 
 template <typename T>
@@ -192,16 +203,16 @@ int ensure_links(stag_links *L, int prec)
         t_errbuf_status = STAG_EINVAL;
         return STAG_EINVAL;
     }
-    const size_t n = links_elems(L, rows);
-    const size_t bytes = n * (prec_is_f32(prec) ? sizeof(float2) : sizeof(double2));
+    const size_t bytes = links_elems(L, rows) * (prec_is_f32(prec) ? sizeof(float2) : sizeof(double2));
+    const size_t n = bytes / 16;                 // 16-byte packets
     void *dst = nullptr;
     CU(cudaMalloc(&dst, bytes));
     const unsigned grid = (unsigned)((n + 255) / 256);
     const double2 *src = (const double2 *)L->L[STAG_PREC_F64];
     switch (prec) {
-    case STAG_PREC_F32:     derive_links_kernel<float, 3><<<grid, 256, 0, t_stream>>>((float2 *)dst, src, (long)n); break;
+    case STAG_PREC_F32:     derive_links_kernel<float, 3><<<grid, 256, 0, t_stream>>>((float4 *)dst, src, (long)n); break;
     case STAG_PREC_F64_R12: derive_links_kernel<double, 2><<<grid, 256, 0, t_stream>>>((double2 *)dst, src, (long)n); break;
-    case STAG_PREC_F32_R12: derive_links_kernel<float, 2><<<grid, 256, 0, t_stream>>>((float2 *)dst, src, (long)n); break;
+    case STAG_PREC_F32_R12: derive_links_kernel<float, 2><<<grid, 256, 0, t_stream>>>((float4 *)dst, src, (long)n); break;
     default: cudaFree(dst); return STAG_EINVAL;
     }
     count_launch();
@@ -221,11 +232,12 @@ int ensure_tmp(stag_links *L, int f32)
 // ---- Dslash launcher ---------------------------------------------------------------------
 template <typename T, int NR>
 int launch_hop_t(const stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx_t<T> *in,
-                 int parity, double m2, const cplx_t<T> *own, double *partials, CgCtrl *ctrl,
+                 int parity, double m2, const cplx_t<T> *own, double *partials, const CgCtrl *ctrl,
                  cudaStream_t s)
 {
     const Geom &g = L->g;
-    const cplx_t<T> *field = (const cplx_t<T> *)L->L[prec] + (size_t)parity * L->ntiles * 8 * (3 * NR) * TILE;
+    const pkt_t<T> *field = (const pkt_t<T> *)L->L[prec] +
+                            (size_t)parity * L->ntiles * (8 * (3 * NR) / Pkt<T>::CPP) * TILE;
     const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
     switch (hop) {
     case HOP_PLAIN:
@@ -244,7 +256,7 @@ int launch_hop_t(const stag_links *L, int prec, int hop, cplx_t<T> *out, const c
 }
 
 int launch_hop(const stag_links *L, int prec, int hop, void *out, const void *in, int parity,
-               double m2, const void *own, double *partials, CgCtrl *ctrl, cudaStream_t s)
+               double m2, const void *own, double *partials, const CgCtrl *ctrl, cudaStream_t s)
 {
     switch (prec) {
     case STAG_PREC_F64:
@@ -430,7 +442,9 @@ namespace {
 
 struct Workspace {
     CgCtrl *ctrl;
-    double *partials;
+    double *partials;       // block partials of the vector kernels' reductions
+    double *hop_partials;   // block partials of <d,Ad> written by the second hop
+    int n_hop;              // = grid of the hop
     double *r64, *q64, *tmp64, *d64;
     float *y32, *r32, *d32, *q32, *tmp32;
 };
@@ -439,9 +453,10 @@ int ensure_workspace(stag_links *L, Workspace &w)
 {
     const size_t n = (size_t)6 * L->g.Vh_pad;
     const size_t nb64 = align_up(n * sizeof(double), 256), nb32 = align_up(n * sizeof(float), 256);
-    const size_t npart = (size_t)L->g.Vh_pad / DSLASH_BLOCK + 1 + (size_t)blas_grid((long)n);
-    const size_t pb = align_up(npart * sizeof(double), 256);
-    const size_t total = 256 + pb + 4 * nb64 + 5 * nb32;
+    const size_t n_hop = ((size_t)L->g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK;
+    const size_t pb = align_up((size_t)blas_grid((long)n) * sizeof(double), 256);
+    const size_t hb = align_up(n_hop * sizeof(double), 256);
+    const size_t total = 256 + pb + hb + 4 * nb64 + 5 * nb32;
     if (!L->ws) {
         CU(cudaMalloc((void **)&L->ws, total));
         L->ws_bytes = total;
@@ -450,6 +465,8 @@ int ensure_workspace(stag_links *L, Workspace &w)
     char *p = L->ws;
     w.ctrl = (CgCtrl *)p; p += 256;
     w.partials = (double *)p; p += pb;
+    w.hop_partials = (double *)p; p += hb;
+    w.n_hop = (int)n_hop;
     w.r64 = (double *)p; p += nb64;
     w.q64 = (double *)p; p += nb64;
     w.tmp64 = (double *)p; p += nb64;
@@ -511,9 +528,9 @@ struct Solver {
         KCHECK();
         int rc = launch_hop(L, prec_lo, HOP_PLAIN, tmp, d, 1, 0.0, nullptr, nullptr, w.ctrl, st);   // D_oe d
         if (rc) return rc;
-        rc = launch_hop(L, prec_lo, HOP_XPAY_DOT, q, tmp, 0, m2, d, w.partials, w.ctrl, st);  // q = A d, alpha
+        rc = launch_hop(L, prec_lo, HOP_XPAY_DOT, q, tmp, 0, m2, d, w.hop_partials, w.ctrl, st);  // q = A d, <d,q>
         if (rc) return rc;
-        update_kernel<T><<<gb, BLAS_BLOCK, 0, st>>>(y, r, d, q, n, w.partials, w.ctrl);      // y, r, delta, beta
+        update_kernel<T><<<gb, BLAS_BLOCK, 0, st>>>(y, r, d, q, n, w.hop_partials, w.n_hop, w.partials, w.ctrl);  // alpha, y, r, delta, beta
         count_launch();
         KCHECK();
         return STAG_OK;
