@@ -7,6 +7,7 @@
 // device, so the host never reads a scalar inside the iteration.
 #pragma once
 #include "stag_common.cuh"
+#include "stag_mem.cuh"
 
 namespace stag {
 
@@ -56,8 +57,8 @@ xpay_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const CgCtrl *__
     const long nv = n / N;
     for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)gridDim.x * BLAS_BLOCK) {
         T a[N], b[N];
-        unpack<T>(reinterpret_cast<const V *>(r)[i], a);
-        unpack<T>(reinterpret_cast<const V *>(d)[i], b);
+        unpack<T>(ld_keep(reinterpret_cast<const V *>(r) + i), a);
+        unpack<T>(ld_keep(reinterpret_cast<const V *>(d) + i), b);
         if (beta == (T)0) {
 #pragma unroll
             for (int k = 0; k < N; ++k) b[k] = a[k];
@@ -65,7 +66,7 @@ xpay_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const CgCtrl *__
 #pragma unroll
             for (int k = 0; k < N; ++k) b[k] = fma(beta, b[k], a[k]);
         }
-        reinterpret_cast<V *>(d)[i] = pack(b);
+        st_keep(reinterpret_cast<V *>(d) + i, pack(b));
     }
 }
 
@@ -73,8 +74,20 @@ xpay_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const CgCtrl *__
 // block: every block that calls it with the same arguments gets the same bits.
 __device__ __forceinline__ double block_total_fixed(const double *__restrict__ v, int n, double *red)
 {
+    // eight independent loads in flight per thread (a one-load-per-trip loop costs one L2
+    // round trip per element: 13 us of the 37 us update_kernel took on 28^3 x 96); the adds
+    // stay in index order, and an out-of-range slot adds +0.0, which changes nothing
     double t = 0.0;
-    for (int i = threadIdx.x; i < n; i += blockDim.x) t += __ldcg(v + i);
+    for (int base = threadIdx.x; base < n; base += 8 * blockDim.x) {
+        double e[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int i = base + u * blockDim.x;
+            e[u] = (i < n) ? __ldcg(v + i) : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) t += e[u];
+    }
     t = block_sum(t, red);
     __shared__ double total;
     if (threadIdx.x == 0) total = t;
@@ -105,18 +118,18 @@ update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
     double s = 0.0;
     for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)gridDim.x * BLAS_BLOCK) {
         T yy[N], rr[N], dd[N], qq[N];
-        unpack<T>(reinterpret_cast<const V *>(y)[i], yy);
-        unpack<T>(reinterpret_cast<const V *>(r)[i], rr);
-        unpack<T>(reinterpret_cast<const V *>(d)[i], dd);
-        unpack<T>(reinterpret_cast<const V *>(q)[i], qq);
+        unpack<T>(ld_pass(reinterpret_cast<const V *>(y) + i), yy);
+        unpack<T>(ld_keep(reinterpret_cast<const V *>(r) + i), rr);
+        unpack<T>(ld_keep(reinterpret_cast<const V *>(d) + i), dd);
+        unpack<T>(ld_keep(reinterpret_cast<const V *>(q) + i), qq);
 #pragma unroll
         for (int k = 0; k < N; ++k) {
             yy[k] = fma(alpha, dd[k], yy[k]);
             rr[k] = fma(-alpha, qq[k], rr[k]);
             s += (double)rr[k] * (double)rr[k];
         }
-        reinterpret_cast<V *>(y)[i] = pack(yy);
-        reinterpret_cast<V *>(r)[i] = pack(rr);
+        st_pass(reinterpret_cast<V *>(y) + i, pack(yy));
+        st_keep(reinterpret_cast<V *>(r) + i, pack(rr));
     }
     double bs = block_sum(s, red), dn;
     if (!finish_reduction(bs, partials, &ctrl->ticket[1], red, &dn)) return;

@@ -15,6 +15,7 @@
 // 1.05 of the measured copy bandwidth (profiles/README.md, round-1 sweep).
 #pragma once
 #include "stag_common.cuh"
+#include "stag_mem.cuh"
 
 namespace stag {
 
@@ -100,7 +101,7 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
 #pragma unroll
         for (int d = 0; d < 8; ++d)
 #pragma unroll
-            for (int c = 0; c < 3; ++c) v[d][c] = __ldg(in + (size_t)c * g.Vh_pad + s.nbr[d]);
+            for (int c = 0; c < 3; ++c) v[d][c] = ld_keep_nc(in + (size_t)c * g.Vh_pad + s.nbr[d]);
 
         C acc[3];
 #pragma unroll
@@ -110,7 +111,7 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
         for (int grp = 0; grp < NG; ++grp) {
             P pk[KG];
 #pragma unroll
-            for (int i = 0; i < KG; ++i) pk[i] = __ldcs(L + (grp * KG + i) * TILE);
+            for (int i = 0; i < KG; ++i) pk[i] = ld_stream(L + (grp * KG + i) * TILE);
 #pragma unroll
             for (int dd = 0; dd < DPG; ++dd) {
                 const int d = grp * DPG + dd;
@@ -127,15 +128,15 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
 
         if (MODE == HOP_PLAIN) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) out[(size_t)c * g.Vh_pad + cb] = acc[c];
+            for (int c = 0; c < 3; ++c) st_keep(out + (size_t)c * g.Vh_pad + cb, acc[c]);
         } else {
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const C o = own[(size_t)c * g.Vh_pad + cb];
+                const C o = ld_keep_nc(own + (size_t)c * g.Vh_pad + cb);
                 C r;
                 r.x = fma(m2, o.x, -acc[c].x);
                 r.y = fma(m2, o.y, -acc[c].y);
-                out[(size_t)c * g.Vh_pad + cb] = r;
+                st_keep(out + (size_t)c * g.Vh_pad + cb, r);
                 if (MODE == HOP_XPAY_DOT)
                     dot += (double)o.x * (double)r.x + (double)o.y * (double)r.y;
             }
