@@ -3,8 +3,10 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config NAME]
 
-One STEP = one full mixed-precision CG solve (mode 3: fp32 iteration with the corrected
-restart + reliable + group-wise updates of section 3.2, tol 1e-10) of A x = b on the
+One STEP = one full mixed-precision CG solve (mode 3: fp32 iteration on 12-real compressed
+links -- the paper's single-precision kernel also reads compressed links, P:L113 -- with the
+corrected restart + reliable + group-wise updates of section 3.2 done in fp64 on the full
+18-real links, tol 1e-10) of A x = b on the
 28^3 x 96 lattice of BASELINE.json configs[3] (the lattice the paper's numbers are quoted on,
 P:L62): every row S1-S7 of the hot path runs.  `value` is the paper's own figure of merit,
 "GFLOPS derived from the entire CG sequence" (Table 1 caption), with the flop
@@ -152,11 +154,11 @@ def run_reference(args):
 
 
 def workload_config(cfg, n_gpus, **extra):
-    c = {"workload": "%s staggered mixed-precision CG solve (mode 3), random SU(3) links with eta and antiperiodic-t folded in, Gaussian even-site source, m=%g, tol=%g" % (cfg.name, cfg.mass, cfg.tol),
+    c = {"workload": "%s staggered mixed-precision CG solve (mode 3, fp32 iteration on 12-real links, fp64 updates on 18-real links), random SU(3) links with eta and antiperiodic-t folded in, Gaussian even-site source, m=%g, tol=%g" % (cfg.name, cfg.mass, cfg.tol),
          "dims": list(cfg.dims), "even_sites": cfg.vh, "mass": cfg.mass, "tol": cfg.tol,
          "maxiter": cfg.maxiter, "parallelism": "replicas x%d (no collective)" % n_gpus,
          "flop_convention": "1224 flop / even site / iteration = 2 x 576 (P:L62) + 72",
-         "l2": "inputs exceed L2 (fp32 links 607 MB + fp64 links 1214 MB streamed per iteration / update; 126 MB L2)"}
+         "l2": "inputs exceed L2 (fp32 12-real links 405 MB per hop, 809 MB per iteration, fp64 links 1214 MB per update hop; 126 MB L2); the stand-alone Dslash timing rotates six input/output spinors"}
     c.update(extra)
     return c
 
@@ -216,11 +218,11 @@ def run_ours(args):
     x_host = torch.zeros_like(b_host).pin_memory()
 
     def solve_device():
-        return stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE)
+        return stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True)
 
     def solve_host():
         x_host.zero_()
-        return stag.cg_solve_host(b_host, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, x_host=x_host)
+        return stag.cg_solve_host(b_host, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, x_host=x_host, recon12=True)
 
     def timed(fn, steps, warmup):
         for _ in range(warmup):
@@ -251,14 +253,15 @@ def run_ours(args):
 
     # ---- rank 0, N = any: the per-kernel numbers and the CPU baseline ---------------------------
     dsl = {stag.PREC_NAMES[p]: time_dslash(stag, torch, fieldgen, cfg, L, p) for p in range(4)}
-    dom = dsl["fp32/18"]
-    roofline = {"bound": "hbm", "kernel": "dslash_kernel<float,3,*> (fp32, 18-real links)",
+    dom = dsl["fp32/12"]
+    roofline = {"bound": "hbm", "kernel": "dslash_kernel<float,2,*> (fp32, 12-real links: the hop of the timed solve)",
                 "achieved": dom["gbs"], "peak": peak, "unit": "GB/s", "frac": dom["gbs"] / peak,
-                "peak_source": peak_src, "traffic": args.traffic,
+                "peak_source": peak_src, "traffic": args.traffic if cfg.name == "c4_28^3x96" else None,
+                "traffic_source": "profiles/r1b_dslash_fp32r12_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum, one launch)",
                 "algorithmic_bytes_per_launch": dom["algorithmic_bytes_per_site"] * cfg.vh,
                 "us_per_launch": dom["us"], "frac_of_nominal_8TBs": dom["gbs"] / 8000.0}
     x64, st64 = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_F64)
-    x12, st12 = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True)
+    x18, st18 = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE)
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -285,7 +288,8 @@ def run_ours(args):
                "true_resid": st["true_resid"], "time_to_solution_s": st["seconds"],
                "ms_per_iteration": st["seconds"] / max(1, st["iters"]) * 1e3,
                "fp64_cg": {"iters": st64["iters"], "time_to_solution_s": st64["seconds"], "true_resid": st64["true_resid"]},
-               "mixed_recon12": {"iters": st12["iters"], "time_to_solution_s": st12["seconds"], "true_resid": st12["true_resid"]},
+               "mixed_18real_links": {"iters": st18["iters"], "time_to_solution_s": st18["seconds"], "true_resid": st18["true_resid"],
+                                      "ms_per_iteration": st18["seconds"] / max(1, st18["iters"]) * 1e3},
                "speedup_mixed_vs_fp64": st64["seconds"] / st["seconds"]},
         "dslash": dsl,
         "setup_s0_seconds": setup_s,
@@ -304,8 +308,9 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", default="c4_28^3x96")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--traffic", type=float, default=None,
-                    help="dram bytes per launch of the dominant kernel from an ncu --set full capture")
+    ap.add_argument("--traffic", type=float, default=436.4e6,
+                    help="dram bytes (read + write) per launch of the dominant kernel from the ncu --set full "
+                         "capture profiles/r1b_dslash_fp32r12_ncu_full.md (28^3x96, fp32/12 plain hop)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
