@@ -50,6 +50,11 @@ def _load():
         lib.so_cg.argtypes = [dp, dp, dp, ip, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                               ip, dp, ip]
         lib.so_cg.restype = ctypes.c_int
+        lib.so_apply_M.argtypes = [dp, dp, dp, ip, ctypes.c_double]
+        lib.so_apply_M.restype = ctypes.c_int
+        lib.so_solve_M.argtypes = [dp, dp, dp, ip, ctypes.c_double, ctypes.c_double, ctypes.c_int,
+                                   ip, dp]
+        lib.so_solve_M.restype = ctypes.c_int
         lib.so_redot.argtypes = [dp, dp, ctypes.c_long]
         lib.so_redot.restype = ctypes.c_double
         _lib = lib
@@ -128,3 +133,33 @@ def redot(a, b) -> float:
     a = np.ascontiguousarray(a, dtype=np.complex128)
     b = np.ascontiguousarray(b, dtype=np.complex128)
     return _load().so_redot(_dp(a), _dp(b), a.size * 2)
+
+
+def _check_full(W, dims, *vecs):
+    vh = _vh(dims)
+    _check(W, dims)
+    for v in vecs:
+        if v.dtype != np.complex128 or v.shape != (2, vh, 3) or not v.flags.c_contiguous:
+            raise ValueError("full-lattice spinor must be C-contiguous complex128 [2][Vh][3]")
+
+
+def apply_M(psi, W, dims, mass: float):
+    """(D + m) psi on the whole lattice; psi[parity][cb][3] (Q23)."""
+    _check_full(W, dims, psi)
+    out = np.empty_like(psi)
+    if _load().so_apply_M(_dp(out), _dp(psi), _dp(W), _cdims(dims), float(mass)):
+        raise ValueError("so_apply_M: bad argument")
+    return out
+
+
+def solve_M(h, W, dims, mass: float, tol: float, maxiter: int):
+    """(D + m) psi = h through the even-site solve of A.  Returns (psi, iters, resid, rc)."""
+    _check_full(W, dims, h)
+    psi = np.zeros_like(h)
+    it = ctypes.c_int(0)
+    rho = ctypes.c_double(0.0)
+    rc = _load().so_solve_M(_dp(psi), _dp(h), _dp(W), _cdims(dims), float(mass), float(tol),
+                            int(maxiter), ctypes.byref(it), ctypes.byref(rho))
+    if rc < 0:
+        raise ValueError("so_solve_M: bad argument")
+    return psi, it.value, rho.value, rc
