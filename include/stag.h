@@ -147,6 +147,21 @@ int stag_dslash(void *out, const void *in, const stag_links_t *links, int parity
 int stag_apply_A(void *out_even, const void *in_even, const stag_links_t *links, double mass,
                  int prec);
 
+/* ---- several right-hand sides sharing one pass over the links ------------------------
+ *
+ * The hop is bandwidth-bound on the gauge field, and the production use of the
+ * solver inverts on several sources per gauge field (three colours per point source).
+ * The *_mrhs entry points take nrhs spinors stored back to back -- spinor k starts
+ * k * stag_spinor_bytes(dims, prec) bytes after spinor 0 -- and read each link once per chunk
+ * of up to 4 (fp32) or 2 (fp64) right-hand sides instead of once per right-hand side
+ * (DESIGN.md section 13).  nrhs = 1 is exactly the single entry point. */
+#define STAG_MAX_RHS 12    /* most right-hand sides one solve carries */
+
+int stag_dslash_mrhs(void *out, const void *in, const stag_links_t *links, int parity,
+                     const int dims[4], int prec, int nrhs);
+int stag_apply_A_mrhs(void *out_even, const void *in_even, const stag_links_t *links, double mass,
+                      int prec, int nrhs);
+
 /* ---- the solver -------------------------------------------------------- */
 
 /* Optional knobs for stag_cg_solve_ex; zero-initialise, then set what you need
@@ -182,6 +197,30 @@ int stag_cg_solve(void *x_even, const void *b_even, const stag_links_t *links, d
 int stag_cg_solve_ex(void *x_even, const void *b_even, const stag_links_t *links, double mass,
                      double tol, int maxiter, int mode, const stag_cg_params_t *params,
                      stag_cg_stats_t *stats_out);
+
+/* nrhs <= STAG_MAX_RHS independent systems A x_k = b_k solved in lockstep: one Fig. 1
+ * recurrence per right-hand side (its own alpha, beta, residual, stopping test), one shared
+ * iteration loop, every hop applied to all of them at once.  A right-hand side that has met
+ * its target is frozen (no longer updated) while the others finish; in mode 3 a reliable
+ * update triggered by any right-hand side is carried out for all.  x_even / b_even: nrhs fp64
+ * device spinors back to back.  stats_out: nrhs entries (or NULL); iters is the number of loop
+ * passes during which that right-hand side was active.  Returns STAG_OK only if every
+ * right-hand side met tol; STAG_ENOCONV / STAG_EBREAKDOWN / < 0 as stag_cg_solve. */
+int stag_cg_solve_mrhs(void *x_even, const void *b_even, const stag_links_t *links, double mass,
+                       double tol, int maxiter, int mode, int nrhs,
+                       const stag_cg_params_t *params, stag_cg_stats_t *stats_out);
+
+/* The staggered propagator: (D + m) psi = h on the WHOLE lattice (the system whose normal
+ * equations are eq. 2.2-2.3: (D+m)^dag (D+m) = -D^2 + m^2 = A because D^dag = -D, eq. 2.4;
+ * DESIGN.md Q23), for nrhs sources, through one even-site solve:
+ *     b_e = m h_e - D_eo h_o ;   A psi_e = b_e (stag_cg_solve_mrhs) ;   psi_o = (h_o - D_oe psi_e) / m
+ * All four spinor arguments are nrhs fp64 device spinors back to back, one parity each;
+ * psi_even holds the initial guess of the even-site solve on entry.  tol applies to the
+ * even-site system (|b_e - A psi_e| <= tol |b_e|), which bounds |h - (D+m) psi| <= tol |b_e| / m.
+ * mass must be non-zero.  stats_out and the return value are those of the even-site solve. */
+int stag_solve_M(void *psi_even, void *psi_odd, const void *h_even, const void *h_odd,
+                 const stag_links_t *links, double mass, double tol, int maxiter, int mode,
+                 int nrhs, const stag_cg_params_t *params, stag_cg_stats_t *stats_out);
 
 /* The same solve from and to HOST memory in the canonical fp64 layout (Vh*6 doubles each):
  * copies b (and x as the initial guess) to the device, packs, solves, unpacks, copies x back.

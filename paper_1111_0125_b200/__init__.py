@@ -12,6 +12,14 @@ The names mirror the C entry points:
     out   = apply_A(v, links, mass, prec)       # stag_apply_A       (eq. 2.3)
     x, st = cg_solve(b, links, mass, tol, maxiter, mode)   # stag_cg_solve_ex
 
+Several right-hand sides sharing each pass over the links (a batch is a 2-D tensor
+[nrhs][6*Vh_pad], one device spinor per row):
+
+    outs    = dslash_mrhs(vs, links, parity, prec)          # stag_dslash_mrhs
+    outs    = apply_A_mrhs(vs, links, mass, prec)           # stag_apply_A_mrhs
+    xs, sts = cg_solve_mrhs(bs, links, mass, tol, maxiter)  # stag_cg_solve_mrhs
+    pe, po, sts = solve_M(he, ho, links, mass, tol, maxiter)   # stag_solve_M: (D+m) psi = h
+
 There is no CPU fallback: importing works anywhere the shared library loads, but
 every compute entry raises unless a CUDA device is present.
 """
@@ -29,6 +37,8 @@ _HEADER = os.path.join(os.path.dirname(_HERE), "include", "stag.h")
 PREC_F64, PREC_F32, PREC_F64_R12, PREC_F32_R12 = 0, 1, 2, 3
 CG_F64, CG_F32, CG_DEFECT, CG_RELIABLE = 0, 1, 2, 3
 OK, EINVAL, ECUDA, ENOMEM, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, 1, 2
+
+MAX_RHS = 12
 
 PREC_NAMES = {PREC_F64: "fp64/18", PREC_F32: "fp32/18", PREC_F64_R12: "fp64/12", PREC_F32_R12: "fp32/12"}
 
@@ -95,6 +105,14 @@ SIGNATURES = {
                                      ctypes.c_int, _ip, _dp]),
     "stag_cg_solve_ex": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                         ctypes.c_int, ctypes.POINTER(_Params), ctypes.POINTER(_Stats)]),
+    "stag_dslash_mrhs": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, _ip, ctypes.c_int, ctypes.c_int]),
+    "stag_apply_A_mrhs": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_int, ctypes.c_int]),
+    "stag_cg_solve_mrhs": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
+                                          ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Params),
+                                          ctypes.POINTER(_Stats)]),
+    "stag_solve_M": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_double,
+                                    ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Params),
+                                    ctypes.POINTER(_Stats)]),
     "stag_cg_solve_host": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double,
                                           ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Params),
                                           ctypes.POINTER(_Stats)]),
@@ -333,3 +351,80 @@ def cg_solve_host(b_host, links: Links, mass: float, tol: float, maxiter: int,
                                   ctypes.byref(p), ctypes.byref(st))
     _check(rc, allow=(OK, ENOCONV, EBREAKDOWN))
     return x_host, _stats_dict(st, rc)
+
+
+# ---- several right-hand sides (include/stag.h "several right-hand sides") -------------------
+
+def spinor_pack_mrhs(chis, dims, prec):
+    """list of canonical spinors -> batch tensor [nrhs][6*Vh_pad] (one device spinor per row)."""
+    torch = _require_cuda()
+    return torch.stack([spinor_pack(c, dims, prec) for c in chis]).contiguous()
+
+
+def spinor_unpack_mrhs(vs, dims, prec):
+    return [spinor_unpack(vs[k], dims, prec) for k in range(vs.shape[0])]
+
+
+def _batch(vs):
+    if vs.dim() != 2 or not vs.is_contiguous():
+        raise ValueError("a batch is a contiguous 2-D tensor [nrhs][6*Vh_pad]")
+    return int(vs.shape[0])
+
+
+def dslash_mrhs(vs, links: Links, parity: int, prec, out=None):
+    """One hop of eq. 2.5 applied to every spinor of the batch, links read once per chunk."""
+    torch = _require_cuda()
+    use_current_stream()
+    n = _batch(vs)
+    if out is None:
+        out = torch.empty_like(vs)
+    _check(lib().stag_dslash_mrhs(ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(vs.data_ptr()),
+                                  links.handle, int(parity), _cdims(links.dims), int(prec), n))
+    return out
+
+
+def apply_A_mrhs(vs_even, links: Links, mass: float, prec, out=None):
+    torch = _require_cuda()
+    use_current_stream()
+    n = _batch(vs_even)
+    if out is None:
+        out = torch.empty_like(vs_even)
+    _check(lib().stag_apply_A_mrhs(ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(vs_even.data_ptr()),
+                                   links.handle, float(mass), int(prec), n))
+    return out
+
+
+def cg_solve_mrhs(bs, links: Links, mass: float, tol: float, maxiter: int, mode: int = CG_RELIABLE,
+                  x0=None, eps_in=None, recon12=False, graph_chunk=None, recon12_f64=False):
+    """nrhs systems A x_k = b_k in lockstep.  bs, x0: fp64 batches.  Returns (xs, [stats])."""
+    torch = _require_cuda()
+    use_current_stream()
+    n = _batch(bs)
+    xs = torch.zeros_like(bs) if x0 is None else x0.clone()
+    sts = (_Stats * n)()
+    p = _params(eps_in, recon12, graph_chunk, recon12_f64)
+    rc = lib().stag_cg_solve_mrhs(ctypes.c_void_p(xs.data_ptr()), ctypes.c_void_p(bs.data_ptr()),
+                                  links.handle, float(mass), float(tol), int(maxiter), int(mode), n,
+                                  ctypes.byref(p), sts)
+    _check(rc, allow=(OK, ENOCONV, EBREAKDOWN))
+    return xs, [_stats_dict(sts[k], rc) for k in range(n)]
+
+
+def solve_M(h_even, h_odd, links: Links, mass: float, tol: float, maxiter: int,
+            mode: int = CG_RELIABLE, eps_in=None, recon12=False, graph_chunk=None, recon12_f64=False):
+    """(D + m) psi = h on the whole lattice for a batch of sources (fp64 batches, one parity
+    each).  Returns (psi_even, psi_odd, [stats of the even-site solve])."""
+    torch = _require_cuda()
+    use_current_stream()
+    n = _batch(h_even)
+    if _batch(h_odd) != n:
+        raise ValueError("h_even and h_odd must hold the same number of sources")
+    pe, po = torch.zeros_like(h_even), torch.empty_like(h_odd)
+    sts = (_Stats * n)()
+    p = _params(eps_in, recon12, graph_chunk, recon12_f64)
+    rc = lib().stag_solve_M(ctypes.c_void_p(pe.data_ptr()), ctypes.c_void_p(po.data_ptr()),
+                            ctypes.c_void_p(h_even.data_ptr()), ctypes.c_void_p(h_odd.data_ptr()),
+                            links.handle, float(mass), float(tol), int(maxiter), int(mode), n,
+                            ctypes.byref(p), sts)
+    _check(rc, allow=(OK, ENOCONV, EBREAKDOWN))
+    return pe, po, [_stats_dict(sts[k], rc) for k in range(n)]

@@ -1,10 +1,13 @@
 // stag_blas.cuh -- the CG vector algebra of Fig. 1 as fused, streaming kernels.
 //
-// Vectors are the flat device spinors (6*Vh_pad reals, pads zero).  Every inner product is
-// accumulated in fp64 whatever the vector precision.  Reductions are two-stage and
-// fixed-order: each block writes one partial, the last block to finish (ticket) adds the
-// partials in index order and runs the scalar epilogue (alpha, beta, stopping tests) on the
-// device, so the host never reads a scalar inside the iteration.
+// Vectors are the flat device spinors (n = 6*Vh_pad reals, pads zero); a solve carries nrhs of
+// them back to back (right-hand side k starts k*n reals in) and every kernel here runs on a
+// 2-D grid: blockIdx.y = k, blockIdx.x strides over the packets of that one vector, so each
+// block works with the scalars of a single right-hand side.  Every inner product is accumulated
+// in fp64 whatever the vector precision.  Reductions are two-stage and fixed-order:
+// each block writes one partial, the last block of the whole grid to finish (ticket) adds the
+// partials of every right-hand side in index order and runs the scalar epilogue (alpha, beta,
+// stopping tests) on the device, so the host never reads a scalar inside the iteration.
 #pragma once
 #include "stag_common.cuh"
 #include "stag_mem.cuh"
@@ -24,24 +27,31 @@ template <typename T> __device__ __forceinline__ void unpack(const double2 &v, T
 __device__ __forceinline__ float4 pack(const float *a) { return make_float4(a[0], a[1], a[2], a[3]); }
 __device__ __forceinline__ double2 pack(const double *a) { return make_double2(a[0], a[1]); }
 
-// Second stage shared by all reducing kernels: returns true in thread 0 of the last block with
-// *total = sum of partials[0..gridDim.x) in fixed order.
+// Second stage shared by all reducing kernels.  Every block calls it with its partial of
+// right-hand side blockIdx.y; in the LAST block of the grid to arrive it returns true (to all
+// threads) with totals[k] = sum of partials[k*gridDim.x .. +gridDim.x) in index order for every
+// k < gridDim.y (totals is shared memory, MAX_RHS doubles).
 __device__ __forceinline__ bool finish_reduction(double block_value, double *partials,
-                                                 unsigned *ticket, double *red, double *total)
+                                                 unsigned *ticket, double *red, double *totals)
 {
     __shared__ bool last;
     if (threadIdx.x == 0) {
-        partials[blockIdx.x] = block_value;
+        partials[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = block_value;
         __threadfence();
-        last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+        last = (atomicAdd(ticket, 1u) == gridDim.x * gridDim.y - 1);
     }
     __syncthreads();
     if (!last) return false;
-    double t = 0.0;
-    for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x) t += __ldcg(partials + i);
-    t = block_sum(t, red);
-    if (threadIdx.x == 0) { *total = t; *ticket = 0; return true; }
-    return false;
+    for (unsigned k = 0; k < gridDim.y; ++k) {
+        double t = 0.0;
+        for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x)
+            t += __ldcg(partials + (size_t)k * gridDim.x + i);
+        t = block_sum(t, red);
+        if (threadIdx.x == 0) totals[k] = t;
+    }
+    if (threadIdx.x == 0) *ticket = 0;
+    __syncthreads();
+    return true;
 }
 
 // d = r + beta d   (Fig. 1; eq. 3.1 P:L91 when it follows an update).  beta = 0
@@ -50,23 +60,26 @@ template <typename T>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 xpay_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const CgCtrl *__restrict__ ctrl)
 {
-    if (ctrl->state != CG_RUN) return;
+    const int k = blockIdx.y;
+    if (ctrl->state != CG_RUN || !ctrl->active[k]) return;
     using V = typename Vec4<T>::type;
     constexpr int N = Vec4<T>::N;
-    const T beta = (T)ctrl->beta;
+    const T beta = (T)ctrl->beta[k];
     const long nv = n / N;
+    V *dk = reinterpret_cast<V *>(d + (size_t)k * n);
+    const V *rk = reinterpret_cast<const V *>(r + (size_t)k * n);
     for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)gridDim.x * BLAS_BLOCK) {
         T a[N], b[N];
-        unpack<T>(ld_keep(reinterpret_cast<const V *>(r) + i), a);
-        unpack<T>(ld_keep(reinterpret_cast<const V *>(d) + i), b);
+        unpack<T>(ld_keep(rk + i), a);
+        unpack<T>(ld_keep(dk + i), b);
         if (beta == (T)0) {
 #pragma unroll
-            for (int k = 0; k < N; ++k) b[k] = a[k];
+            for (int j = 0; j < N; ++j) b[j] = a[j];
         } else {
 #pragma unroll
-            for (int k = 0; k < N; ++k) b[k] = fma(beta, b[k], a[k]);
+            for (int j = 0; j < N; ++j) b[j] = fma(beta, b[j], a[j]);
         }
-        st_keep(reinterpret_cast<V *>(d) + i, pack(b));
+        st_keep(dk + i, pack(b));
     }
 }
 
@@ -96,70 +109,97 @@ __device__ __forceinline__ double block_total_fixed(const double *__restrict__ v
 }
 
 // alpha = delta / <d,Ad> ; y += alpha d ; r -= alpha q ; delta' = |r|^2 ; then the scalar part
-// of the iteration (P:L51-54 and the trigger of P:L97) in the last block.
-// <d,Ad> arrives as the per-block partial sums of the second hop (stag_dslash.cuh); every block
-// adds them in the same order, so all blocks use the same alpha and no extra launch or
-// device-wide fence is needed between the hop and this kernel.
+// of the iteration (P:L51-54 and the trigger of P:L97) in the last block, for every right-hand
+// side.  <d,Ad> arrives as the per-block partial sums of the second hop (stag_dslash.cuh): every
+// block of right-hand side k adds the n_hop partials of k in the same order, so all of them use
+// the same alpha and no extra launch or device-wide fence is needed between the hop and this
+// kernel.  A frozen right-hand side (active == 0) is not touched.
 template <typename T>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
               const T *__restrict__ q, long n, const double *__restrict__ hop_partials,
-              int n_hop_partials, double *__restrict__ partials, CgCtrl *__restrict__ ctrl)
+              int n_hop, double *__restrict__ partials, CgCtrl *__restrict__ ctrl)
 {
     if (ctrl->state != CG_RUN) return;
     using V = typename Vec4<T>::type;
     constexpr int N = Vec4<T>::N;
     __shared__ double red[32];
-    const double dAd = block_total_fixed(hop_partials, n_hop_partials, red);
-    const bool ok = dAd > 0.0;                       // false also for NaN
-    const double alpha_d = ok ? ctrl->delta / dAd : 0.0;   // alpha = delta_new / d^dag A d
-    const T alpha = (T)alpha_d;
-    const long nv = n / N;
+    __shared__ double totals[MAX_RHS];
+    const int k = blockIdx.y;
     double s = 0.0;
-    for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)gridDim.x * BLAS_BLOCK) {
-        T yy[N], rr[N], dd[N], qq[N];
-        unpack<T>(ld_pass(reinterpret_cast<const V *>(y) + i), yy);
-        unpack<T>(ld_keep(reinterpret_cast<const V *>(r) + i), rr);
-        unpack<T>(ld_keep(reinterpret_cast<const V *>(d) + i), dd);
-        unpack<T>(ld_keep(reinterpret_cast<const V *>(q) + i), qq);
+    if (ctrl->active[k]) {
+        const double dAd = block_total_fixed(hop_partials + (size_t)k * n_hop, n_hop, red);
+        const bool ok = dAd > 0.0;                       // false also for NaN
+        const double alpha_d = ok ? ctrl->delta[k] / dAd : 0.0;   // alpha = delta_new / d^dag A d
+        if (blockIdx.x == 0 && threadIdx.x == 0) { ctrl->dAd[k] = dAd; ctrl->alpha[k] = alpha_d; }
+        const T alpha = (T)alpha_d;
+        const long nv = n / N;
+        V *yk = reinterpret_cast<V *>(y + (size_t)k * n);
+        V *rk = reinterpret_cast<V *>(r + (size_t)k * n);
+        const V *dk = reinterpret_cast<const V *>(d + (size_t)k * n);
+        const V *qk = reinterpret_cast<const V *>(q + (size_t)k * n);
+        for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)gridDim.x * BLAS_BLOCK) {
+            T yy[N], rr[N], dd[N], qq[N];
+            unpack<T>(ld_pass(yk + i), yy);
+            unpack<T>(ld_keep(rk + i), rr);
+            unpack<T>(ld_keep(dk + i), dd);
+            unpack<T>(ld_keep(qk + i), qq);
 #pragma unroll
-        for (int k = 0; k < N; ++k) {
-            yy[k] = fma(alpha, dd[k], yy[k]);
-            rr[k] = fma(-alpha, qq[k], rr[k]);
-            s += (double)rr[k] * (double)rr[k];
+            for (int j = 0; j < N; ++j) {
+                yy[j] = fma(alpha, dd[j], yy[j]);
+                rr[j] = fma(-alpha, qq[j], rr[j]);
+                s += (double)rr[j] * (double)rr[j];
+            }
+            st_pass(yk + i, pack(yy));
+            st_keep(rk + i, pack(rr));
         }
-        st_pass(reinterpret_cast<V *>(y) + i, pack(yy));
-        st_keep(reinterpret_cast<V *>(r) + i, pack(rr));
     }
-    double bs = block_sum(s, red), dn;
-    if (!finish_reduction(bs, partials, &ctrl->ticket[1], red, &dn)) return;
+    const double bs = block_sum(s, red);
+    if (!finish_reduction(bs, partials, &ctrl->ticket[1], red, totals)) return;
+    if (threadIdx.x != 0) return;
 
     // ---- scalar epilogue, one thread ------------------------------------------------
-    const int it = ctrl->iter + 1;
+    const int it = ctrl->iter + 1, mode = ctrl->mode, nrhs = ctrl->nrhs;
     ctrl->iter = it;
-    ctrl->dAd = dAd;
-    ctrl->alpha = alpha_d;
-    int st = CG_RUN;
-    if (!ok || !(dn == dn)) st = CG_BREAKDOWN;
-    else if (ctrl->mode == STAG_CG_RELIABLE) {
-        const double rn = sqrt(dn);
-        if (dn <= ctrl->tol2b || rn < ctrl->eps_in * ctrl->maxr) st = CG_UPDATE;   // P:L97, Q11
-        else ctrl->maxr = fmax(ctrl->maxr, rn);                                    // Q9
-    } else if (ctrl->mode == STAG_CG_DEFECT) {
-        if (dn <= ctrl->inner2) st = CG_CONVERGED;                                 // Fig. 2 inner
-    } else {
-        if (dn <= ctrl->tol2b) st = CG_CONVERGED;                                  // Fig. 1
+    bool breakdown = false, trigger = false;
+    unsigned conv = 0;
+    for (int j = 0; j < nrhs; ++j) {
+        if (!ctrl->active[j]) continue;
+        ctrl->iters[j] += 1;
+        const double dn = totals[j];
+        ctrl->sum1[j] = dn;
+        // dAd[j] was written by another block of this launch: read it past L1
+        if (!(__ldcg(&ctrl->dAd[j]) > 0.0) || !(dn == dn)) { breakdown = true; continue; }
+        if (mode == STAG_CG_RELIABLE) {
+            const double rn = sqrt(dn);
+            if (dn <= ctrl->tol2b[j] || rn < ctrl->eps_in * ctrl->maxr[j]) trigger = true;   // P:L97, Q11
+            else ctrl->maxr[j] = fmax(ctrl->maxr[j], rn);                                    // Q9
+        } else if (mode == STAG_CG_DEFECT) {
+            if (dn <= ctrl->inner2[j]) conv |= 1u << j;                                      // Fig. 2 inner
+        } else {
+            if (dn <= ctrl->tol2b[j]) conv |= 1u << j;                                       // Fig. 1
+        }
     }
-    if (st != CG_UPDATE) {            // on an update beta is formed from the corrected residual
-        ctrl->beta = dn / ctrl->delta;
-        ctrl->delta = dn;
+    int st = CG_RUN;
+    if (breakdown) st = CG_BREAKDOWN;
+    else if (trigger) st = CG_UPDATE;     // beta is then formed from the corrected residuals (Q10)
+    else {
+        bool any = false;
+        for (int j = 0; j < nrhs; ++j) {
+            if (!ctrl->active[j]) continue;
+            const double dn = totals[j];
+            ctrl->beta[j] = dn / ctrl->delta[j];
+            ctrl->delta[j] = dn;
+            if (conv & (1u << j)) ctrl->active[j] = 0;      // this right-hand side is done: freeze it
+            else any = true;
+        }
+        if (!any) st = CG_CONVERGED;
     }
     if (st == CG_RUN && it >= ctrl->maxiter) st = CG_MAXITER;
-    ctrl->sum1 = dn;
     ctrl->state = st;
 }
 
-// x64 += y ; y = 0  (group-wise update)
+// x64 += y ; y = 0  (group-wise update); the vectors are nrhs*n reals long
 template <typename T>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 accumulate_kernel(double *__restrict__ x, T *__restrict__ y, long n)
@@ -172,10 +212,13 @@ accumulate_kernel(double *__restrict__ x, T *__restrict__ y, long n)
 
 enum { RES_INIT = 0, RES_UPDATE = 1, RES_FINAL = 2, RES_NORM = 3 };
 
-// r = b - q in fp64, |r|^2, and optionally the fp32 copy of r (reliable update).
-// With WHAT == RES_NORM it only computes |b|^2.  The last block then sets the solver scalars:
-//   RES_INIT   start or restart: delta = |r|^2, beta = 0, maxr = |r|
-//   RES_UPDATE after x += y (eq. 3.1): beta = |r|^2 / delta_old, delta = |r|^2
+// r = b - q in fp64, |r|^2, and optionally the fp32 copy of r (reliable update), for
+// every right-hand side.  With WHAT == RES_NORM it only computes |b|^2.  The last block then
+// sets the solver scalars of each right-hand side k:
+//   RES_INIT   start, restart or outer step: delta = |r|^2, beta = 0, maxr = |r|, and k is
+//              active iff |r|^2 > tol^2 |b|^2
+//   RES_UPDATE after x += y (eq. 3.1): beta = |r|^2 / delta_old, delta = |r|^2;
+//              an active k whose true residual meets the target is frozen
 //   RES_FINAL  exit: only report |r|^2
 template <typename T, int WHAT>
 __global__ void __launch_bounds__(BLAS_BLOCK)
@@ -183,48 +226,55 @@ residual_kernel(double *__restrict__ r, const double *__restrict__ b,
                 const double *__restrict__ q, T *__restrict__ r_lo, long n,
                 double *__restrict__ partials, CgCtrl *__restrict__ ctrl)
 {
+    const size_t off = (size_t)blockIdx.y * n;
     double s = 0.0;
     for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < n; i += (long)gridDim.x * BLAS_BLOCK) {
         if (WHAT == RES_NORM) {
-            const double v = b[i];
+            const double v = b[off + i];
             s += v * v;
         } else {
-            const double v = b[i] - q[i];
-            r[i] = v;
-            if (r_lo != nullptr) r_lo[i] = (T)v;
+            const double v = b[off + i] - q[off + i];
+            r[off + i] = v;
+            if (r_lo != nullptr) r_lo[off + i] = (T)v;
             s += v * v;
         }
     }
     __shared__ double red[32];
-    double bs = block_sum(s, red), dn;
-    if (!finish_reduction(bs, partials, &ctrl->ticket[2], red, &dn)) return;
+    __shared__ double totals[MAX_RHS];
+    const double bs = block_sum(s, red);
+    if (!finish_reduction(bs, partials, &ctrl->ticket[2], red, totals)) return;
+    if (threadIdx.x != 0) return;
 
-    ctrl->sum0 = dn;
-    if (WHAT == RES_NORM) {
-        ctrl->bnorm2 = dn;
-    } else if (WHAT == RES_INIT) {
-        ctrl->delta = dn;
-        ctrl->beta = 0.0;
-        ctrl->maxr = sqrt(dn);
-        ctrl->inner2 = fmax(ctrl->eps_in * ctrl->eps_in * dn, ctrl->tol2b);   // Fig. 2, Q8
-        int st = CG_RUN;
-        if (!(dn == dn)) st = CG_BREAKDOWN;
-        else if (dn <= ctrl->tol2b) st = CG_CONVERGED;
-        else if (ctrl->iter >= ctrl->maxiter) st = CG_MAXITER;
-        ctrl->state = st;
-    } else if (WHAT == RES_UPDATE) {
-        ctrl->n_updates += 1;
-        ctrl->maxr = sqrt(dn);                                                // Q9
-        int st = CG_RUN;
-        if (!(dn == dn)) st = CG_BREAKDOWN;
-        else if (dn <= ctrl->tol2b) st = CG_CONVERGED;
-        else {
-            ctrl->beta = dn / ctrl->delta;                                    // Q10
-            ctrl->delta = dn;
-            if (ctrl->iter >= ctrl->maxiter) st = CG_MAXITER;
+    const int nrhs = ctrl->nrhs;
+    bool any = false, bad = false;
+    for (int k = 0; k < nrhs; ++k) {
+        const double dn = totals[k];
+        if (WHAT == RES_NORM) { ctrl->bnorm2[k] = dn; continue; }
+        ctrl->sum0[k] = dn;
+        if (WHAT == RES_FINAL) continue;
+        if (!(dn == dn)) { bad = true; continue; }
+        if (WHAT == RES_INIT) {
+            ctrl->delta[k] = dn;
+            ctrl->beta[k] = 0.0;
+            ctrl->maxr[k] = sqrt(dn);
+            ctrl->inner2[k] = fmax(ctrl->eps_in * ctrl->eps_in * dn, ctrl->tol2b[k]);   // Fig. 2, Q8
+            ctrl->active[k] = dn > ctrl->tol2b[k];
+        } else if (ctrl->active[k]) {                     // RES_UPDATE
+            ctrl->maxr[k] = sqrt(dn);                                                   // Q9
+            if (dn <= ctrl->tol2b[k]) ctrl->active[k] = 0;
+            else {
+                ctrl->beta[k] = dn / ctrl->delta[k];                                    // Q10
+                ctrl->delta[k] = dn;
+            }
         }
-        ctrl->state = st;
+        any = any || ctrl->active[k];
     }
+    if (WHAT == RES_NORM || WHAT == RES_FINAL) return;
+    if (WHAT == RES_UPDATE) ctrl->n_updates += 1;
+    int st = any ? CG_RUN : CG_CONVERGED;
+    if (bad) st = CG_BREAKDOWN;
+    else if (any && ctrl->iter >= ctrl->maxiter) st = CG_MAXITER;
+    ctrl->state = st;
 }
 
 // dst = (T) src, elementwise (precision change of a device spinor)

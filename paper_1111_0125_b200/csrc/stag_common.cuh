@@ -138,23 +138,34 @@ __device__ __forceinline__ double block_sum(double v, double *red)
     return t;
 }
 
-// Device-resident solver scalars and control.  One per solve.
+// Device-resident solver scalars and control.  One per solve.  A solve
+// carries nrhs <= MAX_RHS right-hand sides in lockstep: one Fig. 1 recurrence each (its own
+// alpha, beta, delta), one shared iteration counter and one shared state, so that every hop
+// reads the gauge field once for all of them.
+constexpr int MAX_RHS = STAG_MAX_RHS;
+
 struct CgCtrl {
-    double delta;        // |r|^2 entering the iteration (delta_new of Fig. 1)
-    double dAd;          // <d, A d>
-    double alpha, beta;
-    double maxr;         // max |r| since the last update (Q9) / |r| at the last update (mode 2)
-    double tol2b;        // tol^2 |b|^2 : the stopping threshold on delta (Q6)
-    double inner2;       // mode 2: inner stopping threshold on delta
+    double delta[MAX_RHS];   // |r|^2 entering the iteration (delta_new of Fig. 1)
+    double dAd[MAX_RHS];     // <d, A d>
+    double alpha[MAX_RHS], beta[MAX_RHS];
+    double maxr[MAX_RHS];    // max |r| since the last update (Q9) / |r| at the last update (mode 2)
+    double tol2b[MAX_RHS];   // tol^2 |b|^2 : the stopping threshold on delta (Q6)
+    double inner2[MAX_RHS];  // mode 2: inner stopping threshold on delta
+    double bnorm2[MAX_RHS];
+    double sum0[MAX_RHS];    // |b - A x|^2 of the last fp64 residual evaluation
+    double sum1[MAX_RHS];    // the iterated |r|^2 of the last iteration
     double eps_in;
-    double bnorm2;
-    double sum0, sum1;   // scratch results of reductions outside the loop
-    int state;           // CG_RUN ...
-    int iter, maxiter;
+    int active[MAX_RHS];     // 1: this right-hand side is still iterating; 0: frozen (done)
+    int iters[MAX_RHS];      // loop passes during which it was active (Q7)
+    int state;               // CG_RUN ...
+    int iter, maxiter;       // shared loop counter
     int mode;
     int n_updates;
-    unsigned ticket[4];  // last-block tickets, one per reducing kernel role
+    int nrhs;
+    unsigned ticket[4];      // last-block tickets, one per reducing kernel role
 };
+constexpr int CTRL_SLOT = 2048;   // bytes reserved for CgCtrl in the workspace
+static_assert(sizeof(CgCtrl) <= CTRL_SLOT, "CgCtrl must fit its workspace slot");
 
 enum { CG_RUN = 0, CG_CONVERGED = 1, CG_UPDATE = 2, CG_MAXITER = 3, CG_BREAKDOWN = 4 };
 

@@ -21,9 +21,10 @@ namespace stag {
 
 constexpr int DSLASH_BLOCK = 128;
 
-enum { HOP_PLAIN = 0,   // out = D in
-       HOP_XPAY = 1,    // out = m2*own - D in                       (second hop of A, eq. 2.3)
-       HOP_XPAY_DOT = 2 // same, plus per-block partial sums of <own,out>  (Fig. 1)
+enum { HOP_PLAIN = 0,    // out = D in
+       HOP_XPAY = 1,     // out = a*own - D in                        (second hop of A, eq. 2.3: a = m^2)
+       HOP_XPAY_DOT = 2, // same, plus per-block partial sums of <own,out>  (Fig. 1)
+       HOP_AXPBY = 3     // out = a*own - cD * D in                   ((D+m) psi = h wrapper, Q23)
 };
 
 // 16-byte link packets: two complex numbers in fp32, one in fp64.
@@ -57,29 +58,41 @@ __device__ __forceinline__ void rebuild_row2(cplx_t<T> *m, bool neg)
     }
 }
 
-// Launch shape per precision / storage, from the sweep on 28^3 x 96 (profiles/README.md):
-// MINB = resident blocks per SM promised to ptxas, GM = directions' worth of packets loaded
-// ahead (group = K*GM packets).
-template <typename T, int NR> struct HopTune { static constexpr int MINB = 4, GM = 1; };
-template <> struct HopTune<float, 2>         { static constexpr int MINB = 6, GM = 2; };
+// Launch shape per precision / storage / right-hand sides, from the sweeps on 28^3 x 96
+// (profiles/README.md): MINB = resident blocks per SM promised to ptxas, GM = directions' worth
+// of packets loaded ahead (group = K*GM packets).  With N > 1 right-hand sides the registers go
+// to the N accumulators and the N neighbour vectors of one group instead.
+template <typename T, int NR, int N> struct HopTune { static constexpr int MINB = (N == 1) ? 4 : 3, GM = 1; };
+template <> struct HopTune<float, 2, 1>            { static constexpr int MINB = 6, GM = 2; };
+template <int N> struct HopTune<double, 3, N>      { static constexpr int MINB = (N == 1) ? 4 : 2, GM = 1; };
+template <int N> struct HopTune<double, 2, N>      { static constexpr int MINB = (N == 1) ? 4 : 2, GM = 1; };
+
+// Largest N instantiated per precision: more right-hand sides go through in chunks.
+template <typename T> struct HopMaxRhs;
+template <> struct HopMaxRhs<float>  { static constexpr int value = 4; };
+template <> struct HopMaxRhs<double> { static constexpr int value = 2; };
 
 // T: float or double.  NR: rows of each link held in memory (3 = 18-real, 2 = 12-real).
+// N: right-hand sides handled by one thread; spinor k of a batch starts rs complex numbers after
+// spinor k-1 (rs = 3*Vh_pad: the batch is N device spinors back to back).
 // links: the gathered field of the OUTPUT parity as packets, L[tile][j][lane], packet j holding
 // complex numbers CPP*j .. CPP*j+CPP-1 of the site's run c = d*K + k (d = direction 0..7,
 // k = 3*row+col).  in: the other parity's spinor planes; out / own: this parity's.
-// partials: HOP_XPAY_DOT writes sum over the block of Re<own,out> (fp64) to
-// partials[blockIdx.x]; the kernel that needs <d,Ad> adds them in index order (stag_blas.cuh).
-template <typename T, int NR, int MODE>
-__global__ void __launch_bounds__(DSLASH_BLOCK, HopTune<T, NR>::MINB)
+// MODE HOP_XPAY*: out = a*own - D in;  HOP_AXPBY: out = a*own - cD * D in.
+// partials: HOP_XPAY_DOT writes sum over the block of Re<own,out> (fp64) of right-hand
+// side k to partials[k*gridDim.x + blockIdx.x]; the kernel that needs <d,Ad> adds them in index
+// order (stag_blas.cuh).
+template <typename T, int NR, int MODE, int N>
+__global__ void __launch_bounds__(DSLASH_BLOCK, HopTune<T, NR, N>::MINB)
 dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
-              const pkt_t<T> *__restrict__ links, const Geom g, const int p, const T m2,
+              const pkt_t<T> *__restrict__ links, const Geom g, const int p, const T a, const T cD,
               const cplx_t<T> *__restrict__ own, double *__restrict__ partials,
               const CgCtrl *__restrict__ ctrl)
 {
     using C = cplx_t<T>;
     using P = pkt_t<T>;
     constexpr int K = 3 * NR;
-    constexpr int GM = HopTune<T, NR>::GM;
+    constexpr int GM = HopTune<T, NR, N>::GM;
     constexpr int DPG = Pkt<T>::CPP * GM;     // directions per group
     constexpr int NG = 8 / DPG;               // groups per site
     constexpr int KG = K * GM;                // packets per group
@@ -87,7 +100,10 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
     if (ctrl != nullptr && ctrl->state != CG_RUN) return;
 
     const int cb = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
-    double dot = 0.0;
+    const size_t rs = (size_t)3 * g.Vh_pad;
+    double dot[N];
+#pragma unroll
+    for (int k = 0; k < N; ++k) dot[k] = 0.0;
     if (cb < g.Vh_pad) {
         // pad lanes (cb >= Vh) read zero links, so they produce zeros without a branch
         Site s;
@@ -97,21 +113,38 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
         unsigned neg = 0;
         if (NR == 2) neg = det_sign_mask(g, s);
 
-        C v[8][3];
+        // one right-hand side: all 24 neighbour loads are issued before the link stream;
+        // several: the neighbours of one group of directions at a time (register budget)
+        constexpr int V1D = (N == 1) ? 8 : 1, VGN = (N == 1) ? 1 : N, VGD = (N == 1) ? 1 : DPG;
+        C v1[V1D][3];
+        if constexpr (N == 1) {
 #pragma unroll
-        for (int d = 0; d < 8; ++d)
+            for (int d = 0; d < 8; ++d)
 #pragma unroll
-            for (int c = 0; c < 3; ++c) v[d][c] = ld_keep_nc(in + (size_t)c * g.Vh_pad + s.nbr[d]);
+                for (int c = 0; c < 3; ++c) v1[d][c] = ld_keep_nc(in + (size_t)c * g.Vh_pad + s.nbr[d]);
+        }
 
-        C acc[3];
+        C acc[N][3];
 #pragma unroll
-        for (int i = 0; i < 3; ++i) acc[i] = mk<T>(0, 0);
+        for (int k = 0; k < N; ++k)
+#pragma unroll
+            for (int i = 0; i < 3; ++i) acc[k][i] = mk<T>(0, 0);
 
 #pragma unroll
         for (int grp = 0; grp < NG; ++grp) {
             P pk[KG];
 #pragma unroll
             for (int i = 0; i < KG; ++i) pk[i] = ld_stream(L + (grp * KG + i) * TILE);
+            C vg[VGN][VGD][3];
+            if constexpr (N > 1) {
+#pragma unroll
+                for (int k = 0; k < N; ++k)
+#pragma unroll
+                    for (int dd = 0; dd < DPG; ++dd)
+#pragma unroll
+                        for (int c = 0; c < 3; ++c)
+                            vg[k][dd][c] = ld_keep_nc(in + k * rs + (size_t)c * g.Vh_pad + s.nbr[grp * DPG + dd]);
+            }
 #pragma unroll
             for (int dd = 0; dd < DPG; ++dd) {
                 const int d = grp * DPG + dd;
@@ -120,25 +153,38 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
                 for (int k = 0; k < K; ++k) m[k] = pk_get(pk, dd * K + k);
                 if (NR == 2) rebuild_row2<T>(m, (neg >> d) & 1u);
 #pragma unroll
-                for (int i = 0; i < 3; ++i)
+                for (int k = 0; k < N; ++k)
 #pragma unroll
-                    for (int j = 0; j < 3; ++j) cfma(acc[i], m[3 * i + j], v[d][j]);
+                    for (int i = 0; i < 3; ++i)
+#pragma unroll
+                        for (int j = 0; j < 3; ++j) {
+                            if constexpr (N == 1) cfma(acc[k][i], m[3 * i + j], v1[d][j]);
+                            else cfma(acc[k][i], m[3 * i + j], vg[k][dd][j]);
+                        }
             }
         }
 
-        if (MODE == HOP_PLAIN) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) st_keep(out + (size_t)c * g.Vh_pad + cb, acc[c]);
-        } else {
+        for (int k = 0; k < N; ++k) {
+            if (MODE == HOP_PLAIN) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const C o = ld_keep_nc(own + (size_t)c * g.Vh_pad + cb);
-                C r;
-                r.x = fma(m2, o.x, -acc[c].x);
-                r.y = fma(m2, o.y, -acc[c].y);
-                st_keep(out + (size_t)c * g.Vh_pad + cb, r);
-                if (MODE == HOP_XPAY_DOT)
-                    dot += (double)o.x * (double)r.x + (double)o.y * (double)r.y;
+                for (int c = 0; c < 3; ++c) st_keep(out + k * rs + (size_t)c * g.Vh_pad + cb, acc[k][c]);
+            } else {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const C o = ld_keep_nc(own + k * rs + (size_t)c * g.Vh_pad + cb);
+                    C r;
+                    if (MODE == HOP_AXPBY) {
+                        r.x = fma(a, o.x, -cD * acc[k][c].x);
+                        r.y = fma(a, o.y, -cD * acc[k][c].y);
+                    } else {
+                        r.x = fma(a, o.x, -acc[k][c].x);
+                        r.y = fma(a, o.y, -acc[k][c].y);
+                    }
+                    st_keep(out + k * rs + (size_t)c * g.Vh_pad + cb, r);
+                    if (MODE == HOP_XPAY_DOT)
+                        dot[k] += (double)o.x * (double)r.x + (double)o.y * (double)r.y;
+                }
             }
         }
     }
@@ -148,8 +194,11 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
         // neighbour gathers of the co-resident blocks.  The kernel boundary orders the
         // partials for their reader.
         __shared__ double red[32];
-        const double bs = block_sum(dot, red);
-        if (threadIdx.x == 0) partials[blockIdx.x] = bs;
+#pragma unroll
+        for (int k = 0; k < N; ++k) {
+            const double bs = block_sum(dot[k], red);
+            if (threadIdx.x == 0) partials[(size_t)k * gridDim.x + blockIdx.x] = bs;
+        }
     }
 }
 

@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <type_traits>
 
 #include "stag_blas.cuh"
 #include "stag_common.cuh"
@@ -53,8 +54,9 @@ inline bool prec_is_f32(int prec) { return prec == STAG_PREC_F32 || prec == STAG
 inline int prec_rows(int prec) { return (prec == STAG_PREC_F64_R12 || prec == STAG_PREC_F32_R12) ? 2 : 3; }
 
 // Grid of the streaming vector kernels: 4 resident blocks of 256 threads per SM (a multiple of
-// the SM count), fewer when the vector is too short to feed them.
-int blas_grid(long n_reals)
+// the SM count) shared among the nrhs right-hand sides (grid.y = nrhs), fewer when the vector
+// is too short to feed them.  Returns grid.x, the blocks per right-hand side.
+int blas_full_grid()
 {
     static int full = 0;
     if (full == 0) {
@@ -63,8 +65,14 @@ int blas_grid(long n_reals)
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         full = sms * 4;
     }
+    return full;
+}
+int blas_grid(long n_reals, int nrhs)
+{
+    const long per = blas_full_grid() / (nrhs < 1 ? 1 : nrhs);
     const long need = (n_reals / 2 + BLAS_BLOCK - 1) / BLAS_BLOCK;
-    return (int)(need < full ? (need < 1 ? 1 : need) : full);
+    const long g = need < per ? need : per;
+    return (int)(g < 1 ? 1 : g);
 }
 
 }  // namespace
@@ -78,14 +86,18 @@ struct stag_links {
     int ntiles;            // Vh_pad / TILE
     void *L[4];            // gathered link fields by precision enum; L[STAG_PREC_F64] always set
     double recon_err;
-    void *tmp_odd[2];      // scratch odd-parity spinor for stag_apply_A: [0] fp64, [1] fp32
+    void *tmp_odd[2];      // scratch odd-parity spinors for stag_apply_A: [0] fp64, [1] fp32
+    int tmp_odd_rhs[2];    // how many right-hand sides each holds
     // CG workspace (lazy)
     char *ws;
     size_t ws_bytes;
+    int ws_rhs;            // right-hand sides the workspace was sized for
     CgCtrl *h_ctrl;        // pinned mirror
     cudaStream_t cap_stream;
     // staging for stag_cg_solve_host (lazy)
     double *stage_dev;     // 2 canonical spinors + 2 device-layout fp64 spinors
+    void *wrap_b;          // stag_solve_M: b_e of the even-site system, wrap_b_rhs spinors (lazy)
+    int wrap_b_rhs;
     cudaEvent_t ev0, ev1;
 };
 
@@ -222,18 +234,20 @@ int ensure_links(stag_links *L, int prec)
     return STAG_OK;
 }
 
-int ensure_tmp(stag_links *L, int f32)
+int ensure_tmp(stag_links *L, int f32, int nrhs)
 {
-    if (L->tmp_odd[f32]) return STAG_OK;
-    CU(cudaMalloc(&L->tmp_odd[f32], (size_t)3 * L->g.Vh_pad * (f32 ? sizeof(float2) : sizeof(double2))));
+    if (L->tmp_odd[f32] && L->tmp_odd_rhs[f32] >= nrhs) return STAG_OK;
+    if (L->tmp_odd[f32]) { CU(cudaFree(L->tmp_odd[f32])); L->tmp_odd[f32] = nullptr; }
+    CU(cudaMalloc(&L->tmp_odd[f32], (size_t)nrhs * 3 * L->g.Vh_pad * (f32 ? sizeof(float2) : sizeof(double2))));
+    L->tmp_odd_rhs[f32] = nrhs;
     return STAG_OK;
 }
 
 // ---- Dslash launcher ---------------------------------------------------------------------
-template <typename T, int NR>
-int launch_hop_t(const stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx_t<T> *in,
-                 int parity, double m2, const cplx_t<T> *own, double *partials, const CgCtrl *ctrl,
-                 cudaStream_t s)
+template <typename T, int NR, int N>
+int launch_hop_n(const stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx_t<T> *in,
+                 int parity, double a, double cD, const cplx_t<T> *own, double *partials,
+                 const CgCtrl *ctrl, cudaStream_t s)
 {
     const Geom &g = L->g;
     const pkt_t<T> *field = (const pkt_t<T> *)L->L[prec] +
@@ -241,13 +255,19 @@ int launch_hop_t(const stag_links *L, int prec, int hop, cplx_t<T> *out, const c
     const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
     switch (hop) {
     case HOP_PLAIN:
-        dslash_kernel<T, NR, HOP_PLAIN><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)m2, own, partials, ctrl);
+        dslash_kernel<T, NR, HOP_PLAIN, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl);
         break;
     case HOP_XPAY:
-        dslash_kernel<T, NR, HOP_XPAY><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)m2, own, partials, ctrl);
+        dslash_kernel<T, NR, HOP_XPAY, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl);
+        break;
+    case HOP_AXPBY:   // only the fp64 wrapper steps use it
+        if constexpr (std::is_same<T, double>::value)
+            dslash_kernel<T, NR, HOP_AXPBY, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl);
+        else
+            return STAG_EINVAL;
         break;
     default:
-        dslash_kernel<T, NR, HOP_XPAY_DOT><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)m2, own, partials, ctrl);
+        dslash_kernel<T, NR, HOP_XPAY_DOT, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl);
         break;
     }
     count_launch();
@@ -255,18 +275,46 @@ int launch_hop_t(const stag_links *L, int prec, int hop, cplx_t<T> *out, const c
     return STAG_OK;
 }
 
+// nrhs right-hand sides in chunks of at most HopMaxRhs<T>: each chunk is one pass over the links.
+template <typename T, int NR>
+int launch_hop_t(const stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx_t<T> *in,
+                 int parity, double a, double cD, const cplx_t<T> *own, double *partials,
+                 const CgCtrl *ctrl, int nrhs, cudaStream_t s)
+{
+    constexpr int NB = HopMaxRhs<T>::value;
+    const size_t rs = (size_t)3 * L->g.Vh_pad;
+    const size_t n_hop = ((size_t)L->g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK;
+    for (int k0 = 0; k0 < nrhs; k0 += NB) {
+        const int nb = nrhs - k0 < NB ? nrhs - k0 : NB;
+        cplx_t<T> *o = out + k0 * rs;
+        const cplx_t<T> *i = in + k0 * rs;
+        const cplx_t<T> *w = own ? own + k0 * rs : nullptr;
+        double *pp = partials ? partials + k0 * n_hop : nullptr;
+        int rc = STAG_EINVAL;
+        if (nb == 1) rc = launch_hop_n<T, NR, 1>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+        if (nb == 2) rc = launch_hop_n<T, NR, 2>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+        if constexpr (NB >= 4) {
+            if (nb == 3) rc = launch_hop_n<T, NR, 3>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+            if (nb == 4) rc = launch_hop_n<T, NR, 4>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+        }
+        if (rc) return rc;
+    }
+    return STAG_OK;
+}
+
 int launch_hop(const stag_links *L, int prec, int hop, void *out, const void *in, int parity,
-               double m2, const void *own, double *partials, const CgCtrl *ctrl, cudaStream_t s)
+               double a, double cD, const void *own, double *partials, const CgCtrl *ctrl,
+               int nrhs, cudaStream_t s)
 {
     switch (prec) {
     case STAG_PREC_F64:
-        return launch_hop_t<double, 3>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, m2, (const double2 *)own, partials, ctrl, s);
+        return launch_hop_t<double, 3>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, cD, (const double2 *)own, partials, ctrl, nrhs, s);
     case STAG_PREC_F32:
-        return launch_hop_t<float, 3>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, m2, (const float2 *)own, partials, ctrl, s);
+        return launch_hop_t<float, 3>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, cD, (const float2 *)own, partials, ctrl, nrhs, s);
     case STAG_PREC_F64_R12:
-        return launch_hop_t<double, 2>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, m2, (const double2 *)own, partials, ctrl, s);
+        return launch_hop_t<double, 2>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, cD, (const double2 *)own, partials, ctrl, nrhs, s);
     case STAG_PREC_F32_R12:
-        return launch_hop_t<float, 2>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, m2, (const float2 *)own, partials, ctrl, s);
+        return launch_hop_t<float, 2>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, cD, (const float2 *)own, partials, ctrl, nrhs, s);
     }
     return STAG_EINVAL;
 }
@@ -360,6 +408,7 @@ extern "C" void stag_links_destroy(stag_links_t *L)
     if (L->ws) cudaFree(L->ws);
     if (L->h_ctrl) cudaFreeHost(L->h_ctrl);
     if (L->stage_dev) cudaFree(L->stage_dev);
+    if (L->wrap_b) cudaFree(L->wrap_b);
     if (L->cap_stream) cudaStreamDestroy(L->cap_stream);
     if (L->ev0) cudaEventDestroy(L->ev0);
     if (L->ev1) cudaEventDestroy(L->ev1);
@@ -410,29 +459,43 @@ extern "C" int stag_spinor_unpack(double *dst, const void *src, const int dims[4
 // ------------------------------------------------------------------------------------
 // C ABI: the operator
 // ------------------------------------------------------------------------------------
-extern "C" int stag_dslash(void *out, const void *in, const stag_links_t *links, int parity,
-                           const int dims[4], int prec)
+extern "C" int stag_dslash_mrhs(void *out, const void *in, const stag_links_t *links, int parity,
+                                const int dims[4], int prec, int nrhs)
 {
     stag_links *L = const_cast<stag_links *>(links);
-    if (!out || !in || !L || out == in || (parity & ~1) || !prec_ok(prec) || !same_dims(L, dims))
+    if (!out || !in || !L || out == in || (parity & ~1) || !prec_ok(prec) || !same_dims(L, dims) ||
+        nrhs < 1)
         return STAG_EINVAL;
     int rc = ensure_links(L, prec);
     if (rc) return rc;
-    return launch_hop(L, prec, HOP_PLAIN, out, in, parity, 0.0, nullptr, nullptr, nullptr, t_stream);
+    return launch_hop(L, prec, HOP_PLAIN, out, in, parity, 0.0, 1.0, nullptr, nullptr, nullptr, nrhs, t_stream);
+}
+
+extern "C" int stag_dslash(void *out, const void *in, const stag_links_t *links, int parity,
+                           const int dims[4], int prec)
+{
+    return stag_dslash_mrhs(out, in, links, parity, dims, prec, 1);
+}
+
+extern "C" int stag_apply_A_mrhs(void *out_even, const void *in_even, const stag_links_t *links,
+                                 double mass, int prec, int nrhs)
+{
+    stag_links *L = const_cast<stag_links *>(links);
+    if (!out_even || !in_even || !L || out_even == in_even || !prec_ok(prec) || nrhs < 1)
+        return STAG_EINVAL;
+    int rc = ensure_links(L, prec);
+    if (rc) return rc;
+    const int f32 = prec_is_f32(prec) ? 1 : 0;
+    if ((rc = ensure_tmp(L, f32, nrhs))) return rc;
+    // tmp_o = D_oe in_e ;  out_e = m^2 in_e - D_eo tmp_o      (eq. 2.3, P:L37)
+    if ((rc = launch_hop(L, prec, HOP_PLAIN, L->tmp_odd[f32], in_even, 1, 0.0, 1.0, nullptr, nullptr, nullptr, nrhs, t_stream))) return rc;
+    return launch_hop(L, prec, HOP_XPAY, out_even, L->tmp_odd[f32], 0, mass * mass, 1.0, in_even, nullptr, nullptr, nrhs, t_stream);
 }
 
 extern "C" int stag_apply_A(void *out_even, const void *in_even, const stag_links_t *links,
                             double mass, int prec)
 {
-    stag_links *L = const_cast<stag_links *>(links);
-    if (!out_even || !in_even || !L || out_even == in_even || !prec_ok(prec)) return STAG_EINVAL;
-    int rc = ensure_links(L, prec);
-    if (rc) return rc;
-    const int f32 = prec_is_f32(prec) ? 1 : 0;
-    if ((rc = ensure_tmp(L, f32))) return rc;
-    // tmp_o = D_oe in_e ;  out_e = m^2 in_e - D_eo tmp_o      (eq. 2.3, P:L37)
-    if ((rc = launch_hop(L, prec, HOP_PLAIN, L->tmp_odd[f32], in_even, 1, 0.0, nullptr, nullptr, nullptr, t_stream))) return rc;
-    return launch_hop(L, prec, HOP_XPAY, out_even, L->tmp_odd[f32], 0, mass * mass, in_even, nullptr, nullptr, t_stream);
+    return stag_apply_A_mrhs(out_even, in_even, links, mass, prec, 1);
 }
 
 // ------------------------------------------------------------------------------------
@@ -442,28 +505,33 @@ namespace {
 
 struct Workspace {
     CgCtrl *ctrl;
-    double *partials;       // block partials of the vector kernels' reductions
-    double *hop_partials;   // block partials of <d,Ad> written by the second hop
+    double *partials;       // block partials of the vector kernels' reductions, [rhs][block]
+    double *hop_partials;   // block partials of <d,Ad> written by the second hop, [rhs][block]
     int n_hop;              // = grid of the hop
-    double *r64, *q64, *tmp64, *d64;
+    double *r64, *q64, *tmp64, *d64;          // nrhs spinors each
     float *y32, *r32, *d32, *q32, *tmp32;
 };
 
-int ensure_workspace(stag_links *L, Workspace &w)
+// One allocation on the handle, sized for nrhs right-hand sides (grown when a later solve
+// carries more).  Right-hand side k of every vector starts k*n reals in (n = 6*Vh_pad).
+int ensure_workspace(stag_links *L, Workspace &w, int nrhs)
 {
     const size_t n = (size_t)6 * L->g.Vh_pad;
-    const size_t nb64 = align_up(n * sizeof(double), 256), nb32 = align_up(n * sizeof(float), 256);
+    if (L->ws && L->ws_rhs < nrhs) { CU(cudaFree(L->ws)); L->ws = nullptr; }
+    const int cap = L->ws ? L->ws_rhs : nrhs;
+    const size_t nb64 = align_up(cap * n * sizeof(double), 256), nb32 = align_up(cap * n * sizeof(float), 256);
     const size_t n_hop = ((size_t)L->g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK;
-    const size_t pb = align_up((size_t)blas_grid((long)n) * sizeof(double), 256);
-    const size_t hb = align_up(n_hop * sizeof(double), 256);
-    const size_t total = 256 + pb + hb + 4 * nb64 + 5 * nb32;
+    const size_t pb = align_up((size_t)MAX_RHS * blas_full_grid() * sizeof(double), 256);
+    const size_t hb = align_up((size_t)cap * n_hop * sizeof(double), 256);
+    const size_t total = CTRL_SLOT + pb + hb + 4 * nb64 + 5 * nb32;
     if (!L->ws) {
         CU(cudaMalloc((void **)&L->ws, total));
         L->ws_bytes = total;
-        CU(cudaMallocHost((void **)&L->h_ctrl, sizeof(CgCtrl)));
+        L->ws_rhs = cap;
     }
+    if (!L->h_ctrl) CU(cudaMallocHost((void **)&L->h_ctrl, sizeof(CgCtrl)));
     char *p = L->ws;
-    w.ctrl = (CgCtrl *)p; p += 256;
+    w.ctrl = (CgCtrl *)p; p += CTRL_SLOT;
     w.partials = (double *)p; p += pb;
     w.hop_partials = (double *)p; p += hb;
     w.n_hop = (int)n_hop;
@@ -479,33 +547,34 @@ int ensure_workspace(stag_links *L, Workspace &w)
     return STAG_OK;
 }
 
-static_assert(sizeof(CgCtrl) <= 256, "CgCtrl must fit its workspace slot");
-
 struct Solver {
     stag_links *L;
     Workspace w;
     cudaStream_t s;
     double m2;
     int mode;
+    int nrhs;
     int prec_lo;     // precision enum of the iteration's Dslash
     int prec_hi;     // precision enum of the fp64 corrections
     long n;          // reals per spinor
-    int gb;          // blas grid
+    int gb;          // blas grid.x (blocks per right-hand side)
     int applies_f64;
+
+    dim3 grid2() const { return dim3((unsigned)gb, (unsigned)nrhs); }
 
     // q64 = A x  in fp64 (two hops), outside the iteration
     int apply_A64(const double *x)
     {
-        int rc = launch_hop(L, prec_hi, HOP_PLAIN, w.tmp64, x, 1, 0.0, nullptr, nullptr, nullptr, s);
+        int rc = launch_hop(L, prec_hi, HOP_PLAIN, w.tmp64, x, 1, 0.0, 1.0, nullptr, nullptr, nullptr, nrhs, s);
         if (rc) return rc;
         ++applies_f64;
-        return launch_hop(L, prec_hi, HOP_XPAY, w.q64, w.tmp64, 0, m2, x, nullptr, nullptr, s);
+        return launch_hop(L, prec_hi, HOP_XPAY, w.q64, w.tmp64, 0, m2, 1.0, x, nullptr, nullptr, nrhs, s);
     }
 
     template <int WHAT>
     int residual(const double *b, bool lo_copy)
     {
-        residual_kernel<float, WHAT><<<gb, BLAS_BLOCK, 0, s>>>(w.r64, b, w.q64, lo_copy ? w.r32 : nullptr, n, w.partials, w.ctrl);
+        residual_kernel<float, WHAT><<<grid2(), BLAS_BLOCK, 0, s>>>(w.r64, b, w.q64, lo_copy ? w.r32 : nullptr, n, w.partials, w.ctrl);
         count_launch();
         KCHECK();
         return STAG_OK;
@@ -513,24 +582,25 @@ struct Solver {
 
     int accumulate(double *x)
     {
-        accumulate_kernel<float><<<gb, BLAS_BLOCK, 0, s>>>(x, w.y32, n);
+        accumulate_kernel<float><<<blas_grid(n * nrhs, 1), BLAS_BLOCK, 0, s>>>(x, w.y32, n * nrhs);
         count_launch();
         KCHECK();
         return STAG_OK;
     }
 
-    // one pass of the loop body of Fig. 1, four launches
+    // one pass of the loop body of Fig. 1, four launches (the hops: one launch per
+    // chunk of right-hand sides)
     template <typename T>
     int iteration(T *y, T *r, T *d, T *q, T *tmp, cudaStream_t st)
     {
-        xpay_kernel<T><<<gb, BLAS_BLOCK, 0, st>>>(d, r, n, w.ctrl);                          // d = r + beta d
+        xpay_kernel<T><<<grid2(), BLAS_BLOCK, 0, st>>>(d, r, n, w.ctrl);                     // d = r + beta d
         count_launch();
         KCHECK();
-        int rc = launch_hop(L, prec_lo, HOP_PLAIN, tmp, d, 1, 0.0, nullptr, nullptr, w.ctrl, st);   // D_oe d
+        int rc = launch_hop(L, prec_lo, HOP_PLAIN, tmp, d, 1, 0.0, 1.0, nullptr, nullptr, w.ctrl, nrhs, st);   // D_oe d
         if (rc) return rc;
-        rc = launch_hop(L, prec_lo, HOP_XPAY_DOT, q, tmp, 0, m2, d, w.hop_partials, w.ctrl, st);  // q = A d, <d,q>
+        rc = launch_hop(L, prec_lo, HOP_XPAY_DOT, q, tmp, 0, m2, 1.0, d, w.hop_partials, w.ctrl, nrhs, st);  // q = A d, <d,q>
         if (rc) return rc;
-        update_kernel<T><<<gb, BLAS_BLOCK, 0, st>>>(y, r, d, q, n, w.hop_partials, w.n_hop, w.partials, w.ctrl);  // alpha, y, r, delta, beta
+        update_kernel<T><<<grid2(), BLAS_BLOCK, 0, st>>>(y, r, d, q, n, w.hop_partials, w.n_hop, w.partials, w.ctrl);  // alpha, y, r, delta, beta
         count_launch();
         KCHECK();
         return STAG_OK;
@@ -550,8 +620,10 @@ struct Solver {
     }
 };
 
+// nrhs right-hand sides in lockstep.  x, b: nrhs fp64 device spinors
+// back to back.  stats: nrhs entries, or null.
 int cg_solve_device(double *x, const double *b, stag_links *L, double mass, double tol, int maxiter,
-                    int mode, const stag_cg_params_t *prm, stag_cg_stats_t *stats)
+                    int mode, int nrhs, const stag_cg_params_t *prm, stag_cg_stats_t *stats)
 {
     stag_cg_params_t P;
     memset(&P, 0, sizeof(P));
@@ -564,55 +636,66 @@ int cg_solve_device(double *x, const double *b, stag_links *L, double mass, doub
     S.s = t_stream;
     S.m2 = mass * mass;
     S.mode = mode;
+    S.nrhs = nrhs;
     S.prec_lo = (mode == STAG_CG_F64) ? (P.recon12 ? STAG_PREC_F64_R12 : STAG_PREC_F64)
                                        : (P.recon12 ? STAG_PREC_F32_R12 : STAG_PREC_F32);
     S.prec_hi = P.recon12_f64 ? STAG_PREC_F64_R12 : STAG_PREC_F64;
     S.n = (long)6 * L->g.Vh_pad;
-    S.gb = blas_grid(S.n);
+    S.gb = blas_grid(S.n, nrhs);
     S.applies_f64 = 0;
     int rc;
     if ((rc = ensure_links(L, S.prec_lo))) return rc;
     if ((rc = ensure_links(L, S.prec_hi))) return rc;
-    if ((rc = ensure_workspace(L, S.w))) return rc;
+    if ((rc = ensure_workspace(L, S.w, nrhs))) return rc;
     Workspace &w = S.w;
     cudaStream_t s = S.s;
     const bool lo = (mode != STAG_CG_F64);
+    const size_t vec_bytes = (size_t)S.n * sizeof(double);
 
     CU(cudaEventRecord(L->ev0, s));
 
-    // ---- |b|^2 and the solver scalars ---------------------------------------------------
+    // ---- |b_k|^2 and the solver scalars ---------------------------------------------------
     CgCtrl *h = L->h_ctrl;
     memset(h, 0, sizeof(*h));
     h->mode = mode;
     h->maxiter = maxiter;
     h->eps_in = P.eps_in;
+    h->nrhs = nrhs;
     CU(cudaMemcpyAsync(w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, s));
-    residual_kernel<float, RES_NORM><<<S.gb, BLAS_BLOCK, 0, s>>>(nullptr, b, nullptr, nullptr, S.n, w.partials, w.ctrl);
+    residual_kernel<float, RES_NORM><<<S.grid2(), BLAS_BLOCK, 0, s>>>(nullptr, b, nullptr, nullptr, S.n, w.partials, w.ctrl);
     count_launch();
     KCHECK();
     if ((rc = S.read_ctrl())) return rc;
-    const double bnorm2 = h->bnorm2;
-
-    stag_cg_stats_t st;
-    memset(&st, 0, sizeof(st));
-    if (bnorm2 == 0.0) {   // b = 0  =>  x = 0, nothing to iterate
-        CU(cudaMemsetAsync(x, 0, (size_t)S.n * sizeof(double), s));
-        CU(cudaEventRecord(L->ev1, s));
-        CU(cudaStreamSynchronize(s));
-        if (stats) *stats = st;
-        return STAG_OK;
+    double bnorm2[MAX_RHS];
+    bool all_zero = true, bad = false;
+    for (int k = 0; k < nrhs; ++k) {
+        bnorm2[k] = h->bnorm2[k];
+        if (bnorm2[k] != 0.0) all_zero = false;
+        if (!(bnorm2[k] == bnorm2[k]) || std::isinf(bnorm2[k])) bad = true;
     }
-    if (!(bnorm2 == bnorm2) || std::isinf(bnorm2)) {
-        if (stats) { st.true_resid = NAN; *stats = st; }
+
+    stag_cg_stats_t zero;
+    memset(&zero, 0, sizeof(zero));
+    if (bad) {
+        for (int k = 0; stats && k < nrhs; ++k) { stats[k] = zero; stats[k].true_resid = NAN; }
         return STAG_EBREAKDOWN;
     }
-    h->tol2b = tol * tol * bnorm2;
+    // b_k = 0  =>  x_k = 0 exactly, nothing to iterate for k (no 0/0)
+    for (int k = 0; k < nrhs; ++k)
+        if (bnorm2[k] == 0.0) CU(cudaMemsetAsync(x + (size_t)k * S.n, 0, vec_bytes, s));
+    if (all_zero) {
+        CU(cudaEventRecord(L->ev1, s));
+        CU(cudaStreamSynchronize(s));
+        for (int k = 0; stats && k < nrhs; ++k) stats[k] = zero;
+        return STAG_OK;
+    }
+    for (int k = 0; k < nrhs; ++k) h->tol2b[k] = tol * tol * bnorm2[k];
     CU(cudaMemcpyAsync(w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, s));
 
     // ---- r = b - A x0 (P:L46 / Fig. 2), in fp64 -------------------------------------
     if ((rc = S.apply_A64(x))) return rc;
     if ((rc = S.residual<RES_INIT>(b, lo))) return rc;
-    if (lo) CU(cudaMemsetAsync(w.y32, 0, (size_t)S.n * sizeof(float), s));
+    if (lo) CU(cudaMemsetAsync(w.y32, 0, (size_t)nrhs * S.n * sizeof(float), s));
     // beta = 0 makes the first xpay d = r without reading d, so d needs no initial value
 
     // ---- the iteration as a CUDA graph of `chunk` passes ----------------------------------
@@ -640,7 +723,7 @@ int cg_solve_device(double *x, const double *b, stag_links *L, double mass, doub
 
     int n_restarts = 0, n_outer = 0;
     int final_state = CG_RUN;
-    bool have_true = true;      // ctrl->sum0 holds |b - A x|^2 for the current x
+    bool have_true = true;      // ctrl->sum0[k] holds |b_k - A x_k|^2 for the current x
     bool verifying = false;     // mode 0: the last launch was the true-residual check of Q6b
     for (;;) {
         if ((rc = S.read_ctrl())) return rc;
@@ -706,32 +789,44 @@ int cg_solve_device(double *x, const double *b, stag_links *L, double mass, doub
     float ms = 0.f;
     CU(cudaEventElapsedTime(&ms, L->ev0, L->ev1));
 
-    st.iters = h->iter;
-    st.n_updates = (mode == STAG_CG_DEFECT) ? n_outer : h->n_updates;
-    st.n_restarts = n_restarts;
-    st.iters_f32 = lo ? h->iter : 0;
-    st.applies_f64 = S.applies_f64;
-    st.true_resid = sqrt(h->sum0 / bnorm2);
-    st.iter_resid = sqrt(h->sum1 / bnorm2);
-    st.seconds = ms * 1e-3;
-    if (stats) *stats = st;
+    bool all_met = true;
+    for (int k = 0; k < nrhs; ++k) {
+        stag_cg_stats_t st = zero;
+        st.iters = h->iters[k];
+        st.n_updates = (mode == STAG_CG_DEFECT) ? n_outer : h->n_updates;
+        st.n_restarts = n_restarts;
+        st.iters_f32 = lo ? h->iters[k] : 0;
+        st.applies_f64 = S.applies_f64;
+        st.true_resid = bnorm2[k] > 0.0 ? sqrt(h->sum0[k] / bnorm2[k]) : 0.0;
+        st.iter_resid = bnorm2[k] > 0.0 ? sqrt(h->sum1[k] / bnorm2[k]) : 0.0;
+        st.seconds = ms * 1e-3;
+        if (!(st.true_resid <= tol)) all_met = false;
+        if (stats) stats[k] = st;
+    }
     if (final_state == CG_BREAKDOWN) return STAG_EBREAKDOWN;
-    if (!(st.true_resid <= tol)) return STAG_ENOCONV;
+    if (!all_met) return STAG_ENOCONV;
     return STAG_OK;
 }
 
 }  // namespace
 
+extern "C" int stag_cg_solve_mrhs(void *x_even, const void *b_even, const stag_links_t *links,
+                                  double mass, double tol, int maxiter, int mode, int nrhs,
+                                  const stag_cg_params_t *params, stag_cg_stats_t *stats_out)
+{
+    stag_links *L = const_cast<stag_links *>(links);
+    if (!x_even || !b_even || !L || x_even == b_even || !(tol > 0.0) || maxiter < 0 || mode < 0 ||
+        mode > 3 || nrhs < 1 || nrhs > MAX_RHS)
+        return STAG_EINVAL;
+    return cg_solve_device((double *)x_even, (const double *)b_even, L, mass, tol, maxiter, mode,
+                           nrhs, params, stats_out);
+}
+
 extern "C" int stag_cg_solve_ex(void *x_even, const void *b_even, const stag_links_t *links,
                                 double mass, double tol, int maxiter, int mode,
                                 const stag_cg_params_t *params, stag_cg_stats_t *stats_out)
 {
-    stag_links *L = const_cast<stag_links *>(links);
-    if (!x_even || !b_even || !L || x_even == b_even || !(tol > 0.0) || maxiter < 0 || mode < 0 ||
-        mode > 3)
-        return STAG_EINVAL;
-    return cg_solve_device((double *)x_even, (const double *)b_even, L, mass, tol, maxiter, mode,
-                           params, stats_out);
+    return stag_cg_solve_mrhs(x_even, b_even, links, mass, tol, maxiter, mode, 1, params, stats_out);
 }
 
 extern "C" int stag_cg_solve(void *x_even, const void *b_even, const stag_links_t *links,
@@ -767,5 +862,34 @@ extern "C" int stag_cg_solve_host(double *x_host, const double *b_host, const st
     if ((rc = stag_spinor_unpack(cx, dx, L->dims, STAG_PREC_F64))) return rc;
     CU(cudaMemcpyAsync(x_host, cx, nc * sizeof(double), cudaMemcpyDeviceToHost, t_stream));
     CU(cudaStreamSynchronize(t_stream));
+    return solve_rc;
+}
+
+// (D + m) psi = h on the whole lattice through the even-site solve (Q23):
+//   b_e = m h_e - D_eo h_o ;  A psi_e = b_e ;  psi_o = (h_o - D_oe psi_e) / m
+// The two extra hops run in fp64 on the 18-real links; b_e lives in scratch on the handle.
+extern "C" int stag_solve_M(void *psi_even, void *psi_odd, const void *h_even, const void *h_odd,
+                            const stag_links_t *links, double mass, double tol, int maxiter,
+                            int mode, int nrhs, const stag_cg_params_t *params,
+                            stag_cg_stats_t *stats_out)
+{
+    stag_links *L = const_cast<stag_links *>(links);
+    if (!psi_even || !psi_odd || !h_even || !h_odd || !L || psi_even == h_even ||
+        psi_odd == h_odd || !(tol > 0.0) || maxiter < 0 || mode < 0 || mode > 3 || nrhs < 1 ||
+        nrhs > MAX_RHS || mass == 0.0)
+        return STAG_EINVAL;
+    int rc;
+    if ((rc = ensure_links(L, STAG_PREC_F64))) return rc;
+    const size_t bytes = (size_t)nrhs * 6 * L->g.Vh_pad * sizeof(double);
+    if (L->wrap_b && L->wrap_b_rhs < nrhs) { CU(cudaFree(L->wrap_b)); L->wrap_b = nullptr; }
+    if (!L->wrap_b) { CU(cudaMalloc(&L->wrap_b, bytes)); L->wrap_b_rhs = nrhs; }
+    // step 1: b_e = m h_e - D_eo h_o
+    if ((rc = launch_hop(L, STAG_PREC_F64, HOP_XPAY, L->wrap_b, h_odd, 0, mass, 1.0, h_even, nullptr, nullptr, nrhs, t_stream))) return rc;
+    // step 2: A psi_e = b_e (psi_even holds the initial guess on entry)
+    const int solve_rc = cg_solve_device((double *)psi_even, (const double *)L->wrap_b, L, mass, tol,
+                                         maxiter, mode, nrhs, params, stats_out);
+    if (solve_rc < 0) return solve_rc;
+    // step 3: psi_o = (1/m) h_o - (1/m) D_oe psi_e
+    if ((rc = launch_hop(L, STAG_PREC_F64, HOP_AXPBY, psi_odd, psi_even, 1, 1.0 / mass, 1.0 / mass, h_odd, nullptr, nullptr, nrhs, t_stream))) return rc;
     return solve_rc;
 }
