@@ -187,6 +187,32 @@ def time_dslash(stag, torch, fieldgen, cfg, L, prec, launches=60, nrot=6):
             "paper_convention_gbs": paper_bytes * cfg.vh / sec * 1e-9}
 
 
+def time_dslash_mrhs(stag, torch, fieldgen, cfg, L, prec, nrhs, launches=30, nrot=3):
+    """The same for a batch of nrhs spinors through stag_dslash_mrhs (links read once per chunk of
+    4 fp32 / 2 fp64 right-hand sides)."""
+    srcs = [fieldgen.spinor_gaussian(cfg.dims, 0, seed=300 + k) for k in range(nrhs)]
+    ins = [stag.spinor_pack_mrhs(srcs, cfg.dims, prec) for _ in range(nrot)]
+    outs = [torch.empty_like(ins[0]) for _ in range(nrot)]
+    for i in range(3):
+        stag.dslash_mrhs(ins[i % nrot], L, 1, prec, out=outs[i % nrot])
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(launches):
+        stag.dslash_mrhs(ins[i % nrot], L, 1, prec, out=outs[i % nrot])
+    e1.record()
+    torch.cuda.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3 / launches
+    f32 = prec in (stag.PREC_F32, stag.PREC_F32_R12)
+    rows = 2 if prec in (stag.PREC_F64_R12, stag.PREC_F32_R12) else 3
+    sz = 4 if f32 else 8
+    chunks = -(-nrhs // (4 if f32 else 2))
+    bytes_site = (chunks * 8 * 6 * rows + nrhs * 12) * sz       # links once per chunk + in/out per rhs
+    return {"nrhs": nrhs, "us": sec * 1e6, "us_per_rhs": sec * 1e6 / nrhs,
+            "algorithmic_bytes_per_site": bytes_site, "gbs": bytes_site * cfg.vh / sec * 1e-9,
+            "gflops": FLOP_PER_SITE_HOP * nrhs * cfg.vh / sec * 1e-9}
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -263,6 +289,19 @@ def run_ours(args):
     x64, st64 = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_F64)
     x18, st18 = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE)
 
+    # several right-hand sides sharing each pass over the links: three
+    # Gaussian sources in lockstep, and the batch hop alone
+    b3 = stag.spinor_pack_mrhs([fieldgen.spinor_gaussian(cfg.dims, 0, seed + 1000 + k) for k in range(3)],
+                               cfg.dims, stag.PREC_F64)
+    x3, st3 = stag.cg_solve_mrhs(b3, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True)
+    mrhs = {"nrhs": 3, "iters": [t["iters"] for t in st3], "true_resid": [t["true_resid"] for t in st3],
+            "time_to_solution_s": st3[0]["seconds"],
+            "gflops": sum(t["iters"] for t in st3) * FLOP_PER_SITE_ITER * cfg.vh / st3[0]["seconds"] * 1e-9,
+            "us_per_iteration_per_rhs": st3[0]["seconds"] / max(1, max(t["iters"] for t in st3)) / 3 * 1e6,
+            "dslash": {"%s x%d" % (stag.PREC_NAMES[p], n): time_dslash_mrhs(stag, torch, fieldgen, cfg, L, p, n)
+                       for p, n in ((stag.PREC_F32_R12, 3), (stag.PREC_F32_R12, 4), (stag.PREC_F32, 4), (stag.PREC_F64, 2))}}
+    del b3, x3
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         r = oracle_sample(cfg, W, b_np, 15.0)
@@ -292,6 +331,7 @@ def run_ours(args):
                                       "ms_per_iteration": st18["seconds"] / max(1, st18["iters"]) * 1e3},
                "speedup_mixed_vs_fp64": st64["seconds"] / st["seconds"]},
         "dslash": dsl,
+        "mrhs": mrhs,
         "setup_s0_seconds": setup_s,
         "paper_context": "GTX480: 145 GFLOPS SP / 55 DP per GPU pure-GPU CG (P:L131), 1.04 / 2.77 ms per Dirac op on a quarter lattice (Table 1)",
     }

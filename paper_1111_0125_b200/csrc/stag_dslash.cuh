@@ -62,7 +62,7 @@ __device__ __forceinline__ void rebuild_row2(cplx_t<T> *m, bool neg)
 // (profiles/README.md): MINB = resident blocks per SM promised to ptxas, GM = directions' worth
 // of packets loaded ahead (group = K*GM packets).  With N > 1 right-hand sides the registers go
 // to the N accumulators and the N neighbour vectors of one group instead.
-template <typename T, int NR, int N> struct HopTune { static constexpr int MINB = (N == 1) ? 4 : 3, GM = 1; };
+template <typename T, int NR, int N> struct HopTune { static constexpr int MINB = 4, GM = 1; };
 template <> struct HopTune<float, 2, 1>            { static constexpr int MINB = 6, GM = 2; };
 template <int N> struct HopTune<double, 3, N>      { static constexpr int MINB = (N == 1) ? 4 : 2, GM = 1; };
 template <int N> struct HopTune<double, 2, N>      { static constexpr int MINB = (N == 1) ? 4 : 2, GM = 1; };
