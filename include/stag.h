@@ -116,6 +116,13 @@ void stag_reset_launch_count(void);
  * The fp64/18 form is built by this call; the other three are built on first use. */
 int stag_links_create(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
                       const double *W, int on_device);
+/* The same from the BARE gauge field U_mu(x) (same layout, no phases): eta_mu(x) =
+ * (-1)^(x0+..+x_{mu-1}) and, when antiperiodic_t, the -1 on the mu=3 links leaving x3 = X3-1
+ * are folded in on the device while gathering -- the paper's "gauge link preconditioning"
+ * done by the library instead of the caller.  Multiplication by +-1 is exact: the
+ * handle is bit-identical to the one stag_links_create builds from the folded field. */
+int stag_links_create_unfolded(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
+                               const double *U, int on_device);
 void stag_links_destroy(stag_links_t *links);
 
 /* Largest | row2 - s conj(row0 x row1) | over all links, measured when the handle was made.

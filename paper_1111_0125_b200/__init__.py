@@ -94,6 +94,7 @@ SIGNATURES = {
     "stag_launch_count": (ctypes.c_ulonglong, []),
     "stag_reset_launch_count": (None, []),
     "stag_links_create": (ctypes.c_int, [ctypes.POINTER(_vp), _ip, ctypes.c_int, _vp, ctypes.c_int]),
+    "stag_links_create_unfolded": (ctypes.c_int, [ctypes.POINTER(_vp), _ip, ctypes.c_int, _vp, ctypes.c_int]),
     "stag_links_destroy": (None, [_vp]),
     "stag_links_recon_error": (ctypes.c_int, [_vp, _dp]),
     "stag_spinor_bytes": (ctypes.c_size_t, [_ip, ctypes.c_int]),
@@ -194,7 +195,9 @@ class Links:
     """Owner of a stag_links_t handle.  W: canonical complex128 [4][2][Vh][3][3] (numpy, host)
     or a CUDA float64 tensor holding the same 4*2*Vh*18 doubles."""
 
-    def __init__(self, dims, W, antiperiodic_t: bool = True):
+    def __init__(self, dims, W, antiperiodic_t: bool = True, folded: bool = True):
+        """folded=False: W is the bare U; eta and the time boundary sign are folded in on the
+        device (stag_links_create_unfolded)."""
         torch = _require_cuda()
         use_current_stream()
         self.dims = tuple(int(v) for v in dims)
@@ -215,8 +218,8 @@ class Links:
                 raise ValueError("host W must have shape (4,2,Vh,3,3)")
             ptr, on_dev = ctypes.c_void_p(W.ctypes.data), 0
         self._keep = W
-        _check(lib().stag_links_create(ctypes.byref(self._h), _cdims(self.dims),
-                                       int(bool(antiperiodic_t)), ptr, on_dev))
+        create = lib().stag_links_create if folded else lib().stag_links_create_unfolded
+        _check(create(ctypes.byref(self._h), _cdims(self.dims), int(bool(antiperiodic_t)), ptr, on_dev))
         torch.cuda.current_stream().synchronize()
         self._keep = None
 

@@ -110,11 +110,15 @@ size_t links_elems(const stag_links *L, int rows)   // complex numbers in one ga
 
 // ---- S0 kernels ----------------------------------------------------------------------
 
-// canonical W[mu][p][cb][3][3] (fp64, eta*bc folded) -> gathered fp64/18 field
-// L[p][tile][d][k][lane]; also measures how well row 2 is rebuilt from rows 0,1 (Q12).
+// canonical W[mu][p][cb][3][3] (fp64) -> gathered fp64/18 field L[p][tile][d][k][lane]; also
+// measures how well row 2 is rebuilt from rows 0,1 (Q12).  fold = 0: W already carries
+// eta*bc (the caller folded it); fold = 1: W is the bare U and each link is multiplied
+// here by eta_mu(x') bc_mu(x') of ITS OWN site x' (x for the forward link, x - mu^ for the
+// backward one), the device-side form of the paper's "gauge link preconditioning".
+// The sign comes from det_sign_mask: det M_d = eta bc for d < 4 and -(eta bc) for d >= 4.
 __global__ void __launch_bounds__(128)
 gather_links_kernel(double2 *__restrict__ L, const double *__restrict__ W, const Geom g,
-                    unsigned long long *__restrict__ err_bits)
+                    unsigned long long *__restrict__ err_bits, const int fold)
 {
     const long idx = blockIdx.x * 128L + threadIdx.x;
     if (idx >= 2L * g.Vh_pad) return;
@@ -139,6 +143,11 @@ gather_links_kernel(double2 *__restrict__ L, const double *__restrict__ W, const
             for (int i = 0; i < 3; ++i)
                 for (int j = 0; j < 3; ++j)   // M = -W^dag : M_ij = -conj(W_ji)
                     m[3 * i + j] = make_double2(-src[2 * (3 * j + i)], src[2 * (3 * j + i) + 1]);
+        }
+        if (fold) {
+            const bool det_neg = (neg >> d) & 1u;
+            const double sg = (d < 4) ? (det_neg ? -1.0 : 1.0) : (det_neg ? 1.0 : -1.0);
+            for (int k = 0; k < 9; ++k) { m[k].x *= sg; m[k].y *= sg; }
         }
         for (int k = 0; k < 9; ++k) dst[(d * 9 + k) * TILE] = m[k];
         double2 t[9];
@@ -355,8 +364,23 @@ extern "C" void stag_reset_launch_count(void) { g_launches.store(0); }
 // ------------------------------------------------------------------------------------
 // C ABI: links
 // ------------------------------------------------------------------------------------
+static int links_create(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
+                        const double *W, int on_device, int fold);
+
 extern "C" int stag_links_create(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
                                  const double *W, int on_device)
+{
+    return links_create(links_out, dims, antiperiodic_t, W, on_device, 0);
+}
+
+extern "C" int stag_links_create_unfolded(stag_links_t **links_out, const int dims[4],
+                                          int antiperiodic_t, const double *U, int on_device)
+{
+    return links_create(links_out, dims, antiperiodic_t, U, on_device, 1);
+}
+
+static int links_create(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
+                        const double *W, int on_device, int fold)
 {
     if (!links_out || !W) return STAG_EINVAL;
     *links_out = nullptr;
@@ -383,7 +407,7 @@ extern "C" int stag_links_create(stag_links_t **links_out, const int dims[4], in
         if ((e = cudaMalloc(&err, sizeof(*err))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(err)", __LINE__); break; }
         if ((e = cudaMemsetAsync(err, 0, sizeof(*err), t_stream)) != cudaSuccess) { rc = cuda_fail(e, "cudaMemsetAsync", __LINE__); break; }
         const unsigned grid = (unsigned)((2L * g.Vh_pad + 127) / 128);
-        gather_links_kernel<<<grid, 128, 0, t_stream>>>((double2 *)L->L[STAG_PREC_F64], on_device ? W : Wd, g, err);
+        gather_links_kernel<<<grid, 128, 0, t_stream>>>((double2 *)L->L[STAG_PREC_F64], on_device ? W : Wd, g, err, fold);
         count_launch();
         if ((e = cudaGetLastError()) != cudaSuccess) { rc = cuda_fail(e, "gather_links_kernel", __LINE__); break; }
         unsigned long long bits = 0;
