@@ -169,6 +169,47 @@ int stag_dslash_mrhs(void *out, const void *in, const stag_links_t *links, int p
 int stag_apply_A_mrhs(void *out_even, const void *in_even, const stag_links_t *links, double mass,
                       int prec, int nrhs);
 
+/* ---- T-slabs: the hop on a lattice split along time over several GPUs --------------------
+ *
+ * The paper's subject is the multi-GPU Dirac operation: kernel, boundary collect, memcpy to the
+ * host, MPI, memcpy back (Table 1), with GPU-to-GPU copies planned.  Here
+ * rank r of nranks holds time slices [r*X3/nranks, (r+1)*X3/nranks) of the global lattice
+ * (X3/nranks even); one process per GPU.  A slab handle owns its gathered links (the backward
+ * t-links of its first slice included, so links are never exchanged) and an EXCHANGE REGION: two
+ * flags and double-buffered halo buffers for the neighbour slices x3 = -1 and x3 = X3 of a
+ * hop's input spinor.  stag_slab_push stores the slab's last / first slice of `in` directly into
+ * the forward / backward neighbour's halo (peer-to-peer stores) and then release-stores the
+ * exchange number into their flags; stag_slab_hop computes the slab's hop, its boundary-slice
+ * threads (visited last) acquire-waiting on the slab's own flags.  All ranks must issue the same
+ * sequence of pushes and hops.  Spinors are ordinary device spinors of the LOCAL dims.
+ *
+ * Wiring: every rank publishes its region (stag_slab_ipc_handle, 64 bytes, to be exchanged by
+ * any means, e.g. torch.distributed), opens its two neighbours' (stag_slab_ipc_open) and calls
+ * stag_slab_connect.  Slabs living in one process connect with the raw pointers from
+ * stag_slab_info.  nranks = 1 connects to itself.  DESIGN.md section 14. */
+#define STAG_IPC_HANDLE_BYTES 64
+
+/* W_global: canonical fp64 links of the WHOLE lattice global_dims (eta*bc folded). */
+int stag_slab_create(stag_links_t **slab_out, const int global_dims[4], int antiperiodic_t,
+                     const double *W_global, int on_device, int rank, int nranks);
+/* Any output pointer may be NULL. */
+int stag_slab_info(const stag_links_t *slab, int local_dims_out[4], int *rank_out, int *nranks_out,
+                   void **exchange_ptr_out, size_t *exchange_bytes_out);
+int stag_slab_ipc_handle(const stag_links_t *slab, unsigned char handle_out[STAG_IPC_HANDLE_BYTES]);
+int stag_slab_ipc_open(const unsigned char handle[STAG_IPC_HANDLE_BYTES], void **ptr_out);
+int stag_slab_ipc_close(void *ptr);
+/* bwd / fwd: device-accessible addresses of the exchange regions of ranks r-1 and r+1 (mod nranks) */
+int stag_slab_connect(stag_links_t *slab, void *bwd_exchange, void *fwd_exchange);
+
+/* Start exchange number e = (pushes so far) + 1 with the faces of `in` (one parity, precision of prec). */
+int stag_slab_push(const void *in, stag_links_t *slab, int prec);
+/* out (sites of `parity`) = D in on the slab, halo from the last exchange; with own != NULL,
+ * out = a*own - D in (the second hop of A, a = m^2).  STAG_EINVAL before the first push. */
+int stag_slab_hop(void *out, const void *in, stag_links_t *slab, int parity, int prec, double a,
+                  const void *own);
+/* push + hop: what each rank of a real multi-GPU run calls. */
+int stag_slab_dslash(void *out, const void *in, stag_links_t *slab, int parity, int prec);
+
 /* ---- the solver -------------------------------------------------------- */
 
 /* Optional knobs for stag_cg_solve_ex; zero-initialise, then set what you need

@@ -114,6 +114,16 @@ SIGNATURES = {
     "stag_solve_M": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_double,
                                     ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Params),
                                     ctypes.POINTER(_Stats)]),
+    "stag_slab_create": (ctypes.c_int, [ctypes.POINTER(_vp), _ip, ctypes.c_int, _vp, ctypes.c_int,
+                                        ctypes.c_int, ctypes.c_int]),
+    "stag_slab_info": (ctypes.c_int, [_vp, _ip, _ip, _ip, ctypes.POINTER(_vp), ctypes.POINTER(ctypes.c_size_t)]),
+    "stag_slab_ipc_handle": (ctypes.c_int, [_vp, ctypes.c_char_p]),
+    "stag_slab_ipc_open": (ctypes.c_int, [ctypes.c_char_p, ctypes.POINTER(_vp)]),
+    "stag_slab_ipc_close": (ctypes.c_int, [_vp]),
+    "stag_slab_connect": (ctypes.c_int, [_vp, _vp, _vp]),
+    "stag_slab_push": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
+    "stag_slab_hop": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, ctypes.c_int, ctypes.c_double, _vp]),
+    "stag_slab_dslash": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, ctypes.c_int]),
     "stag_cg_solve_host": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double,
                                           ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Params),
                                           ctypes.POINTER(_Stats)]),

@@ -17,6 +17,8 @@ struct Geom {
     int Vh, Vh_pad;        // sites per parity, rounded up to TILE
     int s1, s2, s3;        // checkerboard strides of mu = 1,2,3
     int antiperiodic;      // caller folded bc = -1 into W_3 at x3 = X3-1 (only 12-real needs it)
+    int t0, X3g;           // T-slab of a larger lattice (stag_slab_*): this lattice is time slices
+                           // [t0, t0+X3) of a global extent X3g; a whole lattice has t0 = 0, X3g = X3
 };
 
 inline bool make_geom(Geom &g, const int dims[4], int antiperiodic)
@@ -33,6 +35,7 @@ inline bool make_geom(Geom &g, const int dims[4], int antiperiodic)
     g.Vh_pad = (g.Vh + TILE - 1) / TILE * TILE;
     g.s1 = g.X0h; g.s2 = g.X0h * g.X1; g.s3 = g.X0h * g.X1 * g.X2;
     g.antiperiodic = antiperiodic ? 1 : 0;
+    g.t0 = 0; g.X3g = g.X3;
     return true;
 }
 
@@ -102,8 +105,8 @@ __device__ __forceinline__ unsigned det_sign_mask(const Geom &g, const Site &s)
     const unsigned e1 = (unsigned)s.x0 & 1u;
     const unsigned e2 = (unsigned)(s.x0 + s.x1) & 1u;
     const unsigned e3 = (unsigned)(s.x0 + s.x1 + s.x2) & 1u;
-    const unsigned bf = (g.antiperiodic && s.x3 == g.X3 - 1) ? 1u : 0u;
-    const unsigned bb = (g.antiperiodic && s.x3 == 0) ? 1u : 0u;
+    const unsigned bf = (g.antiperiodic && s.x3 + g.t0 == g.X3g - 1) ? 1u : 0u;   // global time
+    const unsigned bb = (g.antiperiodic && s.x3 + g.t0 == 0) ? 1u : 0u;
     unsigned m = 0;
     m |= 0u << 0;                 // eta_0 = +1
     m |= e1 << 1;

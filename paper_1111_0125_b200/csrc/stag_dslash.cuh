@@ -72,6 +72,25 @@ template <typename T> struct HopMaxRhs;
 template <> struct HopMaxRhs<float>  { static constexpr int value = 4; };
 template <> struct HopMaxRhs<double> { static constexpr int value = 2; };
 
+// ---- T-slab halo (stag_slab_*) ------------------------------------
+// A slab is time slices [t0, t0+X3) of a larger lattice held by one GPU.  The neighbour slices
+// x3 = -1 and x3 = X3 of the INPUT spinor live in two halo buffers, [colour][s3] complex each,
+// that the neighbouring GPUs fill with peer-to-peer stores (face_push_kernel) and then mark by
+// storing the exchange's epoch into flag_back / flag_fwd with system-scope release.
+template <typename T> struct HaloArgs {
+    const cplx_t<T> *back, *fwd;
+    const unsigned long long *flag_back, *flag_fwd;
+    unsigned long long epoch;
+};
+
+__device__ __forceinline__ void wait_flag(const unsigned long long *f, unsigned long long epoch)
+{
+    unsigned long long v;
+    do {
+        asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(f) : "memory");
+    } while (v < epoch);
+}
+
 // T: float or double.  NR: rows of each link held in memory (3 = 18-real, 2 = 12-real).
 // N: right-hand sides handled by one thread; spinor k of a batch starts rs complex numbers after
 // spinor k-1 (rs = 3*Vh_pad: the batch is N device spinors back to back).
@@ -82,13 +101,18 @@ template <> struct HopMaxRhs<double> { static constexpr int value = 2; };
 // partials: HOP_XPAY_DOT writes sum over the block of Re<own,out> (fp64) of right-hand
 // side k to partials[k*gridDim.x + blockIdx.x]; the kernel that needs <d,Ad> adds them in index
 // order (stag_blas.cuh).
-template <typename T, int NR, int MODE, int N>
+// HALO (N = 1 only): the lattice is a T-slab; the +-t neighbours of the first and last time
+// slice come from the halo buffers once their flag shows this exchange's epoch.  Sites are
+// visited rotated by one time slice (slices 1 .. X3-1, then slice 0), so the blocks that may
+// have to wait for a neighbouring GPU run last and the interior overlaps the exchange.
+template <typename T, int NR, int MODE, int N, bool HALO = false>
 __global__ void __launch_bounds__(DSLASH_BLOCK, HopTune<T, NR, N>::MINB)
 dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
               const pkt_t<T> *__restrict__ links, const Geom g, const int p, const T a, const T cD,
               const cplx_t<T> *__restrict__ own, double *__restrict__ partials,
-              const CgCtrl *__restrict__ ctrl)
+              const CgCtrl *__restrict__ ctrl, const HaloArgs<T> halo)
 {
+    static_assert(!HALO || N == 1, "slab hops carry one right-hand side");
     using C = cplx_t<T>;
     using P = pkt_t<T>;
     constexpr int K = 3 * NR;
@@ -99,7 +123,13 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
     static_assert(8 % DPG == 0, "group must divide the eight directions");
     if (ctrl != nullptr && ctrl->state != CG_RUN) return;
 
-    const int cb = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
+    int cb = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
+    if constexpr (HALO) {
+        if (cb < g.Vh_pad) {
+            cb += g.s3;
+            if (cb >= g.Vh_pad) cb -= g.Vh_pad;
+        }
+    }
     const size_t rs = (size_t)3 * g.Vh_pad;
     double dot[N];
 #pragma unroll
@@ -122,6 +152,21 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
             for (int d = 0; d < 8; ++d)
 #pragma unroll
                 for (int c = 0; c < 3; ++c) v1[d][c] = ld_keep_nc(in + (size_t)c * g.Vh_pad + s.nbr[d]);
+            if constexpr (HALO) {
+                // decode_site wrapped the +-t neighbours of the boundary slices onto the slab's
+                // own other end; their in-slice index is what addresses the halo buffers
+                if (s.x3 == g.X3 - 1) {
+                    wait_flag(halo.flag_fwd, halo.epoch);
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) v1[3][c] = __ldcg(halo.fwd + (size_t)c * g.s3 + s.nbr[3]);
+                }
+                if (s.x3 == 0) {
+                    wait_flag(halo.flag_back, halo.epoch);
+#pragma unroll
+                    for (int c = 0; c < 3; ++c)
+                        v1[7][c] = __ldcg(halo.back + (size_t)c * g.s3 + (s.nbr[7] - (g.X3 - 1) * g.s3));
+                }
+            }
         }
 
         C acc[N][3];

@@ -10,6 +10,7 @@
 #include "stag_blas.cuh"
 #include "stag_common.cuh"
 #include "stag_dslash.cuh"
+#include "stag_slab.cuh"
 
 using namespace stag;
 
@@ -82,7 +83,10 @@ int blas_grid(long n_reals, int nrhs)
 // ------------------------------------------------------------------------------------
 struct stag_links {
     Geom g;
-    int dims[4];
+    int dims[4];           // extents of the lattice this handle covers (the slab's, for a slab)
+    int gdims[4];          // extents of the whole lattice
+    int rank, nranks;      // T-slab: time slices [rank*X3, (rank+1)*X3) of nranks*X3; else 0, 1
+    int is_slab;           // made by stag_slab_create: operator calls go through stag_slab_*
     int ntiles;            // Vh_pad / TILE
     void *L[4];            // gathered link fields by precision enum; L[STAG_PREC_F64] always set
     double recon_err;
@@ -96,6 +100,11 @@ struct stag_links {
     cudaStream_t cap_stream;
     // staging for stag_cg_solve_host (lazy)
     double *stage_dev;     // 2 canonical spinors + 2 device-layout fp64 spinors
+    // T-slab exchange (stag_slab_*): my exchange region, the neighbours' (peer memory), and the
+    // number of exchanges started so far
+    char *xch;
+    char *peer_bwd, *peer_fwd;
+    unsigned long long epoch;
     void *wrap_b;          // stag_solve_M: b_e of the even-site system, wrap_b_rhs spinors (lazy)
     int wrap_b_rhs;
     cudaEvent_t ev0, ev1;
@@ -116,9 +125,13 @@ size_t links_elems(const stag_links *L, int rows)   // complex numbers in one ga
 // here by eta_mu(x') bc_mu(x') of ITS OWN site x' (x for the forward link, x - mu^ for the
 // backward one), the device-side form of the paper's "gauge link preconditioning".
 // The sign comes from det_sign_mask: det M_d = eta bc for d < 4 and -(eta bc) for d >= 4.
+// g is the geometry of the lattice the handle covers, gg that of the lattice W covers: the same
+// for a whole-lattice handle; for a T-slab (stag_slab_create) g is the slab (time slices
+// [g.t0, g.t0 + g.X3) of gg) and every link, including the backward t-links of the slab's first
+// slice that belong to the neighbouring slab, is read from the whole field.
 __global__ void __launch_bounds__(128)
 gather_links_kernel(double2 *__restrict__ L, const double *__restrict__ W, const Geom g,
-                    unsigned long long *__restrict__ err_bits, const int fold)
+                    const Geom gg, unsigned long long *__restrict__ err_bits, const int fold)
 {
     const long idx = blockIdx.x * 128L + threadIdx.x;
     if (idx >= 2L * g.Vh_pad) return;
@@ -129,17 +142,19 @@ gather_links_kernel(double2 *__restrict__ L, const double *__restrict__ W, const
         for (int k = 0; k < 72; ++k) dst[k * TILE] = make_double2(0.0, 0.0);
         return;
     }
+    // time slices are contiguous in the checkerboard index: global cb = local cb + t0 * s3
+    const int cbg = cb + g.t0 * g.s3;
     Site s;
-    decode_site(g, p, cb, s);
-    const unsigned neg = det_sign_mask(g, s);
+    decode_site(gg, p, cbg, s);                 // global coordinates and global neighbours
+    const unsigned neg = det_sign_mask(gg, s);
     double worst = 0.0;
     for (int d = 0; d < 8; ++d) {
         double2 m[9];
         if (d < 4) {
-            const double *src = W + (((size_t)d * 2 + p) * g.Vh + cb) * 18;
+            const double *src = W + (((size_t)d * 2 + p) * gg.Vh + cbg) * 18;
             for (int k = 0; k < 9; ++k) m[k] = make_double2(src[2 * k], src[2 * k + 1]);
         } else {
-            const double *src = W + (((size_t)(d - 4) * 2 + (1 - p)) * g.Vh + s.nbr[d]) * 18;
+            const double *src = W + (((size_t)(d - 4) * 2 + (1 - p)) * gg.Vh + s.nbr[d]) * 18;
             for (int i = 0; i < 3; ++i)
                 for (int j = 0; j < 3; ++j)   // M = -W^dag : M_ij = -conj(W_ji)
                     m[3 * i + j] = make_double2(-src[2 * (3 * j + i)], src[2 * (3 * j + i) + 1]);
@@ -264,19 +279,19 @@ int launch_hop_n(const stag_links *L, int prec, int hop, cplx_t<T> *out, const c
     const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
     switch (hop) {
     case HOP_PLAIN:
-        dslash_kernel<T, NR, HOP_PLAIN, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl);
+        dslash_kernel<T, NR, HOP_PLAIN, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl, HaloArgs<T>{});
         break;
     case HOP_XPAY:
-        dslash_kernel<T, NR, HOP_XPAY, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl);
+        dslash_kernel<T, NR, HOP_XPAY, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl, HaloArgs<T>{});
         break;
     case HOP_AXPBY:   // only the fp64 wrapper steps use it
         if constexpr (std::is_same<T, double>::value)
-            dslash_kernel<T, NR, HOP_AXPBY, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl);
+            dslash_kernel<T, NR, HOP_AXPBY, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl, HaloArgs<T>{});
         else
             return STAG_EINVAL;
         break;
     default:
-        dslash_kernel<T, NR, HOP_XPAY_DOT, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl);
+        dslash_kernel<T, NR, HOP_XPAY_DOT, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl, HaloArgs<T>{});
         break;
     }
     count_launch();
@@ -365,35 +380,44 @@ extern "C" void stag_reset_launch_count(void) { g_launches.store(0); }
 // C ABI: links
 // ------------------------------------------------------------------------------------
 static int links_create(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
-                        const double *W, int on_device, int fold);
+                        const double *W, int on_device, int fold, int rank, int nranks);
 
 extern "C" int stag_links_create(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
                                  const double *W, int on_device)
 {
-    return links_create(links_out, dims, antiperiodic_t, W, on_device, 0);
+    return links_create(links_out, dims, antiperiodic_t, W, on_device, 0, 0, 1);
 }
 
 extern "C" int stag_links_create_unfolded(stag_links_t **links_out, const int dims[4],
                                           int antiperiodic_t, const double *U, int on_device)
 {
-    return links_create(links_out, dims, antiperiodic_t, U, on_device, 1);
+    return links_create(links_out, dims, antiperiodic_t, U, on_device, 1, 0, 1);
 }
 
+// dims: the lattice W covers.  nranks > 1 (or slab != 0): the handle covers time slices
+// [rank*X3/nranks, (rank+1)*X3/nranks) only and is a T-slab (exchange region allocated).
 static int links_create(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
-                        const double *W, int on_device, int fold)
+                        const double *W, int on_device, int fold, int rank, int nranks)
 {
     if (!links_out || !W) return STAG_EINVAL;
     *links_out = nullptr;
-    Geom g;
-    if (!make_geom(g, dims, antiperiodic_t)) return STAG_EINVAL;
+    Geom gg, g;
+    if (!make_geom(gg, dims, antiperiodic_t)) return STAG_EINVAL;
+    if (nranks < 1 || rank < 0 || rank >= nranks || dims[3] % nranks) return STAG_EINVAL;
+    const int ldims[4] = { dims[0], dims[1], dims[2], dims[3] / nranks };
+    if (!make_geom(g, ldims, antiperiodic_t)) return STAG_EINVAL;     // local extent even, >= 2
+    g.t0 = rank * ldims[3];
+    g.X3g = dims[3];
     stag_links *L = new (std::nothrow) stag_links();
     if (!L) return STAG_ENOMEM;
     memset(L, 0, sizeof(*L));
     L->g = g;
-    for (int m = 0; m < 4; ++m) L->dims[m] = dims[m];
+    for (int m = 0; m < 4; ++m) { L->dims[m] = ldims[m]; L->gdims[m] = dims[m]; }
+    L->rank = rank;
+    L->nranks = nranks;
     L->ntiles = g.Vh_pad / TILE;
 
-    const size_t canon_bytes = (size_t)4 * 2 * g.Vh * 18 * sizeof(double);
+    const size_t canon_bytes = (size_t)4 * 2 * gg.Vh * 18 * sizeof(double);
     double *Wd = nullptr;
     unsigned long long *err = nullptr;
     int rc = STAG_OK;
@@ -407,7 +431,7 @@ static int links_create(stag_links_t **links_out, const int dims[4], int antiper
         if ((e = cudaMalloc(&err, sizeof(*err))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(err)", __LINE__); break; }
         if ((e = cudaMemsetAsync(err, 0, sizeof(*err), t_stream)) != cudaSuccess) { rc = cuda_fail(e, "cudaMemsetAsync", __LINE__); break; }
         const unsigned grid = (unsigned)((2L * g.Vh_pad + 127) / 128);
-        gather_links_kernel<<<grid, 128, 0, t_stream>>>((double2 *)L->L[STAG_PREC_F64], on_device ? W : Wd, g, err, fold);
+        gather_links_kernel<<<grid, 128, 0, t_stream>>>((double2 *)L->L[STAG_PREC_F64], on_device ? W : Wd, g, gg, err, fold);
         count_launch();
         if ((e = cudaGetLastError()) != cudaSuccess) { rc = cuda_fail(e, "gather_links_kernel", __LINE__); break; }
         unsigned long long bits = 0;
@@ -433,6 +457,7 @@ extern "C" void stag_links_destroy(stag_links_t *L)
     if (L->h_ctrl) cudaFreeHost(L->h_ctrl);
     if (L->stage_dev) cudaFree(L->stage_dev);
     if (L->wrap_b) cudaFree(L->wrap_b);
+    if (L->xch) cudaFree(L->xch);
     if (L->cap_stream) cudaStreamDestroy(L->cap_stream);
     if (L->ev0) cudaEventDestroy(L->ev0);
     if (L->ev1) cudaEventDestroy(L->ev1);
@@ -488,7 +513,7 @@ extern "C" int stag_dslash_mrhs(void *out, const void *in, const stag_links_t *l
 {
     stag_links *L = const_cast<stag_links *>(links);
     if (!out || !in || !L || out == in || (parity & ~1) || !prec_ok(prec) || !same_dims(L, dims) ||
-        nrhs < 1)
+        nrhs < 1 || L->is_slab)      // a slab's hop needs its halo: stag_slab_hop
         return STAG_EINVAL;
     int rc = ensure_links(L, prec);
     if (rc) return rc;
@@ -505,7 +530,7 @@ extern "C" int stag_apply_A_mrhs(void *out_even, const void *in_even, const stag
                                  double mass, int prec, int nrhs)
 {
     stag_links *L = const_cast<stag_links *>(links);
-    if (!out_even || !in_even || !L || out_even == in_even || !prec_ok(prec) || nrhs < 1)
+    if (!out_even || !in_even || !L || out_even == in_even || !prec_ok(prec) || nrhs < 1 || L->is_slab)
         return STAG_EINVAL;
     int rc = ensure_links(L, prec);
     if (rc) return rc;
@@ -840,7 +865,7 @@ extern "C" int stag_cg_solve_mrhs(void *x_even, const void *b_even, const stag_l
 {
     stag_links *L = const_cast<stag_links *>(links);
     if (!x_even || !b_even || !L || x_even == b_even || !(tol > 0.0) || maxiter < 0 || mode < 0 ||
-        mode > 3 || nrhs < 1 || nrhs > MAX_RHS)
+        mode > 3 || nrhs < 1 || nrhs > MAX_RHS || L->is_slab)
         return STAG_EINVAL;
     return cg_solve_device((double *)x_even, (const double *)b_even, L, mass, tol, maxiter, mode,
                            nrhs, params, stats_out);
@@ -900,7 +925,7 @@ extern "C" int stag_solve_M(void *psi_even, void *psi_odd, const void *h_even, c
     stag_links *L = const_cast<stag_links *>(links);
     if (!psi_even || !psi_odd || !h_even || !h_odd || !L || psi_even == h_even ||
         psi_odd == h_odd || !(tol > 0.0) || maxiter < 0 || mode < 0 || mode > 3 || nrhs < 1 ||
-        nrhs > MAX_RHS || mass == 0.0)
+        nrhs > MAX_RHS || mass == 0.0 || L->is_slab)
         return STAG_EINVAL;
     int rc;
     if ((rc = ensure_links(L, STAG_PREC_F64))) return rc;
@@ -916,4 +941,145 @@ extern "C" int stag_solve_M(void *psi_even, void *psi_odd, const void *h_even, c
     // step 3: psi_o = (1/m) h_o - (1/m) D_oe psi_e
     if ((rc = launch_hop(L, STAG_PREC_F64, HOP_AXPBY, psi_odd, psi_even, 1, 1.0 / mass, 1.0 / mass, h_odd, nullptr, nullptr, nrhs, t_stream))) return rc;
     return solve_rc;
+}
+
+// ------------------------------------------------------------------------------------
+// C ABI: T-slab decomposition (include/stag.h "T-slabs"; stag_slab.cuh)
+// ------------------------------------------------------------------------------------
+extern "C" int stag_slab_create(stag_links_t **slab_out, const int global_dims[4], int antiperiodic_t,
+                                const double *W_global, int on_device, int rank, int nranks)
+{
+    int rc = links_create(slab_out, global_dims, antiperiodic_t, W_global, on_device, 0, rank, nranks);
+    if (rc) return rc;
+    stag_links *L = *slab_out;
+    L->is_slab = 1;
+    const size_t bytes = xch_bytes(L->g.s3);
+    cudaError_t e = cudaMalloc((void **)&L->xch, bytes);
+    if (e == cudaSuccess) e = cudaMemsetAsync(L->xch, 0, bytes, t_stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(t_stream);
+    if (e != cudaSuccess) { rc = cuda_fail(e, "slab exchange region", __LINE__); stag_links_destroy(L); *slab_out = nullptr; return rc; }
+    if (nranks == 1) L->peer_bwd = L->peer_fwd = L->xch;     // periodic wrap through my own halo
+    return STAG_OK;
+}
+
+extern "C" int stag_slab_info(const stag_links_t *L, int local_dims_out[4], int *rank_out,
+                              int *nranks_out, void **exchange_ptr_out, size_t *exchange_bytes_out)
+{
+    if (!L || !L->is_slab) return STAG_EINVAL;
+    if (local_dims_out) for (int m = 0; m < 4; ++m) local_dims_out[m] = L->dims[m];
+    if (rank_out) *rank_out = L->rank;
+    if (nranks_out) *nranks_out = L->nranks;
+    if (exchange_ptr_out) *exchange_ptr_out = L->xch;
+    if (exchange_bytes_out) *exchange_bytes_out = xch_bytes(L->g.s3);
+    return STAG_OK;
+}
+
+static_assert(sizeof(cudaIpcMemHandle_t) == STAG_IPC_HANDLE_BYTES, "IPC handle size");
+
+extern "C" int stag_slab_ipc_handle(const stag_links_t *L, unsigned char handle_out[STAG_IPC_HANDLE_BYTES])
+{
+    if (!L || !L->is_slab || !handle_out) return STAG_EINVAL;
+    cudaIpcMemHandle_t h;
+    CU(cudaIpcGetMemHandle(&h, L->xch));
+    memcpy(handle_out, &h, sizeof(h));
+    return STAG_OK;
+}
+
+extern "C" int stag_slab_ipc_open(const unsigned char handle[STAG_IPC_HANDLE_BYTES], void **ptr_out)
+{
+    if (!handle || !ptr_out) return STAG_EINVAL;
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle, sizeof(h));
+    CU(cudaIpcOpenMemHandle(ptr_out, h, cudaIpcMemLazyEnablePeerAccess));
+    return STAG_OK;
+}
+
+extern "C" int stag_slab_ipc_close(void *ptr)
+{
+    if (!ptr) return STAG_EINVAL;
+    CU(cudaIpcCloseMemHandle(ptr));
+    return STAG_OK;
+}
+
+extern "C" int stag_slab_connect(stag_links_t *L, void *bwd_exchange, void *fwd_exchange)
+{
+    if (!L || !L->is_slab || !bwd_exchange || !fwd_exchange) return STAG_EINVAL;
+    L->peer_bwd = (char *)bwd_exchange;
+    L->peer_fwd = (char *)fwd_exchange;
+    return STAG_OK;
+}
+
+namespace {
+
+template <typename T>
+int slab_push_t(stag_links *L, const cplx_t<T> *in, cudaStream_t s)
+{
+    const Geom &g = L->g;
+    const unsigned long long e = ++L->epoch;
+    XchHeader *mine = (XchHeader *)L->xch, *pf = (XchHeader *)L->peer_fwd, *pb = (XchHeader *)L->peer_bwd;
+    const unsigned grid = (unsigned)((2L * 3 * g.s3 + 255) / 256);
+    face_push_kernel<T><<<grid, 256, 0, s>>>(in, g.Vh, g.Vh_pad, g.s3,
+                                             (cplx_t<T> *)(L->peer_fwd + xch_halo_offset(g.s3, e, 0)),
+                                             (cplx_t<T> *)(L->peer_bwd + xch_halo_offset(g.s3, e, 1)),
+                                             &pf->flag_back, &pb->flag_fwd, e, &mine->ticket);
+    count_launch();
+    KCHECK();
+    return STAG_OK;
+}
+
+template <typename T, int NR>
+int slab_hop_t(stag_links *L, int prec, cplx_t<T> *out, const cplx_t<T> *in, int parity, double a,
+               const cplx_t<T> *own, cudaStream_t s)
+{
+    const Geom &g = L->g;
+    const pkt_t<T> *field = (const pkt_t<T> *)L->L[prec] +
+                            (size_t)parity * L->ntiles * (8 * (3 * NR) / Pkt<T>::CPP) * TILE;
+    const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
+    XchHeader *mine = (XchHeader *)L->xch;
+    HaloArgs<T> h;
+    h.back = (const cplx_t<T> *)(L->xch + xch_halo_offset(g.s3, L->epoch, 0));
+    h.fwd = (const cplx_t<T> *)(L->xch + xch_halo_offset(g.s3, L->epoch, 1));
+    h.flag_back = &mine->flag_back;
+    h.flag_fwd = &mine->flag_fwd;
+    h.epoch = L->epoch;
+    if (own)
+        dslash_kernel<T, NR, HOP_XPAY, 1, true><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)1, own, nullptr, nullptr, h);
+    else
+        dslash_kernel<T, NR, HOP_PLAIN, 1, true><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)0, (T)1, nullptr, nullptr, nullptr, h);
+    count_launch();
+    KCHECK();
+    return STAG_OK;
+}
+
+}  // namespace
+
+extern "C" int stag_slab_push(const void *in, stag_links_t *L, int prec)
+{
+    if (!in || !L || !L->is_slab || !prec_ok(prec) || !L->peer_bwd || !L->peer_fwd) return STAG_EINVAL;
+    if (prec_is_f32(prec)) return slab_push_t<float>(L, (const float2 *)in, t_stream);
+    return slab_push_t<double>(L, (const double2 *)in, t_stream);
+}
+
+extern "C" int stag_slab_hop(void *out, const void *in, stag_links_t *L, int parity, int prec,
+                             double a, const void *own)
+{
+    if (!out || !in || !L || !L->is_slab || out == in || (parity & ~1) || !prec_ok(prec) ||
+        L->epoch == 0)
+        return STAG_EINVAL;
+    int rc = ensure_links(L, prec);
+    if (rc) return rc;
+    switch (prec) {
+    case STAG_PREC_F64:     return slab_hop_t<double, 3>(L, prec, (double2 *)out, (const double2 *)in, parity, a, (const double2 *)own, t_stream);
+    case STAG_PREC_F32:     return slab_hop_t<float, 3>(L, prec, (float2 *)out, (const float2 *)in, parity, a, (const float2 *)own, t_stream);
+    case STAG_PREC_F64_R12: return slab_hop_t<double, 2>(L, prec, (double2 *)out, (const double2 *)in, parity, a, (const double2 *)own, t_stream);
+    case STAG_PREC_F32_R12: return slab_hop_t<float, 2>(L, prec, (float2 *)out, (const float2 *)in, parity, a, (const float2 *)own, t_stream);
+    }
+    return STAG_EINVAL;
+}
+
+extern "C" int stag_slab_dslash(void *out, const void *in, stag_links_t *L, int parity, int prec)
+{
+    int rc = stag_slab_push(in, L, prec);
+    if (rc) return rc;
+    return stag_slab_hop(out, in, L, parity, prec, 0.0, nullptr);
 }

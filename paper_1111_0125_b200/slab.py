@@ -1,0 +1,191 @@
+"""T-slab decomposition of the hop over several GPUs (include/stag.h "T-slabs"; DESIGN.md
+section 14): host-side plumbing only.  Every number is computed by the kernels behind
+stag_slab_push / stag_slab_hop; this module
+
+  * says which time slices a rank owns and who its neighbours are (pure host logic, tested with a
+    world-size-2 gloo group on CPU),
+  * scatters / gathers canonical spinors between the whole lattice and the slabs (time slices are
+    contiguous in the checkerboard index, so a slab's part of a one-parity spinor is one slice
+    [t0*s3, (t0+Tl)*s3) of it),
+  * wires the exchange regions: between processes by exchanging the 64-byte CUDA IPC handles through
+    torch.distributed (one process per GPU), inside one process by handing the raw pointers over.
+
+The paper's pipeline for the same step is boundary collect -> memcpy to host -> MPI -> memcpy to
+device (Table 1); here the faces are stored straight into the neighbour GPU's memory.
+"""
+from __future__ import annotations
+
+import ctypes
+
+import paper_1111_0125_b200 as stag
+
+IPC_HANDLE_BYTES = 64
+
+
+# ---- pure host logic ---------------------------------------------------------------------
+def slab_extent(global_dims, nranks: int) -> int:
+    """Local time extent; raises unless X3 splits into nranks even slabs of >= 2 slices."""
+    x3 = int(global_dims[3])
+    if nranks < 1 or x3 % nranks:
+        raise ValueError("X3 = %d does not split into %d slabs" % (x3, nranks))
+    tl = x3 // nranks
+    if tl < 2 or tl % 2:
+        raise ValueError("local time extent %d must be even and >= 2" % tl)
+    return tl
+
+
+def slab_range(global_dims, rank: int, nranks: int):
+    """(t0, t1): rank owns time slices t0 <= x3 < t1."""
+    tl = slab_extent(global_dims, nranks)
+    if not 0 <= rank < nranks:
+        raise ValueError("rank %d outside 0..%d" % (rank, nranks - 1))
+    return rank * tl, (rank + 1) * tl
+
+
+def local_dims(global_dims, nranks: int):
+    return (int(global_dims[0]), int(global_dims[1]), int(global_dims[2]), slab_extent(global_dims, nranks))
+
+
+def neighbours(rank: int, nranks: int):
+    """(backward, forward) ranks along time, periodic."""
+    return (rank - 1) % nranks, (rank + 1) % nranks
+
+
+def slice_sites(global_dims) -> int:
+    """s3: sites of one parity in one time slice."""
+    return int(global_dims[0]) * int(global_dims[1]) * int(global_dims[2]) // 2
+
+
+def scatter_spinor(chi_global, global_dims, rank: int, nranks: int):
+    """The slab's part of a canonical one-parity spinor chi[cb][3] of the whole lattice."""
+    t0, t1 = slab_range(global_dims, rank, nranks)
+    s3 = slice_sites(global_dims)
+    return chi_global[t0 * s3:t1 * s3]
+
+
+def gather_spinor(parts, global_dims):
+    """Inverse of scatter_spinor: parts[r] from rank r, in rank order."""
+    import numpy as np
+    out = np.concatenate(list(parts), axis=0)
+    vh = slice_sites(global_dims) * int(global_dims[3])
+    if out.shape[0] != vh:
+        raise ValueError("parts hold %d sites, the lattice has %d per parity" % (out.shape[0], vh))
+    return out
+
+
+def exchange_handles(my_handle: bytes, rank: int, nranks: int, group=None):
+    """All ranks' IPC handles through torch.distributed (any backend); returns the
+    (backward, forward) neighbours' handles."""
+    import torch.distributed as dist
+    if len(my_handle) != IPC_HANDLE_BYTES:
+        raise ValueError("an IPC handle is %d bytes" % IPC_HANDLE_BYTES)
+    world = dist.get_world_size(group)
+    if world != nranks:
+        raise ValueError("group has %d ranks, the decomposition %d" % (world, nranks))
+    allh = [None] * world
+    dist.all_gather_object(allh, bytes(my_handle), group=group)
+    b, f = neighbours(rank, nranks)
+    return allh[b], allh[f]
+
+
+# ---- the handle --------------------------------------------------------------------------
+class SlabLinks:
+    """One rank's slab (stag_slab_create).  W: canonical complex128 links of the WHOLE lattice."""
+
+    def __init__(self, global_dims, W, rank: int, nranks: int, antiperiodic_t: bool = True):
+        import numpy as np
+        torch = stag._require_cuda()
+        stag.use_current_stream()
+        self.global_dims = tuple(int(v) for v in global_dims)
+        self.dims = local_dims(global_dims, nranks)
+        self.rank, self.nranks = int(rank), int(nranks)
+        self._h = ctypes.c_void_p()
+        self._opened = []
+        W = np.ascontiguousarray(W, dtype=np.complex128)
+        stag._check(stag.lib().stag_slab_create(ctypes.byref(self._h), stag._cdims(self.global_dims),
+                                                int(bool(antiperiodic_t)), ctypes.c_void_p(W.ctypes.data), 0,
+                                                self.rank, self.nranks))
+        torch.cuda.current_stream().synchronize()
+
+    @property
+    def handle(self):
+        return self._h
+
+    def exchange_region(self):
+        """(device pointer, bytes) of this slab's exchange region."""
+        p, n = ctypes.c_void_p(), ctypes.c_size_t()
+        stag._check(stag.lib().stag_slab_info(self._h, None, None, None, ctypes.byref(p), ctypes.byref(n)))
+        return p.value, n.value
+
+    def ipc_handle(self) -> bytes:
+        buf = ctypes.create_string_buffer(IPC_HANDLE_BYTES)
+        stag._check(stag.lib().stag_slab_ipc_handle(self._h, buf))
+        return buf.raw
+
+    def connect_pointers(self, bwd_ptr: int, fwd_ptr: int):
+        stag._check(stag.lib().stag_slab_connect(self._h, ctypes.c_void_p(bwd_ptr), ctypes.c_void_p(fwd_ptr)))
+
+    def connect_distributed(self, group=None):
+        """One process per GPU: exchange IPC handles over torch.distributed and map the two
+        neighbours' exchange regions into this process."""
+        if self.nranks == 1:
+            return
+        hb, hf = exchange_handles(self.ipc_handle(), self.rank, self.nranks, group)
+        ptrs = []
+        for h in (hb, hf):
+            p = ctypes.c_void_p()
+            stag._check(stag.lib().stag_slab_ipc_open(ctypes.c_char_p(h), ctypes.byref(p)))
+            ptrs.append(p.value)
+            self._opened.append(p.value)
+        self.connect_pointers(ptrs[0], ptrs[1])
+
+    # -- the operator; spinors are device spinors of the LOCAL dims -------------------------
+    def push(self, v, prec):
+        stag.use_current_stream()
+        stag._check(stag.lib().stag_slab_push(ctypes.c_void_p(v.data_ptr()), self._h, int(prec)))
+
+    def hop(self, v, parity: int, prec, out=None, a: float = 0.0, own=None):
+        stag.use_current_stream()
+        if out is None:
+            out = stag.empty_spinor(self.dims, prec)
+        stag._check(stag.lib().stag_slab_hop(ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(v.data_ptr()),
+                                             self._h, int(parity), int(prec), float(a),
+                                             ctypes.c_void_p(own.data_ptr()) if own is not None else None))
+        return out
+
+    def dslash(self, v, parity: int, prec, out=None):
+        """push + hop: what each rank of a real multi-GPU run calls (all ranks in step)."""
+        self.push(v, prec)
+        return self.hop(v, parity, prec, out=out)
+
+    def apply_A(self, v_even, mass: float, prec):
+        """m^2 v - D_eo D_oe v on the slab's even sites (eq. 2.3): two exchanges, two hops."""
+        tmp = self.dslash(v_even, 1, prec)
+        self.push(tmp, prec)
+        return self.hop(tmp, 0, prec, a=mass * mass, own=v_even)
+
+    def close(self):
+        for p in self._opened:
+            stag.lib().stag_slab_ipc_close(ctypes.c_void_p(p))
+        self._opened = []
+        if self._h:
+            stag.lib().stag_links_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def connect_in_process(slabs):
+    """Slabs that live in one process (one GPU holding several, or tests): hand each its
+    neighbours' exchange regions as raw device pointers."""
+    n = len(slabs)
+    ptrs = [s.exchange_region()[0] for s in slabs]
+    for r, s in enumerate(slabs):
+        if s.rank != r or s.nranks != n:
+            raise ValueError("slabs must be given in rank order, all of them")
+        b, f = neighbours(r, n)
+        s.connect_pointers(ptrs[b], ptrs[f])

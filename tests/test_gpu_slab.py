@@ -1,0 +1,126 @@
+"""GPU parity of the T-slab hop (stag_slab_push / stag_slab_hop) on ONE device: the slabs of a
+decomposition live in one process, are wired with raw pointers, and run one after the other
+(all pushes of an exchange, then all hops), so no kernel ever waits on a kernel that has not been
+launched.  The data path -- links gathered per slab from the whole field, faces stored into the
+neighbours' halo buffers, flags, halo reads, 12-real signs at the global time boundary -- is the
+multi-GPU one.  Results must equal the whole-lattice kernel BITWISE (same arithmetic per site) and
+the oracle within the usual tolerance."""
+import numpy as np
+import pytest
+
+import fieldgen
+import oracle
+import paper_1111_0125_b200 as stag
+from paper_1111_0125_b200 import slab
+
+pytestmark = pytest.mark.gpu
+
+TOL = {stag.PREC_F64: 1e-13, stag.PREC_F64_R12: 1e-13, stag.PREC_F32: 2e-6, stag.PREC_F32_R12: 2e-6}
+ALL_PREC = [stag.PREC_F64, stag.PREC_F32, stag.PREC_F64_R12, stag.PREC_F32_R12]
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
+
+
+def make_slabs(dims, W, nranks, antiperiodic=True):
+    slabs = [slab.SlabLinks(dims, W, r, nranks, antiperiodic_t=antiperiodic) for r in range(nranks)]
+    slab.connect_in_process(slabs)
+    return slabs
+
+
+def slab_hop_all(slabs, chi, dims, parity, prec):
+    """One decomposed hop: scatter, all pushes, all hops, gather (canonical in, canonical out)."""
+    n = len(slabs)
+    vs = [stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(chi, dims, r, n)), slabs[r].dims, prec)
+          for r in range(n)]
+    for r in range(n):
+        slabs[r].push(vs[r], prec)
+    outs = [slabs[r].hop(vs[r], parity, prec) for r in range(n)]
+    return outs, slab.gather_spinor([stag.spinor_unpack(o, slabs[r].dims, prec) for r, o in enumerate(outs)], dims)
+
+
+# (dims, nranks): several ranks, two ranks (both neighbours the same slab), one rank (its own
+# neighbour), slabs of two slices (every slice is a boundary), ragged Vh (pads), X_mu = 2
+CASES = [((4, 4, 4, 8), 2), ((4, 4, 4, 12), 3), ((4, 4, 4, 8), 4), ((4, 4, 4, 4), 1),
+         ((6, 2, 2, 8), 2), ((2, 2, 2, 4), 2), ((8, 8, 8, 8), 2)]
+
+
+@pytest.mark.parametrize("dims,nranks", CASES)
+@pytest.mark.parametrize("prec", ALL_PREC)
+def test_slab_hop_matches_oracle_and_whole_lattice_kernel(dims, nranks, prec):
+    import torch
+    W = fieldgen.links(dims, "random", seed=61)
+    L = stag.Links(dims, W)
+    slabs = make_slabs(dims, W, nranks)
+    for parity in (0, 1):
+        chi = fieldgen.spinor_gaussian(dims, 1 - parity, seed=62 + parity)
+        outs, got = slab_hop_all(slabs, chi, dims, parity, prec)
+        assert rel_l2(got, oracle.dslash(chi, W, dims, parity)) <= TOL[prec]
+        whole = stag.spinor_unpack(stag.dslash(stag.spinor_pack(chi, dims, prec), L, parity, prec), dims, prec)
+        assert np.array_equal(got, whole)
+        for r, o in enumerate(outs):                      # pads of every slab's output stay zero
+            vh = slabs[r].dims[0] * slabs[r].dims[1] * slabs[r].dims[2] * slabs[r].dims[3] // 2
+            planes = o.view(3, -1, 2)
+            assert float(planes[:, vh:, :].abs().max()) == 0.0 if planes.shape[1] > vh else True
+
+
+@pytest.mark.parametrize("prec", ALL_PREC)
+def test_slab_hop_periodic_time_boundary(prec):
+    dims = (4, 4, 2, 8)
+    W = fieldgen.links(dims, "random", seed=5, antiperiodic_t=False)
+    slabs = make_slabs(dims, W, 2, antiperiodic=False)
+    chi = fieldgen.spinor_gaussian(dims, 0, seed=6)
+    _, got = slab_hop_all(slabs, chi, dims, 1, prec)
+    assert rel_l2(got, oracle.dslash(chi, W, dims, 1)) <= TOL[prec]
+
+
+@pytest.mark.parametrize("nranks", [1, 2, 4])
+@pytest.mark.parametrize("prec", [stag.PREC_F64, stag.PREC_F32_R12])
+def test_slab_apply_A_matches_oracle_over_repeated_exchanges(nranks, prec):
+    """A = m^2 - D_eo D_oe through two exchanges per application, applied three times in a row so
+    both halo buffers and the epoch flags are reused."""
+    cfg = fieldgen.CONFIGS["c2_8^4"]
+    W = cfg.links()
+    slabs = make_slabs(cfg.dims, W, nranks)
+    chi = cfg.source()
+    for rep in range(3):
+        ref = oracle.apply_A(chi, W, cfg.dims, cfg.mass)
+        vs = [stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(chi, cfg.dims, r, nranks)), slabs[r].dims, prec)
+              for r in range(nranks)]
+        for r in range(nranks):
+            slabs[r].push(vs[r], prec)
+        tmps = [slabs[r].hop(vs[r], 1, prec) for r in range(nranks)]
+        for r in range(nranks):
+            slabs[r].push(tmps[r], prec)
+        outs = [slabs[r].hop(tmps[r], 0, prec, a=cfg.mass ** 2, own=vs[r]) for r in range(nranks)]
+        got = slab.gather_spinor([stag.spinor_unpack(o, slabs[r].dims, prec) for r, o in enumerate(outs)], cfg.dims)
+        assert rel_l2(got, ref) <= TOL[prec]
+        chi = np.ascontiguousarray(ref / np.linalg.norm(ref) * np.linalg.norm(chi))
+
+
+def test_single_rank_slab_dslash_entry_and_argument_errors():
+    """nranks = 1: stag_slab_dslash (push + hop in one call) is safe on one device."""
+    import ctypes
+    dims = (4, 4, 4, 4)
+    W = fieldgen.links(dims, "random", seed=1)
+    chi = fieldgen.spinor_gaussian(dims, 0, seed=2)
+    S = slab.SlabLinks(dims, W, 0, 1)
+    v = stag.spinor_pack(chi, dims, 0)
+    out = stag.empty_spinor(dims, 0)
+    lib = stag.lib()
+    vp = ctypes.c_void_p
+    assert lib.stag_slab_hop(vp(out.data_ptr()), vp(v.data_ptr()), S.handle, 1, 0, 0.0, None) == stag.EINVAL  # no push yet
+    got = stag.spinor_unpack(S.dslash(v, 1, 0), dims, 0)
+    assert rel_l2(got, oracle.dslash(chi, W, dims, 1)) <= 1e-13
+    # a slab handle is refused by the whole-lattice entry points, and vice versa
+    cd = (ctypes.c_int * 4)(*dims)
+    assert lib.stag_dslash(vp(out.data_ptr()), vp(v.data_ptr()), S.handle, 1, cd, 0) == stag.EINVAL
+    L = stag.Links(dims, W)
+    assert lib.stag_slab_push(vp(v.data_ptr()), L.handle, 0) == stag.EINVAL
+    h = ctypes.c_void_p()
+    for rank, n in ((0, 3), (2, 2), (0, 4)):     # 4/3 not integer; rank out of range; 1 slice each
+        assert lib.stag_slab_create(ctypes.byref(h), cd, 1, vp(W.ctypes.data), 0, rank, n) == stag.EINVAL
+    two = slab.SlabLinks((4, 4, 4, 8), fieldgen.links((4, 4, 4, 8), "random", seed=1), 0, 2)
+    v8 = stag.empty_spinor(two.dims, 0)
+    assert lib.stag_slab_push(vp(v8.data_ptr()), two.handle, 0) == stag.EINVAL   # not connected yet
