@@ -188,6 +188,7 @@ int stag_apply_A_mrhs(void *out_even, const void *in_even, const stag_links_t *l
  * stag_slab_connect.  Slabs living in one process connect with the raw pointers from
  * stag_slab_info.  nranks = 1 connects to itself.  DESIGN.md section 14. */
 #define STAG_IPC_HANDLE_BYTES 64
+#define STAG_MAX_RANKS 16       /* most slabs a lattice is split into */
 
 /* W_global: canonical fp64 links of the WHOLE lattice global_dims (eta*bc folded). */
 int stag_slab_create(stag_links_t **slab_out, const int global_dims[4], int antiperiodic_t,
@@ -277,6 +278,40 @@ int stag_solve_M(void *psi_even, void *psi_odd, const void *h_even, const void *
 int stag_cg_solve_host(double *x_host, const double *b_host, const stag_links_t *links,
                        double mass, double tol, int maxiter, int mode,
                        const stag_cg_params_t *params, stag_cg_stats_t *stats_out);
+
+/* ---- CG over T-slabs -----------------------------------------------------------------
+ *
+ * The paper's headline is the CG on several GPUs (title; Table 1; 36 / 19 GFLOPS per GPU once
+ * the network is included).  Here every rank runs Fig. 1 (mode 0) or the mixed
+ * driver of section 3.2 (mode 3) on its slab; the hops exchange faces as above, and the two
+ * inner products of an iteration are summed over ranks through the exchange regions: each rank
+ * stores its local total into every rank's slots, and every rank adds the nranks slots in rank
+ * order, so alpha, beta and every stopping decision are bit-identical everywhere and no rank
+ * ever talks to the host inside a chunk of iterations.  Needs stag_slab_connect_all.
+ *
+ * The solve is a sequence of ACTIONS, each a fixed sequence of PHASES:
+ *     stag_slab_cg_begin(...);
+ *     for (;;) { stag_slab_cg_control(slab, &act); if (act == STAG_SLAB_ACT_DONE) break;
+ *                for (ph = 0, more = 1; more; ++ph) stag_slab_cg_step(slab, act, ph, &more); }
+ *     stag_slab_cg_finish(slab, &stats);
+ * One process per GPU runs exactly that loop.  No kernel of a phase waits for a peer's kernel of
+ * the same phase, so slabs that share one device can instead be stepped rank after rank, phase
+ * by phase (how the single-GPU tests run the multi-GPU data path).  x, b: fp64 device spinors of
+ * the slab's local dims; x holds the initial guess.  Modes: STAG_CG_F64, STAG_CG_RELIABLE.
+ * graph_chunk of the params = iterations per ACT_ITER (default 32; plain launches). */
+enum {
+    STAG_SLAB_ACT_DONE = 0, STAG_SLAB_ACT_NORM = 1, STAG_SLAB_ACT_INIT = 2, STAG_SLAB_ACT_ITER = 3,
+    STAG_SLAB_ACT_UPDATE = 4, STAG_SLAB_ACT_VERIFY = 5, STAG_SLAB_ACT_FINAL = 6
+};
+/* regions[r]: device-accessible address of rank r's exchange region, r = 0..nranks-1 (the
+ * slab's own included); also sets the two neighbours.  Host array. */
+int stag_slab_connect_all(stag_links_t *slab, void *const *regions);
+int stag_slab_cg_begin(stag_links_t *slab, void *x_even, const void *b_even, double mass, double tol,
+                       int maxiter, int mode, const stag_cg_params_t *params);
+int stag_slab_cg_control(stag_links_t *slab, int *action_out);
+int stag_slab_cg_step(stag_links_t *slab, int action, int phase, int *more_out);
+/* Returns STAG_OK / STAG_ENOCONV / STAG_EBREAKDOWN like stag_cg_solve; stats as there. */
+int stag_slab_cg_finish(stag_links_t *slab, stag_cg_stats_t *stats_out);
 
 #ifdef __cplusplus
 }

@@ -124,6 +124,12 @@ SIGNATURES = {
     "stag_slab_push": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
     "stag_slab_hop": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, ctypes.c_int, ctypes.c_double, _vp]),
     "stag_slab_dslash": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, ctypes.c_int]),
+    "stag_slab_connect_all": (ctypes.c_int, [_vp, ctypes.POINTER(_vp)]),
+    "stag_slab_cg_begin": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
+                                          ctypes.c_int, ctypes.POINTER(_Params)]),
+    "stag_slab_cg_control": (ctypes.c_int, [_vp, _ip]),
+    "stag_slab_cg_step": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _ip]),
+    "stag_slab_cg_finish": (ctypes.c_int, [_vp, ctypes.POINTER(_Stats)]),
     "stag_cg_solve_host": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double,
                                           ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Params),
                                           ctypes.POINTER(_Stats)]),

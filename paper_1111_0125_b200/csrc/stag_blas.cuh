@@ -108,6 +108,52 @@ __device__ __forceinline__ double block_total_fixed(const double *__restrict__ v
     return total;
 }
 
+// The scalar part of one pass of Fig. 1's loop plus the stopping / trigger tests
+// (Q9-Q11), for every right-hand side, given totals[j] = the new |r_j|^2.  One thread.
+// Shared by update_kernel (one GPU) and the slab path's scalar kernel (stag_slab.cuh), where
+// totals are sums over all ranks and every rank runs this on identical inputs.
+__device__ __forceinline__ void cg_iteration_epilogue(CgCtrl *__restrict__ ctrl, const double *totals)
+{
+    const int it = ctrl->iter + 1, mode = ctrl->mode, nrhs = ctrl->nrhs;
+    ctrl->iter = it;
+    bool breakdown = false, trigger = false;
+    unsigned conv = 0;
+    for (int j = 0; j < nrhs; ++j) {
+        if (!ctrl->active[j]) continue;
+        ctrl->iters[j] += 1;
+        const double dn = totals[j];
+        ctrl->sum1[j] = dn;
+        // dAd[j] was written by another block of this launch: read it past L1
+        if (!(__ldcg(&ctrl->dAd[j]) > 0.0) || !(dn == dn)) { breakdown = true; continue; }
+        if (mode == STAG_CG_RELIABLE) {
+            const double rn = sqrt(dn);
+            if (dn <= ctrl->tol2b[j] || rn < ctrl->eps_in * ctrl->maxr[j]) trigger = true;   // P:L97, Q11
+            else ctrl->maxr[j] = fmax(ctrl->maxr[j], rn);                                    // Q9
+        } else if (mode == STAG_CG_DEFECT) {
+            if (dn <= ctrl->inner2[j]) conv |= 1u << j;                                      // Fig. 2 inner
+        } else {
+            if (dn <= ctrl->tol2b[j]) conv |= 1u << j;                                       // Fig. 1
+        }
+    }
+    int st = CG_RUN;
+    if (breakdown) st = CG_BREAKDOWN;
+    else if (trigger) st = CG_UPDATE;     // beta is then formed from the corrected residuals (Q10)
+    else {
+        bool any = false;
+        for (int j = 0; j < nrhs; ++j) {
+            if (!ctrl->active[j]) continue;
+            const double dn = totals[j];
+            ctrl->beta[j] = dn / ctrl->delta[j];                                             // P:L54
+            ctrl->delta[j] = dn;
+            if (conv & (1u << j)) ctrl->active[j] = 0;      // this right-hand side is done: freeze it
+            else any = true;
+        }
+        if (!any) st = CG_CONVERGED;
+    }
+    if (st == CG_RUN && it >= ctrl->maxiter) st = CG_MAXITER;
+    ctrl->state = st;
+}
+
 // alpha = delta / <d,Ad> ; y += alpha d ; r -= alpha q ; delta' = |r|^2 ; then the scalar part
 // of the iteration (P:L51-54 and the trigger of P:L97) in the last block, for every right-hand
 // side.  <d,Ad> arrives as the per-block partial sums of the second hop (stag_dslash.cuh): every
@@ -158,45 +204,7 @@ update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
     if (!finish_reduction(bs, partials, &ctrl->ticket[1], red, totals)) return;
     if (threadIdx.x != 0) return;
 
-    // ---- scalar epilogue, one thread ------------------------------------------------
-    const int it = ctrl->iter + 1, mode = ctrl->mode, nrhs = ctrl->nrhs;
-    ctrl->iter = it;
-    bool breakdown = false, trigger = false;
-    unsigned conv = 0;
-    for (int j = 0; j < nrhs; ++j) {
-        if (!ctrl->active[j]) continue;
-        ctrl->iters[j] += 1;
-        const double dn = totals[j];
-        ctrl->sum1[j] = dn;
-        // dAd[j] was written by another block of this launch: read it past L1
-        if (!(__ldcg(&ctrl->dAd[j]) > 0.0) || !(dn == dn)) { breakdown = true; continue; }
-        if (mode == STAG_CG_RELIABLE) {
-            const double rn = sqrt(dn);
-            if (dn <= ctrl->tol2b[j] || rn < ctrl->eps_in * ctrl->maxr[j]) trigger = true;   // P:L97, Q11
-            else ctrl->maxr[j] = fmax(ctrl->maxr[j], rn);                                    // Q9
-        } else if (mode == STAG_CG_DEFECT) {
-            if (dn <= ctrl->inner2[j]) conv |= 1u << j;                                      // Fig. 2 inner
-        } else {
-            if (dn <= ctrl->tol2b[j]) conv |= 1u << j;                                       // Fig. 1
-        }
-    }
-    int st = CG_RUN;
-    if (breakdown) st = CG_BREAKDOWN;
-    else if (trigger) st = CG_UPDATE;     // beta is then formed from the corrected residuals (Q10)
-    else {
-        bool any = false;
-        for (int j = 0; j < nrhs; ++j) {
-            if (!ctrl->active[j]) continue;
-            const double dn = totals[j];
-            ctrl->beta[j] = dn / ctrl->delta[j];                                             // P:L54
-            ctrl->delta[j] = dn;
-            if (conv & (1u << j)) ctrl->active[j] = 0;      // this right-hand side is done: freeze it
-            else any = true;
-        }
-        if (!any) st = CG_CONVERGED;
-    }
-    if (st == CG_RUN && it >= ctrl->maxiter) st = CG_MAXITER;
-    ctrl->state = st;
+    cg_iteration_epilogue(ctrl, totals);
 }
 
 // x64 += y ; y = 0  (group-wise update); the vectors are nrhs*n reals long
@@ -211,6 +219,42 @@ accumulate_kernel(double *__restrict__ x, T *__restrict__ y, long n)
 }
 
 enum { RES_INIT = 0, RES_UPDATE = 1, RES_FINAL = 2, RES_NORM = 3 };
+
+// Scalar part of residual_kernel (see there), given totals[k] = |r_k|^2 (or |b_k|^2).  One thread.
+template <int WHAT>
+__device__ __forceinline__ void residual_epilogue(CgCtrl *__restrict__ ctrl, const double *totals)
+{
+    const int nrhs = ctrl->nrhs;
+    bool any = false, bad = false;
+    for (int k = 0; k < nrhs; ++k) {
+        const double dn = totals[k];
+        if (WHAT == RES_NORM) { ctrl->bnorm2[k] = dn; continue; }
+        ctrl->sum0[k] = dn;
+        if (WHAT == RES_FINAL) continue;
+        if (!(dn == dn)) { bad = true; continue; }
+        if (WHAT == RES_INIT) {
+            ctrl->delta[k] = dn;
+            ctrl->beta[k] = 0.0;
+            ctrl->maxr[k] = sqrt(dn);
+            ctrl->inner2[k] = fmax(ctrl->eps_in * ctrl->eps_in * dn, ctrl->tol2b[k]);   // Fig. 2, Q8
+            ctrl->active[k] = dn > ctrl->tol2b[k];
+        } else if (ctrl->active[k]) {                     // RES_UPDATE
+            ctrl->maxr[k] = sqrt(dn);                                                   // Q9
+            if (dn <= ctrl->tol2b[k]) ctrl->active[k] = 0;
+            else {
+                ctrl->beta[k] = dn / ctrl->delta[k];                                    // Q10
+                ctrl->delta[k] = dn;
+            }
+        }
+        any = any || ctrl->active[k];
+    }
+    if (WHAT == RES_NORM || WHAT == RES_FINAL) return;
+    if (WHAT == RES_UPDATE) ctrl->n_updates += 1;
+    int st = any ? CG_RUN : CG_CONVERGED;
+    if (bad) st = CG_BREAKDOWN;
+    else if (any && ctrl->iter >= ctrl->maxiter) st = CG_MAXITER;
+    ctrl->state = st;
+}
 
 // r = b - q in fp64, |r|^2, and optionally the fp32 copy of r (reliable update), for
 // every right-hand side.  With WHAT == RES_NORM it only computes |b|^2.  The last block then
@@ -245,36 +289,7 @@ residual_kernel(double *__restrict__ r, const double *__restrict__ b,
     if (!finish_reduction(bs, partials, &ctrl->ticket[2], red, totals)) return;
     if (threadIdx.x != 0) return;
 
-    const int nrhs = ctrl->nrhs;
-    bool any = false, bad = false;
-    for (int k = 0; k < nrhs; ++k) {
-        const double dn = totals[k];
-        if (WHAT == RES_NORM) { ctrl->bnorm2[k] = dn; continue; }
-        ctrl->sum0[k] = dn;
-        if (WHAT == RES_FINAL) continue;
-        if (!(dn == dn)) { bad = true; continue; }
-        if (WHAT == RES_INIT) {
-            ctrl->delta[k] = dn;
-            ctrl->beta[k] = 0.0;
-            ctrl->maxr[k] = sqrt(dn);
-            ctrl->inner2[k] = fmax(ctrl->eps_in * ctrl->eps_in * dn, ctrl->tol2b[k]);   // Fig. 2, Q8
-            ctrl->active[k] = dn > ctrl->tol2b[k];
-        } else if (ctrl->active[k]) {                     // RES_UPDATE
-            ctrl->maxr[k] = sqrt(dn);                                                   // Q9
-            if (dn <= ctrl->tol2b[k]) ctrl->active[k] = 0;
-            else {
-                ctrl->beta[k] = dn / ctrl->delta[k];                                    // Q10
-                ctrl->delta[k] = dn;
-            }
-        }
-        any = any || ctrl->active[k];
-    }
-    if (WHAT == RES_NORM || WHAT == RES_FINAL) return;
-    if (WHAT == RES_UPDATE) ctrl->n_updates += 1;
-    int st = any ? CG_RUN : CG_CONVERGED;
-    if (bad) st = CG_BREAKDOWN;
-    else if (any && ctrl->iter >= ctrl->maxiter) st = CG_MAXITER;
-    ctrl->state = st;
+    residual_epilogue<WHAT>(ctrl, totals);
 }
 
 // dst = (T) src, elementwise (precision change of a device spinor)

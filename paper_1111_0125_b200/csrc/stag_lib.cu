@@ -81,6 +81,7 @@ int blas_grid(long n_reals, int nrhs)
 // ------------------------------------------------------------------------------------
 // the link handle
 // ------------------------------------------------------------------------------------
+struct stag_slab_cg;
 struct stag_links {
     Geom g;
     int dims[4];           // extents of the lattice this handle covers (the slab's, for a slab)
@@ -105,6 +106,9 @@ struct stag_links {
     char *xch;
     char *peer_bwd, *peer_fwd;
     unsigned long long epoch;
+    char **peers_dev;      // device array: every rank's exchange region (stag_slab_connect_all)
+    int all_connected;
+    struct stag_slab_cg *cg;   // state of the slab CG in progress (stag_slab_cg_*)
     void *wrap_b;          // stag_solve_M: b_e of the even-site system, wrap_b_rhs spinors (lazy)
     int wrap_b_rhs;
     cudaEvent_t ev0, ev1;
@@ -448,6 +452,8 @@ static int links_create(stag_links_t **links_out, const int dims[4], int antiper
     return STAG_OK;
 }
 
+static void stag_slab_cg_free(struct stag_slab_cg *c);
+
 extern "C" void stag_links_destroy(stag_links_t *L)
 {
     if (!L) return;
@@ -458,6 +464,8 @@ extern "C" void stag_links_destroy(stag_links_t *L)
     if (L->stage_dev) cudaFree(L->stage_dev);
     if (L->wrap_b) cudaFree(L->wrap_b);
     if (L->xch) cudaFree(L->xch);
+    if (L->peers_dev) cudaFree(L->peers_dev);
+    stag_slab_cg_free(L->cg);
     if (L->cap_stream) cudaStreamDestroy(L->cap_stream);
     if (L->ev0) cudaEventDestroy(L->ev0);
     if (L->ev1) cudaEventDestroy(L->ev1);
@@ -946,6 +954,8 @@ extern "C" int stag_solve_M(void *psi_even, void *psi_odd, const void *h_even, c
 // ------------------------------------------------------------------------------------
 // C ABI: T-slab decomposition (include/stag.h "T-slabs"; stag_slab.cuh)
 // ------------------------------------------------------------------------------------
+extern "C" int stag_slab_connect_all(stag_links_t *L, void *const *regions);
+
 extern "C" int stag_slab_create(stag_links_t **slab_out, const int global_dims[4], int antiperiodic_t,
                                 const double *W_global, int on_device, int rank, int nranks)
 {
@@ -958,7 +968,10 @@ extern "C" int stag_slab_create(stag_links_t **slab_out, const int global_dims[4
     if (e == cudaSuccess) e = cudaMemsetAsync(L->xch, 0, bytes, t_stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(t_stream);
     if (e != cudaSuccess) { rc = cuda_fail(e, "slab exchange region", __LINE__); stag_links_destroy(L); *slab_out = nullptr; return rc; }
-    if (nranks == 1) L->peer_bwd = L->peer_fwd = L->xch;     // periodic wrap through my own halo
+    if (nranks == 1) {                                       // periodic wrap through my own halo
+        void *self[1] = { L->xch };
+        return stag_slab_connect_all(L, self);
+    }
     return STAG_OK;
 }
 
@@ -1083,3 +1096,376 @@ extern "C" int stag_slab_dslash(void *out, const void *in, stag_links_t *L, int 
     if (rc) return rc;
     return stag_slab_hop(out, in, L, parity, prec, 0.0, nullptr);
 }
+
+// ------------------------------------------------------------------------------------
+// C ABI: CG over T-slabs (include/stag.h "CG over T-slabs")
+// ------------------------------------------------------------------------------------
+struct stag_slab_cg {
+    double *x;
+    const double *b;
+    double mass, m2, tol;
+    int maxiter, mode;
+    stag_cg_params_t P;
+    Workspace w;
+    int prec_lo, prec_hi;
+    long n;
+    int gb;
+    bool lo;
+    unsigned long long red_seq;      // global sums published so far (same on every rank)
+    unsigned long long seq_dAd, seq_rr, seq_res;
+    int stage;                       // 0: nothing done, 1: |b|^2 on its way, 2: in the loop, 3: done
+    bool have_true, verifying;
+    int n_restarts, applies_f64, final_state;
+    double bnorm2;
+    int rc_final;
+};
+
+extern "C" int stag_slab_connect_all(stag_links_t *L, void *const *regions)
+{
+    if (!L || !L->is_slab || !regions || L->nranks > MAX_RANKS) return STAG_EINVAL;
+    for (int r = 0; r < L->nranks; ++r) if (!regions[r]) return STAG_EINVAL;
+    if (!L->peers_dev) CU(cudaMalloc((void **)&L->peers_dev, MAX_RANKS * sizeof(char *)));
+    CU(cudaMemcpyAsync(L->peers_dev, regions, L->nranks * sizeof(char *), cudaMemcpyHostToDevice, t_stream));
+    CU(cudaStreamSynchronize(t_stream));
+    L->peer_bwd = (char *)regions[(L->rank + L->nranks - 1) % L->nranks];
+    L->peer_fwd = (char *)regions[(L->rank + 1) % L->nranks];
+    L->all_connected = 1;
+    return STAG_OK;
+}
+
+namespace {
+
+Comm make_comm(const stag_links *L, unsigned long long seq)
+{
+    Comm c;
+    c.peers = L->peers_dev;
+    c.mine = L->xch;
+    c.nranks = L->nranks;
+    c.myrank = L->rank;
+    c.seq = seq;
+    return c;
+}
+
+template <typename T, int NR>
+int slab_hop_mode_t(stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx_t<T> *in, int parity,
+                    double a, const cplx_t<T> *own, double *partials, const CgCtrl *ctrl, cudaStream_t s)
+{
+    const Geom &g = L->g;
+    const pkt_t<T> *field = (const pkt_t<T> *)L->L[prec] +
+                            (size_t)parity * L->ntiles * (8 * (3 * NR) / Pkt<T>::CPP) * TILE;
+    const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
+    XchHeader *mine = (XchHeader *)L->xch;
+    HaloArgs<T> h;
+    h.back = (const cplx_t<T> *)(L->xch + xch_halo_offset(g.s3, L->epoch, 0));
+    h.fwd = (const cplx_t<T> *)(L->xch + xch_halo_offset(g.s3, L->epoch, 1));
+    h.flag_back = &mine->flag_back;
+    h.flag_fwd = &mine->flag_fwd;
+    h.epoch = L->epoch;
+    switch (hop) {
+    case HOP_PLAIN:
+        dslash_kernel<T, NR, HOP_PLAIN, 1, true><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)0, (T)1, nullptr, nullptr, ctrl, h);
+        break;
+    case HOP_XPAY:
+        dslash_kernel<T, NR, HOP_XPAY, 1, true><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)1, own, nullptr, ctrl, h);
+        break;
+    default:
+        dslash_kernel<T, NR, HOP_XPAY_DOT, 1, true><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)1, own, partials, ctrl, h);
+        break;
+    }
+    count_launch();
+    KCHECK();
+    return STAG_OK;
+}
+
+int slab_hop_mode(stag_links *L, int prec, int hop, void *out, const void *in, int parity, double a,
+                  const void *own, double *partials, const CgCtrl *ctrl, cudaStream_t s)
+{
+    switch (prec) {
+    case STAG_PREC_F64:     return slab_hop_mode_t<double, 3>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, (const double2 *)own, partials, ctrl, s);
+    case STAG_PREC_F32:     return slab_hop_mode_t<float, 3>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, (const float2 *)own, partials, ctrl, s);
+    case STAG_PREC_F64_R12: return slab_hop_mode_t<double, 2>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, (const double2 *)own, partials, ctrl, s);
+    case STAG_PREC_F32_R12: return slab_hop_mode_t<float, 2>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, (const float2 *)own, partials, ctrl, s);
+    }
+    return STAG_EINVAL;
+}
+
+int slab_push_prec(stag_links *L, const void *in, int prec, cudaStream_t s)
+{
+    if (prec_is_f32(prec)) return slab_push_t<float>(L, (const float2 *)in, s);
+    return slab_push_t<double>(L, (const double2 *)in, s);
+}
+
+// r64 = b - A64 x and its global |r|^2 in four phases (0..3); WHAT selects the scalar step.
+template <int WHAT>
+int slab_residual_phase(stag_links *L, stag_slab_cg *C, int ph, bool accumulate_first, bool lo_copy, bool *more)
+{
+    Workspace &w = C->w;
+    cudaStream_t s = t_stream;
+    int rc = STAG_OK;
+    *more = ph < 3;
+    switch (ph) {
+    case 0:
+        if (accumulate_first) {
+            accumulate_kernel<float><<<blas_grid(C->n, 1), BLAS_BLOCK, 0, s>>>(C->x, w.y32, C->n);   // x += y ; y = 0
+            count_launch();
+            KCHECK();
+        }
+        return slab_push_prec(L, C->x, C->prec_hi, s);
+    case 1:
+        if ((rc = slab_hop_mode(L, C->prec_hi, HOP_PLAIN, w.tmp64, C->x, 1, 0.0, nullptr, nullptr, nullptr, s))) return rc;
+        ++C->applies_f64;
+        return slab_push_prec(L, w.tmp64, C->prec_hi, s);
+    case 2:
+        if ((rc = slab_hop_mode(L, C->prec_hi, HOP_XPAY, w.q64, w.tmp64, 0, C->m2, C->x, nullptr, nullptr, s))) return rc;
+        C->seq_res = ++C->red_seq;
+        slab_residual_kernel<float, WHAT><<<C->gb, BLAS_BLOCK, 0, s>>>(w.r64, C->b, w.q64, lo_copy ? w.r32 : nullptr, C->n, w.partials, w.ctrl, make_comm(L, C->seq_res));
+        count_launch();
+        KCHECK();
+        return STAG_OK;
+    case 3:
+        slab_scalar_kernel<WHAT><<<1, 32, 0, s>>>(w.ctrl, make_comm(L, C->seq_res));
+        count_launch();
+        KCHECK();
+        return STAG_OK;
+    }
+    return STAG_EINVAL;
+}
+
+// phase ph of iteration chunk: five phases per pass of Fig. 1's loop
+template <typename T>
+int slab_iteration_phase(stag_links *L, stag_slab_cg *C, int sub, T *y, T *r, T *d, T *q, T *tmp)
+{
+    Workspace &w = C->w;
+    cudaStream_t s = t_stream;
+    int rc;
+    switch (sub) {
+    case 0:   // d = r + beta d ; its faces to the neighbours
+        xpay_kernel<T><<<dim3(C->gb, 1), BLAS_BLOCK, 0, s>>>(d, r, C->n, w.ctrl);
+        count_launch();
+        KCHECK();
+        return slab_push_prec(L, d, C->prec_lo, s);
+    case 1:   // tmp = D_oe d ; its faces
+        if ((rc = slab_hop_mode(L, C->prec_lo, HOP_PLAIN, tmp, d, 1, 0.0, nullptr, nullptr, w.ctrl, s))) return rc;
+        return slab_push_prec(L, tmp, C->prec_lo, s);
+    case 2:   // q = m^2 d - D_eo tmp, local <d,q> published
+        if ((rc = slab_hop_mode(L, C->prec_lo, HOP_XPAY_DOT, q, tmp, 0, C->m2, d, w.hop_partials, w.ctrl, s))) return rc;
+        C->seq_dAd = ++C->red_seq;
+        slab_publish_partials_kernel<<<1, BLAS_BLOCK, 0, s>>>(w.hop_partials, w.n_hop, make_comm(L, C->seq_dAd), w.ctrl);
+        count_launch();
+        KCHECK();
+        return STAG_OK;
+    case 3:   // alpha from the global <d,Ad>; y, r; local |r|^2 published
+        C->seq_rr = ++C->red_seq;
+        slab_update_kernel<T><<<C->gb, BLAS_BLOCK, 0, s>>>(y, r, d, q, C->n, w.partials, w.ctrl, make_comm(L, C->seq_dAd), make_comm(L, C->seq_rr));
+        count_launch();
+        KCHECK();
+        return STAG_OK;
+    case 4:   // beta, stopping tests, trigger: the same epilogue on every rank
+        slab_scalar_kernel<SCALAR_ITER><<<1, 32, 0, s>>>(w.ctrl, make_comm(L, C->seq_rr));
+        count_launch();
+        KCHECK();
+        return STAG_OK;
+    }
+    return STAG_EINVAL;
+}
+
+}  // namespace
+
+extern "C" int stag_slab_cg_begin(stag_links_t *L, void *x_even, const void *b_even, double mass,
+                                  double tol, int maxiter, int mode, const stag_cg_params_t *params)
+{
+    if (!L || !L->is_slab || !L->all_connected || !x_even || !b_even || x_even == b_even ||
+        !(tol > 0.0) || maxiter < 0 || (mode != STAG_CG_F64 && mode != STAG_CG_RELIABLE))
+        return STAG_EINVAL;
+    if (!L->cg) {
+        L->cg = new (std::nothrow) stag_slab_cg();
+        if (!L->cg) return STAG_ENOMEM;
+        L->cg->red_seq = 0;
+    }
+    stag_slab_cg *C = L->cg;
+    const unsigned long long keep_seq = C->red_seq;      // reduction numbers never restart
+    memset(C, 0, sizeof(*C));
+    C->red_seq = keep_seq;
+    if (params) C->P = *params;
+    if (!(C->P.eps_in > 0.0)) C->P.eps_in = 0.1;
+    if (C->P.graph_chunk <= 0) C->P.graph_chunk = 32;    // iterations between host checks (plain launches)
+    C->x = (double *)x_even;
+    C->b = (const double *)b_even;
+    C->mass = mass;
+    C->m2 = mass * mass;
+    C->tol = tol;
+    C->maxiter = maxiter;
+    C->mode = mode;
+    C->lo = (mode != STAG_CG_F64);
+    C->prec_lo = C->lo ? (C->P.recon12 ? STAG_PREC_F32_R12 : STAG_PREC_F32)
+                       : (C->P.recon12 ? STAG_PREC_F64_R12 : STAG_PREC_F64);
+    C->prec_hi = C->P.recon12_f64 ? STAG_PREC_F64_R12 : STAG_PREC_F64;
+    C->n = (long)6 * L->g.Vh_pad;
+    C->gb = blas_grid(C->n, 1);
+    int rc;
+    if ((rc = ensure_links(L, C->prec_lo))) return rc;
+    if ((rc = ensure_links(L, C->prec_hi))) return rc;
+    if ((rc = ensure_workspace(L, C->w, 1))) return rc;
+    CgCtrl *h = L->h_ctrl;
+    memset(h, 0, sizeof(*h));
+    h->mode = mode;
+    h->maxiter = maxiter;
+    h->eps_in = C->P.eps_in;
+    h->nrhs = 1;
+    CU(cudaMemcpyAsync(C->w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, t_stream));
+    CU(cudaEventRecord(L->ev0, t_stream));
+    C->stage = 0;
+    return STAG_OK;
+}
+
+// Decide what every rank does next.  Synchronises the stream and reads the control block; all
+// ranks hold identical scalars, so all ranks get the same answer.
+extern "C" int stag_slab_cg_control(stag_links_t *L, int *action_out)
+{
+    if (!L || !L->is_slab || !L->cg || !action_out) return STAG_EINVAL;
+    stag_slab_cg *C = L->cg;
+    CgCtrl *h = L->h_ctrl;
+    if (C->stage == 0) { C->stage = 1; *action_out = STAG_SLAB_ACT_NORM; return STAG_OK; }
+    if (C->stage == 3) { *action_out = STAG_SLAB_ACT_DONE; return STAG_OK; }
+    CU(cudaMemcpyAsync(h, C->w.ctrl, sizeof(CgCtrl), cudaMemcpyDeviceToHost, t_stream));
+    CU(cudaStreamSynchronize(t_stream));
+    if (C->stage == 1) {                       // |b|^2 (global) has arrived
+        C->bnorm2 = h->bnorm2[0];
+        if (C->bnorm2 == 0.0) {                // b = 0  =>  x = 0, nothing to iterate
+            CU(cudaMemsetAsync(C->x, 0, (size_t)C->n * sizeof(double), t_stream));
+            C->final_state = CG_CONVERGED;
+            C->stage = 3;
+            *action_out = STAG_SLAB_ACT_DONE;
+            return STAG_OK;
+        }
+        if (!(C->bnorm2 == C->bnorm2) || std::isinf(C->bnorm2)) {
+            C->final_state = CG_BREAKDOWN;
+            h->sum0[0] = NAN;
+            C->stage = 3;
+            *action_out = STAG_SLAB_ACT_DONE;
+            return STAG_OK;
+        }
+        h->tol2b[0] = C->tol * C->tol * C->bnorm2;
+        CU(cudaMemcpyAsync(C->w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, t_stream));
+        C->stage = 2;
+        C->have_true = true;
+        *action_out = STAG_SLAB_ACT_INIT;      // r = b - A x0, also sets y = 0
+        return STAG_OK;
+    }
+    const int state = h->state;
+    if (state == CG_RUN) {
+        if (C->verifying) ++C->n_restarts;
+        C->verifying = false;
+        C->have_true = false;
+        *action_out = STAG_SLAB_ACT_ITER;
+        return STAG_OK;
+    }
+    if (state == CG_UPDATE) {                  // section 3.2
+        C->have_true = true;
+        *action_out = STAG_SLAB_ACT_UPDATE;
+        return STAG_OK;
+    }
+    if (state == CG_CONVERGED && !C->have_true && C->mode == STAG_CG_F64) {   // Q6b
+        C->have_true = true;
+        C->verifying = true;
+        *action_out = STAG_SLAB_ACT_VERIFY;
+        return STAG_OK;
+    }
+    if (state == CG_CONVERGED && C->have_true) {
+        C->final_state = CG_CONVERGED;
+        C->stage = 3;
+        *action_out = STAG_SLAB_ACT_DONE;
+        return STAG_OK;
+    }
+    // CG_MAXITER or CG_BREAKDOWN (or a converged state without a true residual): report it
+    C->final_state = state;
+    if (!C->have_true) {
+        C->have_true = true;
+        *action_out = STAG_SLAB_ACT_FINAL;
+        return STAG_OK;
+    }
+    C->stage = 3;
+    *action_out = STAG_SLAB_ACT_DONE;
+    return STAG_OK;
+}
+
+// Enqueue phase `phase` of `action`.  *more_out = 1 while the action has further phases.  Within a
+// phase no kernel waits for a peer's kernel of the SAME phase, so ranks that share a device may be
+// stepped one after the other, phase by phase.
+extern "C" int stag_slab_cg_step(stag_links_t *L, int action, int phase, int *more_out)
+{
+    if (!L || !L->is_slab || !L->cg || phase < 0 || !more_out) return STAG_EINVAL;
+    stag_slab_cg *C = L->cg;
+    Workspace &w = C->w;
+    bool more = false;
+    int rc = STAG_EINVAL;
+    switch (action) {
+    case STAG_SLAB_ACT_NORM:
+        if (phase == 0) {
+            C->seq_res = ++C->red_seq;
+            slab_residual_kernel<float, RES_NORM><<<C->gb, BLAS_BLOCK, 0, t_stream>>>(nullptr, C->b, nullptr, nullptr, C->n, w.partials, w.ctrl, make_comm(L, C->seq_res));
+            count_launch();
+            KCHECK();
+            more = true;
+            rc = STAG_OK;
+        } else if (phase == 1) {
+            slab_scalar_kernel<RES_NORM><<<1, 32, 0, t_stream>>>(w.ctrl, make_comm(L, C->seq_res));
+            count_launch();
+            KCHECK();
+            rc = STAG_OK;
+        }
+        break;
+    case STAG_SLAB_ACT_INIT:
+        if (phase == 0 && C->lo) CU(cudaMemsetAsync(w.y32, 0, (size_t)C->n * sizeof(float), t_stream));
+        rc = slab_residual_phase<RES_INIT>(L, C, phase, false, C->lo, &more);
+        break;
+    case STAG_SLAB_ACT_VERIFY:
+        rc = slab_residual_phase<RES_INIT>(L, C, phase, false, false, &more);
+        break;
+    case STAG_SLAB_ACT_UPDATE:
+        rc = slab_residual_phase<RES_UPDATE>(L, C, phase, true, true, &more);
+        break;
+    case STAG_SLAB_ACT_FINAL:
+        rc = slab_residual_phase<RES_FINAL>(L, C, phase, C->lo, false, &more);
+        break;
+    case STAG_SLAB_ACT_ITER: {
+        const int total = 5 * C->P.graph_chunk;
+        if (phase >= total) return STAG_EINVAL;
+        more = phase + 1 < total;
+        if (C->lo) rc = slab_iteration_phase<float>(L, C, phase % 5, w.y32, w.r32, w.d32, w.q32, w.tmp32);
+        else rc = slab_iteration_phase<double>(L, C, phase % 5, C->x, w.r64, w.d64, w.q64, w.tmp64);
+        break;
+    }
+    default:
+        return STAG_EINVAL;
+    }
+    *more_out = more ? 1 : 0;
+    return rc;
+}
+
+extern "C" int stag_slab_cg_finish(stag_links_t *L, stag_cg_stats_t *stats_out)
+{
+    if (!L || !L->is_slab || !L->cg || L->cg->stage != 3) return STAG_EINVAL;
+    stag_slab_cg *C = L->cg;
+    CgCtrl *h = L->h_ctrl;
+    CU(cudaEventRecord(L->ev1, t_stream));
+    CU(cudaStreamSynchronize(t_stream));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, L->ev0, L->ev1));
+    stag_cg_stats_t st;
+    memset(&st, 0, sizeof(st));
+    st.iters = h->iters[0];
+    st.n_updates = h->n_updates;
+    st.n_restarts = C->n_restarts;
+    st.iters_f32 = C->lo ? h->iters[0] : 0;
+    st.applies_f64 = C->applies_f64;
+    st.true_resid = C->bnorm2 > 0.0 ? sqrt(h->sum0[0] / C->bnorm2) : 0.0;
+    st.iter_resid = C->bnorm2 > 0.0 ? sqrt(h->sum1[0] / C->bnorm2) : 0.0;
+    st.seconds = ms * 1e-3;
+    if (stats_out) *stats_out = st;
+    if (C->final_state == CG_BREAKDOWN) return STAG_EBREAKDOWN;
+    if (!(st.true_resid <= C->tol)) return STAG_ENOCONV;
+    return STAG_OK;
+}
+
+static void stag_slab_cg_free(struct stag_slab_cg *c) { delete c; }

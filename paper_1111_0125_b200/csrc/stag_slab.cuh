@@ -9,6 +9,12 @@
 // epoch into each neighbour's flag.  The consuming hop (dslash_kernel<..., HALO = true>) waits on
 // its own two flags only in the threads of the first and last time slice, which it visits last.
 //
+// The slab CG's global sums go through the same region: a rank stores its local total into slot
+// [seq & 1][its rank] of EVERY rank's XchReduce and then release-stores seq into flag[its rank];
+// whoever needs the sum acquire-waits for all nranks flags and adds the slots in rank order, so
+// every rank forms bit-identical alpha, beta and stopping decisions.  The wait always sits in a
+// kernel launched AFTER the publishing one on every rank, never in the same kernel.
+//
 // Exchange region of one slab (one allocation = one IPC handle), XCH_HDR bytes of header, then
 // halo buffers [epoch & 1][dir][colour][s3] of 16-byte complex slots (fp32 uses the front half):
 //   dir 0 = "back":  the neighbour slice x3 = -1,  written by rank-1 from its LAST slice
@@ -17,17 +23,25 @@
 // neighbours have finished consuming exchange e (its own hop e+1 waits for their push e+1, which
 // follows their hop e in stream order).
 #pragma once
+#include "stag_blas.cuh"
 #include "stag_common.cuh"
 
 namespace stag {
 
-constexpr size_t XCH_HDR = 256;
+constexpr size_t XCH_HDR = 1024;
+constexpr size_t XCH_RED = 256;     // offset of XchReduce inside the header area
+constexpr int MAX_RANKS = STAG_MAX_RANKS;
+struct XchReduce {
+    unsigned long long flag[MAX_RANKS];   // flag[r]: last reduction number rank r has published here
+    double slot[2][MAX_RANKS];            // slot[seq & 1][r]: rank r's local total of reduction seq
+};
+static_assert(XCH_RED + sizeof(XchReduce) <= XCH_HDR, "reduction slots must fit the header area");
 struct XchHeader {
     unsigned long long flag_back;   // epoch of the last completed push into my "back" halo
     unsigned long long flag_fwd;    // ... into my "fwd" halo
     unsigned ticket;                // last-block ticket of MY face_push_kernel (never peer-written)
 };
-static_assert(sizeof(XchHeader) <= XCH_HDR, "exchange header must fit its slot");
+static_assert(sizeof(XchHeader) <= XCH_RED, "exchange header must fit its slot");
 
 inline size_t xch_halo_offset(int s3, unsigned long long epoch, int dir)
 {
@@ -61,6 +75,139 @@ face_push_kernel(const cplx_t<T> *__restrict__ in, const int Vh, const int Vh_pa
         asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(fwd_flag_back), "l"(epoch) : "memory");
         asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(bwd_flag_fwd), "l"(epoch) : "memory");
     }
+}
+
+// ---- global sums of the slab CG ---------------------------------------------------------
+// One thread: store my local total of reduction seq into every rank's slots, then the flags.
+__device__ __forceinline__ void publish_total(char *const *peers, int nranks, int myrank,
+                                              unsigned long long seq, double value)
+{
+    for (int r = 0; r < nranks; ++r) {
+        XchReduce *R = (XchReduce *)(peers[r] + XCH_RED);
+        *(volatile double *)&R->slot[seq & 1ull][myrank] = value;
+    }
+    __threadfence_system();
+    for (int r = 0; r < nranks; ++r) {
+        XchReduce *R = (XchReduce *)(peers[r] + XCH_RED);
+        asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&R->flag[myrank]), "l"(seq) : "memory");
+    }
+}
+
+// Any thread: the sum over ranks of reduction seq, added in rank order (same bits on every rank).
+__device__ __forceinline__ double gather_total(const char *mine, int nranks, unsigned long long seq)
+{
+    const XchReduce *R = (const XchReduce *)(mine + XCH_RED);
+    double t = 0.0;
+    for (int r = 0; r < nranks; ++r) {
+        wait_flag(&R->flag[r], seq);
+        t += __ldcg(&R->slot[seq & 1ull][r]);
+    }
+    return t;
+}
+
+// Comm: what a kernel of the slab CG needs to publish / gather (passed by value)
+struct Comm {
+    char *const *peers;     // device array of nranks pointers to every rank's exchange region
+    const char *mine;
+    int nranks, myrank;
+    unsigned long long seq; // number of THIS launch's reduction (publish) or of the one to gather
+};
+
+// Local fixed-order sum of the second hop's per-block partials of <d,Ad>, published to all ranks.
+__global__ void __launch_bounds__(BLAS_BLOCK)
+slab_publish_partials_kernel(const double *__restrict__ partials, int n, const Comm c,
+                             const CgCtrl *__restrict__ ctrl)
+{
+    if (ctrl->state != CG_RUN) return;
+    __shared__ double red[32];
+    const double t = block_total_fixed(partials, n, red);
+    if (threadIdx.x == 0) publish_total(c.peers, c.nranks, c.myrank, c.seq, t);
+}
+
+// update_kernel for one right-hand side of a slab: <d,Ad> is the all-rank sum of reduction
+// c_in.seq; the local |r|^2 is published as reduction c_out.seq instead of running the epilogue.
+template <typename T>
+__global__ void __launch_bounds__(BLAS_BLOCK)
+slab_update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
+                   const T *__restrict__ q, long n, double *__restrict__ partials,
+                   CgCtrl *__restrict__ ctrl, const Comm c_in, const Comm c_out)
+{
+    if (ctrl->state != CG_RUN) return;
+    using V = typename Vec4<T>::type;
+    constexpr int N = Vec4<T>::N;
+    __shared__ double red[32];
+    __shared__ double totals[MAX_RHS];
+    __shared__ double s_dAd;
+    if (threadIdx.x == 0) s_dAd = gather_total(c_in.mine, c_in.nranks, c_in.seq);
+    __syncthreads();
+    const double dAd = s_dAd;
+    const bool ok = dAd > 0.0;
+    const double alpha_d = ok ? ctrl->delta[0] / dAd : 0.0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) { ctrl->dAd[0] = dAd; ctrl->alpha[0] = alpha_d; }
+    const T alpha = (T)alpha_d;
+    const long nv = n / N;
+    V *yk = reinterpret_cast<V *>(y);
+    V *rk = reinterpret_cast<V *>(r);
+    const V *dk = reinterpret_cast<const V *>(d);
+    const V *qk = reinterpret_cast<const V *>(q);
+    double s = 0.0;
+    for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)gridDim.x * BLAS_BLOCK) {
+        T yy[N], rr[N], dd[N], qq[N];
+        unpack<T>(ld_pass(yk + i), yy);
+        unpack<T>(ld_keep(rk + i), rr);
+        unpack<T>(ld_keep(dk + i), dd);
+        unpack<T>(ld_keep(qk + i), qq);
+#pragma unroll
+        for (int j = 0; j < N; ++j) {
+            yy[j] = fma(alpha, dd[j], yy[j]);
+            rr[j] = fma(-alpha, qq[j], rr[j]);
+            s += (double)rr[j] * (double)rr[j];
+        }
+        st_pass(yk + i, pack(yy));
+        st_keep(rk + i, pack(rr));
+    }
+    const double bs = block_sum(s, red);
+    if (!finish_reduction(bs, partials, &ctrl->ticket[1], red, totals)) return;
+    if (threadIdx.x == 0) publish_total(c_out.peers, c_out.nranks, c_out.myrank, c_out.seq, totals[0]);
+}
+
+// residual_kernel for one right-hand side of a slab: publishes the local |r|^2 (or |b|^2).
+template <typename T, int WHAT>
+__global__ void __launch_bounds__(BLAS_BLOCK)
+slab_residual_kernel(double *__restrict__ r, const double *__restrict__ b,
+                     const double *__restrict__ q, T *__restrict__ r_lo, long n,
+                     double *__restrict__ partials, CgCtrl *__restrict__ ctrl, const Comm c_out)
+{
+    double s = 0.0;
+    for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < n; i += (long)gridDim.x * BLAS_BLOCK) {
+        if (WHAT == RES_NORM) {
+            const double v = b[i];
+            s += v * v;
+        } else {
+            const double v = b[i] - q[i];
+            r[i] = v;
+            if (r_lo != nullptr) r_lo[i] = (T)v;
+            s += v * v;
+        }
+    }
+    __shared__ double red[32];
+    __shared__ double totals[MAX_RHS];
+    const double bs = block_sum(s, red);
+    if (!finish_reduction(bs, partials, &ctrl->ticket[2], red, totals)) return;
+    if (threadIdx.x == 0) publish_total(c_out.peers, c_out.nranks, c_out.myrank, c_out.seq, totals[0]);
+}
+
+// The scalar step that follows a published reduction: gather the all-rank sum and run the same
+// epilogue the one-GPU kernels run in their last block.  WHAT: RES_* or SCALAR_ITER.
+enum { SCALAR_ITER = 100 };
+template <int WHAT>
+__global__ void slab_scalar_kernel(CgCtrl *__restrict__ ctrl, const Comm c_in)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    if (WHAT == SCALAR_ITER && ctrl->state != CG_RUN) return;
+    double total = gather_total(c_in.mine, c_in.nranks, c_in.seq);
+    if (WHAT == SCALAR_ITER) cg_iteration_epilogue(ctrl, &total);
+    else residual_epilogue<WHAT>(ctrl, &total);
 }
 
 }  // namespace stag

@@ -20,6 +20,7 @@ import ctypes
 import paper_1111_0125_b200 as stag
 
 IPC_HANDLE_BYTES = 64
+ACT_DONE, ACT_NORM, ACT_INIT, ACT_ITER, ACT_UPDATE, ACT_VERIFY, ACT_FINAL = range(7)
 
 
 # ---- pure host logic ---------------------------------------------------------------------
@@ -73,9 +74,8 @@ def gather_spinor(parts, global_dims):
     return out
 
 
-def exchange_handles(my_handle: bytes, rank: int, nranks: int, group=None):
-    """All ranks' IPC handles through torch.distributed (any backend); returns the
-    (backward, forward) neighbours' handles."""
+def all_handles(my_handle: bytes, nranks: int, group=None):
+    """Every rank's IPC handle, in rank order, through torch.distributed (any backend)."""
     import torch.distributed as dist
     if len(my_handle) != IPC_HANDLE_BYTES:
         raise ValueError("an IPC handle is %d bytes" % IPC_HANDLE_BYTES)
@@ -84,6 +84,12 @@ def exchange_handles(my_handle: bytes, rank: int, nranks: int, group=None):
         raise ValueError("group has %d ranks, the decomposition %d" % (world, nranks))
     allh = [None] * world
     dist.all_gather_object(allh, bytes(my_handle), group=group)
+    return allh
+
+
+def exchange_handles(my_handle: bytes, rank: int, nranks: int, group=None):
+    """The (backward, forward) neighbours' handles."""
+    allh = all_handles(my_handle, nranks, group)
     b, f = neighbours(rank, nranks)
     return allh[b], allh[f]
 
@@ -125,19 +131,67 @@ class SlabLinks:
     def connect_pointers(self, bwd_ptr: int, fwd_ptr: int):
         stag._check(stag.lib().stag_slab_connect(self._h, ctypes.c_void_p(bwd_ptr), ctypes.c_void_p(fwd_ptr)))
 
+    def connect_all_pointers(self, ptrs):
+        """ptrs[r]: device-accessible address of rank r's exchange region (own included)."""
+        arr = (ctypes.c_void_p * self.nranks)(*[ctypes.c_void_p(p) for p in ptrs])
+        stag._check(stag.lib().stag_slab_connect_all(self._h, arr))
+
     def connect_distributed(self, group=None):
-        """One process per GPU: exchange IPC handles over torch.distributed and map the two
-        neighbours' exchange regions into this process."""
+        """One process per GPU: exchange IPC handles over torch.distributed and map every other
+        rank's exchange region into this process (the hop needs the two neighbours, the CG's
+        global sums every rank)."""
         if self.nranks == 1:
             return
-        hb, hf = exchange_handles(self.ipc_handle(), self.rank, self.nranks, group)
+        allh = all_handles(self.ipc_handle(), self.nranks, group)
         ptrs = []
-        for h in (hb, hf):
+        for r, h in enumerate(allh):
+            if r == self.rank:
+                ptrs.append(self.exchange_region()[0])
+                continue
             p = ctypes.c_void_p()
             stag._check(stag.lib().stag_slab_ipc_open(ctypes.c_char_p(h), ctypes.byref(p)))
             ptrs.append(p.value)
             self._opened.append(p.value)
-        self.connect_pointers(ptrs[0], ptrs[1])
+        self.connect_all_pointers(ptrs)
+
+    # -- CG over the slabs: control flow only, every decision is taken in the library --------
+    def cg_begin(self, x, b, mass, tol, maxiter, mode, eps_in=None, recon12=False, chunk=None, recon12_f64=False):
+        stag.use_current_stream()
+        p = stag._params(eps_in, recon12, chunk, recon12_f64)
+        stag._check(stag.lib().stag_slab_cg_begin(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(b.data_ptr()),
+                                                  float(mass), float(tol), int(maxiter), int(mode), ctypes.byref(p)))
+
+    def cg_control(self) -> int:
+        stag.use_current_stream()
+        a = ctypes.c_int()
+        stag._check(stag.lib().stag_slab_cg_control(self._h, ctypes.byref(a)))
+        return a.value
+
+    def cg_step(self, action: int, phase: int) -> bool:
+        more = ctypes.c_int()
+        stag._check(stag.lib().stag_slab_cg_step(self._h, int(action), int(phase), ctypes.byref(more)))
+        return bool(more.value)
+
+    def cg_finish(self):
+        st = stag._Stats()
+        rc = stag.lib().stag_slab_cg_finish(self._h, ctypes.byref(st))
+        stag._check(rc, allow=(stag.OK, stag.ENOCONV, stag.EBREAKDOWN))
+        return stag._stats_dict(st, rc)
+
+    def cg_solve(self, b, mass, tol, maxiter, mode=stag.CG_RELIABLE, x0=None, **kw):
+        """This rank's part of the solve in a real multi-GPU run (one process per GPU, all ranks
+        call it together).  b, x0: fp64 device spinors of the local dims.  Returns (x, stats)."""
+        torch = stag._require_cuda()
+        x = torch.zeros_like(b) if x0 is None else x0.clone()
+        self.cg_begin(x, b, mass, tol, maxiter, mode, **kw)
+        while True:
+            act = self.cg_control()
+            if act == ACT_DONE:
+                break
+            ph = 0
+            while self.cg_step(act, ph):
+                ph += 1
+        return x, self.cg_finish()
 
     # -- the operator; spinors are device spinors of the LOCAL dims -------------------------
     def push(self, v, prec):
@@ -180,12 +234,34 @@ class SlabLinks:
 
 
 def connect_in_process(slabs):
-    """Slabs that live in one process (one GPU holding several, or tests): hand each its
-    neighbours' exchange regions as raw device pointers."""
+    """Slabs that live in one process (one GPU holding several, or tests): hand each every
+    rank's exchange region as raw device pointers."""
     n = len(slabs)
     ptrs = [s.exchange_region()[0] for s in slabs]
     for r, s in enumerate(slabs):
         if s.rank != r or s.nranks != n:
             raise ValueError("slabs must be given in rank order, all of them")
-        b, f = neighbours(r, n)
-        s.connect_pointers(ptrs[b], ptrs[f])
+        s.connect_all_pointers(ptrs)
+
+
+def cg_solve_in_process(slabs, bs, mass, tol, maxiter, mode=stag.CG_RELIABLE, **kw):
+    """The multi-GPU solve with all slabs in THIS process on one device: every phase is enqueued
+    for rank 0, 1, ... before the next phase, so a kernel that waits for its peers always finds
+    their kernels already launched.  bs[r]: rank r's fp64 device spinor.  Returns (xs, [stats])."""
+    torch = stag._require_cuda()
+    xs = [torch.zeros_like(b) for b in bs]
+    for s, x, b in zip(slabs, xs, bs):
+        s.cg_begin(x, b, mass, tol, maxiter, mode, **kw)
+    while True:
+        acts = [s.cg_control() for s in slabs]
+        if any(a != acts[0] for a in acts):
+            raise RuntimeError("ranks disagree on the next action: %r" % (acts,))
+        if acts[0] == ACT_DONE:
+            break
+        ph = 0
+        while True:
+            more = [s.cg_step(acts[0], ph) for s in slabs]
+            if not more[0]:
+                break
+            ph += 1
+    return xs, [s.cg_finish() for s in slabs]

@@ -124,3 +124,74 @@ def test_single_rank_slab_dslash_entry_and_argument_errors():
     two = slab.SlabLinks((4, 4, 4, 8), fieldgen.links((4, 4, 4, 8), "random", seed=1), 0, 2)
     v8 = stag.empty_spinor(two.dims, 0)
     assert lib.stag_slab_push(vp(v8.data_ptr()), two.handle, 0) == stag.EINVAL   # not connected yet
+
+
+# ---- CG over the slabs -------------------------------------------------------------------
+def _slab_cg(cfg, W, b, nranks, mode, **kw):
+    slabs = make_slabs(cfg.dims, W, nranks)
+    bs = [stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(b, cfg.dims, r, nranks)), slabs[r].dims, 0)
+          for r in range(nranks)]
+    xs, sts = slab.cg_solve_in_process(slabs, bs, cfg.mass, cfg.tol, cfg.maxiter, mode, **kw)
+    x = slab.gather_spinor([stag.spinor_unpack(xs[r], slabs[r].dims, 0) for r in range(nranks)], cfg.dims)
+    return x, sts
+
+
+@pytest.mark.parametrize("nranks", [1, 2, 4])
+@pytest.mark.parametrize("mode", [stag.CG_F64, stag.CG_RELIABLE])
+def test_slab_cg_matches_oracle(nranks, mode):
+    """The multi-GPU solve, all ranks on one device: x against the oracle's solve (to 1e-12),
+    the fp64 true residual recomputed with the oracle's A, iteration count within a few % of
+    the oracle's (Q17), and every rank reporting the same scalars."""
+    cfg = fieldgen.CONFIGS["c2_8^4"]
+    W, b = cfg.links(), cfg.source()
+    x, sts = _slab_cg(cfg, W, b, nranks, mode)
+    x_ref, _, _, _, rc = oracle.cg(b, W, cfg.dims, cfg.mass, 1e-12, 10 * cfg.maxiter)
+    _, it10, _, _, _ = oracle.cg(b, W, cfg.dims, cfg.mass, cfg.tol, cfg.maxiter)
+    assert rc == 0
+    for st in sts:
+        assert st["status"] == stag.OK and st["true_resid"] <= cfg.tol
+        assert (st["iters"], st["true_resid"], st["n_updates"]) == (sts[0]["iters"], sts[0]["true_resid"], sts[0]["n_updates"])
+    assert abs(sts[0]["iters"] - it10) <= 0.05 * it10 + 3
+    res = np.linalg.norm((b - oracle.apply_A(x, W, cfg.dims, cfg.mass)).ravel()) / np.linalg.norm(b.ravel())
+    assert res <= cfg.tol * (1 + 1e-3)
+    assert rel_l2(x, x_ref) <= 1e-8
+    if mode == stag.CG_RELIABLE:
+        assert sts[0]["n_updates"] >= 1 and sts[0]["iters_f32"] == sts[0]["iters"]
+
+
+def test_slab_cg_one_rank_equals_whole_lattice_solver_bitwise():
+    """nranks = 1: the global sums have one term, so the slab path must reproduce the one-GPU
+    solver's iterates exactly (same kernels' arithmetic, same reduction order)."""
+    import torch
+    cfg = fieldgen.CONFIGS["c1_4^4"]
+    W, b = cfg.links(), cfg.source()
+    L = stag.Links(cfg.dims, W)
+    bd = stag.spinor_pack(b, cfg.dims, 0)
+    for mode in (stag.CG_F64, stag.CG_RELIABLE):
+        x1, st1 = stag.cg_solve(bd, L, cfg.mass, cfg.tol, cfg.maxiter, mode)
+        S = make_slabs(cfg.dims, W, 1)
+        xs, sts = slab.cg_solve_in_process(S, [bd], cfg.mass, cfg.tol, cfg.maxiter, mode)
+        assert sts[0]["iters"] == st1["iters"] and sts[0]["n_updates"] == st1["n_updates"]
+        assert torch.equal(xs[0], x1)
+
+
+def test_slab_cg_degenerate_cases():
+    cfg = fieldgen.CONFIGS["c1_4^4"]
+    W, b = cfg.links(), cfg.source()
+    # b = 0 -> x = 0, no iterations
+    x, sts = _slab_cg(cfg, W, np.zeros_like(b), 2, stag.CG_RELIABLE)
+    assert not x.any() and sts[0]["iters"] == 0 and sts[0]["status"] == stag.OK
+    # maxiter = 3 -> ENOCONV with the true residual reported, same on both ranks
+    slabs = make_slabs(cfg.dims, W, 2)
+    bs = [stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(b, cfg.dims, r, 2)), slabs[r].dims, 0) for r in range(2)]
+    xs, sts = slab.cg_solve_in_process(slabs, bs, cfg.mass, cfg.tol, 3, stag.CG_RELIABLE)
+    assert sts[0]["status"] == stag.ENOCONV and sts[0]["iters"] == 3 and sts[0]["true_resid"] > cfg.tol
+    assert sts[0]["true_resid"] == sts[1]["true_resid"]
+    x = slab.gather_spinor([stag.spinor_unpack(xs[r], slabs[r].dims, 0) for r in range(2)], cfg.dims)
+    res = np.linalg.norm((b - oracle.apply_A(x, W, cfg.dims, cfg.mass)).ravel()) / np.linalg.norm(b.ravel())
+    assert abs(res - sts[0]["true_resid"]) <= 1e-12 * max(1.0, res)
+    # a plane-wave source on the free field converges in one iteration on four ranks
+    cfgf = fieldgen.CONFIGS["c2_8^4_free"]
+    pw = fieldgen.spinor_planewave(cfgf.dims, (1, 2, 3, 0))
+    x, sts = _slab_cg(cfgf, cfgf.links(), pw, 4, stag.CG_F64)
+    assert sts[0]["iters"] == 1 and rel_l2(x, pw / 8.588286437626904) <= 1e-12
