@@ -178,9 +178,12 @@ class SlabLinks:
         stag._check(rc, allow=(stag.OK, stag.ENOCONV, stag.EBREAKDOWN))
         return stag._stats_dict(st, rc)
 
-    def cg_solve(self, b, mass, tol, maxiter, mode=stag.CG_RELIABLE, x0=None, **kw):
+    def cg_solve(self, b, mass, tol, maxiter, mode=stag.CG_RELIABLE, x0=None, after_phase=None, **kw):
         """This rank's part of the solve in a real multi-GPU run (one process per GPU, all ranks
-        call it together).  b, x0: fp64 device spinors of the local dims.  Returns (x, stats)."""
+        call it together).  b, x0: fp64 device spinors of the local dims.  Returns (x, stats).
+        after_phase: called after every enqueued phase; ranks that SHARE a device pass a
+        "synchronise + barrier" here so that no kernel ever waits for a kernel of another
+        process that has not run yet (tests; never needed with one GPU per rank)."""
         torch = stag._require_cuda()
         x = torch.zeros_like(b) if x0 is None else x0.clone()
         self.cg_begin(x, b, mass, tol, maxiter, mode, **kw)
@@ -189,7 +192,12 @@ class SlabLinks:
             if act == ACT_DONE:
                 break
             ph = 0
-            while self.cg_step(act, ph):
+            while True:
+                more = self.cg_step(act, ph)
+                if after_phase is not None:
+                    after_phase()
+                if not more:
+                    break
                 ph += 1
         return x, self.cg_finish()
 
