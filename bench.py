@@ -340,6 +340,110 @@ def run_ours(args):
     return 0
 
 
+def run_slabs(args):
+    """--decomp slabs: ONE lattice split along time over the N ranks (strong scaling): the T-slab
+    hop with peer-to-peer halo exchange and the slab CG with its global sums through peer memory
+    (DESIGN.md section 14).  One process per GPU; torch.distributed only carries the IPC handles,
+    the barrier around the timed region and the max over ranks of the time."""
+    import numpy as np
+    import torch
+    import fieldgen
+    import paper_1111_0125_b200 as stag
+    from paper_1111_0125_b200 import replicas, slab
+
+    if not torch.cuda.is_available():
+        print("bench.py: no CUDA device; the hot path has no CPU fallback", file=sys.stderr)
+        return 2
+    rank, local, world = replicas.init("nccl")
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    stag.lib()
+    cfg = fieldgen.CONFIGS[args.config]
+    peak, peak_src = measured_peaks()
+    W = cfg.links()
+    b_np = cfg.source()
+    S = slab.SlabLinks(cfg.dims, W, rank, world)
+    del W
+    S.connect_distributed()
+    b_loc = np.ascontiguousarray(slab.scatter_spinor(b_np, cfg.dims, rank, world))
+    b_dev = stag.spinor_pack(b_loc, S.dims, stag.PREC_F64)
+    b_host = torch.from_numpy(b_loc.view(np.float64).reshape(-1).copy()).pin_memory()
+    x_host = torch.zeros_like(b_host).pin_memory()
+
+    def solve_device():
+        return S.cg_solve(b_dev, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True)
+
+    def solve_host():
+        bd = stag.spinor_pack(b_host.to(dev, non_blocking=True), S.dims, stag.PREC_F64)
+        x, st = S.cg_solve(bd, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True)
+        x_host.copy_(stag.spinor_unpack(x, S.dims, stag.PREC_F64, to_numpy=False))
+        return x, st
+
+    def timed(fn, steps, warmup):
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize(); replicas.barrier(); torch.cuda.synchronize()
+        stag.reset_launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        last = None
+        for _ in range(steps):
+            _, last = fn()
+        e1.record()
+        torch.cuda.synchronize(); replicas.barrier(); torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3, last, stag.launch_count()
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    sec, st, launches = timed(solve_device, args.steps, args.warmup)
+    clocks = sampler.stop() if sampler else None
+    tmax = replicas.max_over_ranks(sec, dev)
+    flops = args.steps * st["iters"] * FLOP_PER_SITE_ITER * cfg.vh          # the whole lattice
+    sec_e2e, st_e2e, _ = timed(solve_host, args.steps, 1)
+    tmax_e2e = replicas.max_over_ranks(sec_e2e, dev)
+
+    # the slab hop alone (push + hop), this rank's share of the lattice
+    vh_loc = cfg.vh // world
+    prec = stag.PREC_F32_R12
+    vs = [stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(fieldgen.spinor_gaussian(cfg.dims, 0, seed=100 + i), cfg.dims, rank, world)), S.dims, prec) for i in range(4)]
+    outs = [stag.empty_spinor(S.dims, prec) for _ in range(4)]
+    for i in range(4):
+        S.dslash(vs[i], 1, prec, out=outs[i])
+    torch.cuda.synchronize(); replicas.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(40):
+        S.dslash(vs[i % 4], 1, prec, out=outs[i % 4])
+    e1.record()
+    torch.cuda.synchronize(); replicas.barrier()
+    hop_us = replicas.max_over_ranks(e0.elapsed_time(e1) / 40 * 1e3, dev)
+    if rank != 0:
+        replicas.finalize()
+        return 0
+    hop_bytes = 432 * vh_loc
+    line = {
+        "metric": METRIC, "value": flops / tmax * 1e-9, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": tmax / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "strong", "vs_baseline": None, "dtype": "f32 iteration + f64 reliable updates",
+        "data": "synthetic",
+        "config": workload_config(cfg, world, parallelism="T-slabs x%d: peer-to-peer halo exchange per hop, two global sums per iteration through peer memory" % world),
+        "e2e": {"value": args.steps * st_e2e["iters"] * FLOP_PER_SITE_ITER * cfg.vh / tmax_e2e * 1e-9, "unit": UNIT,
+                "h2d_bytes_per_step": cfg.vh * 48, "d2h_bytes_per_step": cfg.vh * 48,
+                "ms_per_step": tmax_e2e / args.steps * 1e3,
+                "entry": "slab.SlabLinks.cg_solve with each rank's b in pinned host memory and x copied back"},
+        "gpu_launches": int(launches), "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": "face_push_kernel + dslash_kernel<float,2,PLAIN,1,HALO> on one slab",
+                     "achieved": hop_bytes / hop_us * 1e-3, "peak": peak, "unit": "GB/s",
+                     "frac": hop_bytes / hop_us * 1e-3 / peak, "peak_source": peak_src, "traffic": None,
+                     "algorithmic_bytes_per_launch": hop_bytes, "us_per_launch": hop_us},
+        "cpu_baseline": None,
+        "cg": {"iters": st["iters"], "n_updates": st["n_updates"], "true_resid": st["true_resid"],
+               "time_to_solution_s": st["seconds"], "ms_per_iteration": st["seconds"] / max(1, st["iters"]) * 1e3},
+    }
+    print(json.dumps(line), flush=True)
+    replicas.finalize()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -348,12 +452,16 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", default="c4_28^3x96")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--decomp", choices=["replicas", "slabs"], default="replicas",
+                    help="N > 1: independent replicas (weak scaling, default) or one lattice in T-slabs (strong)")
     ap.add_argument("--traffic", type=float, default=436.4e6,
                     help="dram bytes (read + write) per launch of the dominant kernel from the ncu --set full "
                          "capture profiles/r1b_dslash_fp32r12_ncu_full.md (28^3x96, fp32/12 plain hop)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.decomp == "slabs":
+        return run_slabs(args)
     return run_ours(args)
 
 

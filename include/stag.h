@@ -312,6 +312,10 @@ int stag_slab_cg_control(stag_links_t *slab, int *action_out);
 int stag_slab_cg_step(stag_links_t *slab, int action, int phase, int *more_out);
 /* Returns STAG_OK / STAG_ENOCONV / STAG_EBREAKDOWN like stag_cg_solve; stats as there. */
 int stag_slab_cg_finish(stag_links_t *slab, stag_cg_stats_t *stats_out);
+/* begin + the loop above + finish: the call of a one-process-per-GPU run (all ranks together).
+ * NOT for slabs sharing a device: there a waiting kernel would block the kernel it waits for. */
+int stag_slab_cg_run(stag_links_t *slab, void *x_even, const void *b_even, double mass, double tol,
+                     int maxiter, int mode, const stag_cg_params_t *params, stag_cg_stats_t *stats_out);
 
 #ifdef __cplusplus
 }

@@ -130,6 +130,8 @@ SIGNATURES = {
     "stag_slab_cg_control": (ctypes.c_int, [_vp, _ip]),
     "stag_slab_cg_step": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _ip]),
     "stag_slab_cg_finish": (ctypes.c_int, [_vp, ctypes.POINTER(_Stats)]),
+    "stag_slab_cg_run": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
+                                        ctypes.c_int, ctypes.POINTER(_Params), ctypes.POINTER(_Stats)]),
     "stag_cg_solve_host": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double,
                                           ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Params),
                                           ctypes.POINTER(_Stats)]),

@@ -1468,4 +1468,24 @@ extern "C" int stag_slab_cg_finish(stag_links_t *L, stag_cg_stats_t *stats_out)
     return STAG_OK;
 }
 
+// begin + the control / step loop + finish in one call: what each process of a one-process-per-GPU
+// run uses (every rank calls it at the same time; kernels of a phase may wait for peers' kernels
+// of earlier phases, which are running or queued on the OTHER devices).
+extern "C" int stag_slab_cg_run(stag_links_t *L, void *x_even, const void *b_even, double mass,
+                                double tol, int maxiter, int mode, const stag_cg_params_t *params,
+                                stag_cg_stats_t *stats_out)
+{
+    int rc = stag_slab_cg_begin(L, x_even, b_even, mass, tol, maxiter, mode, params);
+    if (rc) return rc;
+    for (;;) {
+        int act = STAG_SLAB_ACT_DONE;
+        if ((rc = stag_slab_cg_control(L, &act))) return rc;
+        if (act == STAG_SLAB_ACT_DONE) break;
+        int more = 1;
+        for (int ph = 0; more; ++ph)
+            if ((rc = stag_slab_cg_step(L, act, ph, &more))) return rc;
+    }
+    return stag_slab_cg_finish(L, stats_out);
+}
+
 static void stag_slab_cg_free(struct stag_slab_cg *c) { delete c; }

@@ -186,6 +186,15 @@ class SlabLinks:
         process that has not run yet (tests; never needed with one GPU per rank)."""
         torch = stag._require_cuda()
         x = torch.zeros_like(b) if x0 is None else x0.clone()
+        if after_phase is None:                 # the whole loop in the library: stag_slab_cg_run
+            stag.use_current_stream()
+            st = stag._Stats()
+            p = stag._params(kw.get("eps_in"), kw.get("recon12", False), kw.get("chunk"), kw.get("recon12_f64", False))
+            rc = stag.lib().stag_slab_cg_run(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(b.data_ptr()),
+                                             float(mass), float(tol), int(maxiter), int(mode), ctypes.byref(p),
+                                             ctypes.byref(st))
+            stag._check(rc, allow=(stag.OK, stag.ENOCONV, stag.EBREAKDOWN))
+            return x, stag._stats_dict(st, rc)
         self.cg_begin(x, b, mass, tol, maxiter, mode, **kw)
         while True:
             act = self.cg_control()

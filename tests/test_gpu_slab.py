@@ -195,3 +195,16 @@ def test_slab_cg_degenerate_cases():
     pw = fieldgen.spinor_planewave(cfgf.dims, (1, 2, 3, 0))
     x, sts = _slab_cg(cfgf, cfgf.links(), pw, 4, stag.CG_F64)
     assert sts[0]["iters"] == 1 and rel_l2(x, pw / 8.588286437626904) <= 1e-12
+
+
+def test_slab_cg_run_single_call_on_one_rank():
+    """stag_slab_cg_run (the call of a one-process-per-GPU run) on a one-slab decomposition:
+    same iterates as the stepped loop."""
+    import torch
+    cfg = fieldgen.CONFIGS["c1_4^4"]
+    W, b = cfg.links(), cfg.source()
+    bd = stag.spinor_pack(b, cfg.dims, 0)
+    S = make_slabs(cfg.dims, W, 1)
+    xs, sts = slab.cg_solve_in_process(S, [bd], cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE)
+    x, st = S[0].cg_solve(bd, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE)
+    assert st["iters"] == sts[0]["iters"] and torch.equal(x, xs[0])
