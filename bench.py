@@ -178,9 +178,10 @@ def time_dslash(stag, torch, fieldgen, cfg, L, prec, launches=60, nrot=6):
     e1.record()
     torch.cuda.synchronize()
     sec = e0.elapsed_time(e1) * 1e-3 / launches
-    f32 = prec in (stag.PREC_F32, stag.PREC_F32_R12)
-    rows = 2 if prec in (stag.PREC_F64_R12, stag.PREC_F32_R12) else 3
-    bytes_site = (8 * 6 * rows + 6 + 6) * (4 if f32 else 8)     # 8 links + 1 vector in + 1 out
+    f32 = prec in (stag.PREC_F32, stag.PREC_F32_R12, stag.PREC_F32_R8)
+    reals = {stag.PREC_F64: 18, stag.PREC_F32: 18, stag.PREC_F64_R12: 12, stag.PREC_F32_R12: 12,
+             stag.PREC_F64_R8: 8, stag.PREC_F32_R8: 8}[prec]
+    bytes_site = (8 * reals + 6 + 6) * (4 if f32 else 8)        # 8 links + 1 vector in + 1 out
     paper_bytes = (8 * 18 + 8 * 6 + 6) * (4 if f32 else 8)      # P:L62 convention, no reuse
     return {"us": sec * 1e6, "algorithmic_bytes_per_site": bytes_site,
             "gbs": bytes_site * cfg.vh / sec * 1e-9, "gflops": FLOP_PER_SITE_HOP * cfg.vh / sec * 1e-9,
@@ -278,7 +279,9 @@ def run_ours(args):
         return 0
 
     # ---- rank 0, N = any: the per-kernel numbers and the CPU baseline ---------------------------
-    dsl = {stag.PREC_NAMES[p]: time_dslash(stag, torch, fieldgen, cfg, L, p) for p in range(4)}
+    dsl = {stag.PREC_NAMES[p]: time_dslash(stag, torch, fieldgen, cfg, L, p) for p in range(6)}
+    dsl["fp32/8"]["rebuilt_entry_error"] = L.recon8_error(stag.PREC_F32_R8)
+    dsl["fp64/8"]["rebuilt_entry_error"] = L.recon8_error(stag.PREC_F64_R8)
     dom = dsl["fp32/12"]
     roofline = {"bound": "hbm", "kernel": "dslash_kernel<float,2,*> (fp32, 12-real links: the hop of the timed solve)",
                 "achieved": dom["gbs"], "peak": peak, "unit": "GB/s", "frac": dom["gbs"] / peak,

@@ -69,7 +69,14 @@ enum {
     STAG_PREC_F64    = 0,
     STAG_PREC_F32    = 1,
     STAG_PREC_F64_R12 = 2,
-    STAG_PREC_F32_R12 = 3
+    STAG_PREC_F32_R12 = 3,
+    /* 8-parameter form (the paper names and rejects it for its round-off; its Ref. [6]):
+     * four complex slots per link, a2, a3, b1 and the phases of a1 and c1; the rest follows from
+     * unitarity and det = +-1 with a division by |a2|^2+|a3|^2.  Whole-lattice handles only;
+     * refused (STAG_EINVAL) for fields whose rebuilt entries are off by more than 1e-9 (fp64) /
+     * 1e-3 (fp32), e.g. unit links.  A measured accuracy / bandwidth trade-off next to 12-real. */
+    STAG_PREC_F64_R8  = 4,
+    STAG_PREC_F32_R8  = 5
 };
 
 /* ---- CG modes ---------------------------------------------------------- */
@@ -128,6 +135,10 @@ void stag_links_destroy(stag_links_t *links);
 /* Largest | row2 - s conj(row0 x row1) | over all links, measured when the handle was made.
  * 12-real precisions are refused (STAG_EINVAL) when it exceeds 1e-10. */
 int stag_links_recon_error(const stag_links_t *links, double *err_out);
+/* The same for the 8-parameter form of precision prec (STAG_PREC_F64_R8 / _F32_R8), rebuilt in
+ * that precision's arithmetic exactly as the hop rebuilds it.  Builds the form on first use;
+ * returns STAG_EINVAL (with *err_out still set) when the field is refused. */
+int stag_links_recon8_error(const stag_links_t *links, int prec, double *err_out);
 
 /* ---- spinors ----------------------------------------------------------- */
 
@@ -222,6 +233,7 @@ typedef struct stag_cg_params {
     int    graph_chunk;   /* CG iterations per CUDA-graph replay between host checks
                              (default 32); < 0 disables graphs (plain launches)               */
     int    recon12_f64;   /* 1: the fp64 correction steps use 12-real links too               */
+    int    recon8;        /* 1: the iteration's Dslash uses 8-parameter links (overrides recon12) */
 } stag_cg_params_t;
 
 typedef struct stag_cg_stats {

@@ -34,13 +34,14 @@ _CSRC = os.path.join(_HERE, "csrc")
 _LIB = os.path.join(_HERE, "libstag.so")
 _HEADER = os.path.join(os.path.dirname(_HERE), "include", "stag.h")
 
-PREC_F64, PREC_F32, PREC_F64_R12, PREC_F32_R12 = 0, 1, 2, 3
+PREC_F64, PREC_F32, PREC_F64_R12, PREC_F32_R12, PREC_F64_R8, PREC_F32_R8 = 0, 1, 2, 3, 4, 5
 CG_F64, CG_F32, CG_DEFECT, CG_RELIABLE = 0, 1, 2, 3
 OK, EINVAL, ECUDA, ENOMEM, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, 1, 2
 
 MAX_RHS = 12
 
-PREC_NAMES = {PREC_F64: "fp64/18", PREC_F32: "fp32/18", PREC_F64_R12: "fp64/12", PREC_F32_R12: "fp32/12"}
+PREC_NAMES = {PREC_F64: "fp64/18", PREC_F32: "fp32/18", PREC_F64_R12: "fp64/12", PREC_F32_R12: "fp32/12",
+              PREC_F64_R8: "fp64/8", PREC_F32_R8: "fp32/8"}
 
 
 class StagError(RuntimeError):
@@ -74,7 +75,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 class _Params(ctypes.Structure):
     _fields_ = [("eps_in", ctypes.c_double), ("recon12", ctypes.c_int),
-                ("graph_chunk", ctypes.c_int), ("recon12_f64", ctypes.c_int)]
+                ("graph_chunk", ctypes.c_int), ("recon12_f64", ctypes.c_int), ("recon8", ctypes.c_int)]
 
 
 class _Stats(ctypes.Structure):
@@ -97,6 +98,7 @@ SIGNATURES = {
     "stag_links_create_unfolded": (ctypes.c_int, [ctypes.POINTER(_vp), _ip, ctypes.c_int, _vp, ctypes.c_int]),
     "stag_links_destroy": (None, [_vp]),
     "stag_links_recon_error": (ctypes.c_int, [_vp, _dp]),
+    "stag_links_recon8_error": (ctypes.c_int, [_vp, ctypes.c_int, _dp]),
     "stag_spinor_bytes": (ctypes.c_size_t, [_ip, ctypes.c_int]),
     "stag_spinor_pack": (ctypes.c_int, [_vp, _vp, _ip, ctypes.c_int]),
     "stag_spinor_unpack": (ctypes.c_int, [_vp, _vp, _ip, ctypes.c_int]),
@@ -196,7 +198,7 @@ def spinor_bytes(dims, prec) -> int:
 
 
 def _is_f32(prec):
-    return prec in (PREC_F32, PREC_F32_R12)
+    return prec in (PREC_F32, PREC_F32_R12, PREC_F32_R8)
 
 
 def empty_spinor(dims, prec):
@@ -244,6 +246,12 @@ class Links:
     @property
     def handle(self):
         return self._h
+
+    def recon8_error(self, prec) -> float:
+        """Largest rebuilt-entry error of the 8-parameter form (builds it); raises if refused."""
+        e = ctypes.c_double()
+        _check(lib().stag_links_recon8_error(self._h, int(prec), ctypes.byref(e)))
+        return e.value
 
     def recon_error(self) -> float:
         e = ctypes.c_double()
@@ -312,8 +320,9 @@ def apply_A(v_even, links: Links, mass: float, prec, out=None):
     return out
 
 
-def _params(eps_in, recon12, graph_chunk, recon12_f64):
+def _params(eps_in, recon12, graph_chunk, recon12_f64, recon8=False):
     p = _Params()
+    p.recon8 = int(bool(recon8))
     p.eps_in = float(eps_in or 0.0)
     p.recon12 = int(bool(recon12))
     p.graph_chunk = int(graph_chunk or 0)
@@ -328,14 +337,14 @@ def _stats_dict(st: _Stats, status: int):
 
 
 def cg_solve(b, links: Links, mass: float, tol: float, maxiter: int, mode: int = CG_RELIABLE,
-             x0=None, eps_in=None, recon12=False, graph_chunk=None, recon12_f64=False):
+             x0=None, eps_in=None, recon12=False, graph_chunk=None, recon12_f64=False, recon8=False):
     """Solve A x = b on the even sites.  b, x0: fp64 device spinors.  Returns (x, stats dict);
     stats["status"] is 0, ENOCONV or EBREAKDOWN.  Errors (< 0) raise StagError."""
     torch = _require_cuda()
     use_current_stream()
     x = torch.zeros_like(b) if x0 is None else x0.clone()
     st = _Stats()
-    p = _params(eps_in, recon12, graph_chunk, recon12_f64)
+    p = _params(eps_in, recon12, graph_chunk, recon12_f64, recon8)
     rc = lib().stag_cg_solve_ex(ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(b.data_ptr()),
                                 links.handle, float(mass), float(tol), int(maxiter), int(mode),
                                 ctypes.byref(p), ctypes.byref(st))

@@ -58,12 +58,71 @@ __device__ __forceinline__ void rebuild_row2(cplx_t<T> *m, bool neg)
     }
 }
 
+// The 8-parameter form (P:L113 names it and rejects it for its round-off; Ref. [6] of the paper
+// defines it).  A matrix M = s*U, U in SU(3) with rows a, b, c, s = det M = +-1, is stored as four
+// complex slots  a2, a3, b1, (theta1, theta2)  with theta1 = arg a1, theta2 = arg c1, and rebuilt:
+//   |a1|^2 = 1 - |a2|^2 - |a3|^2            (row a has unit norm)
+//   |c1|^2 = 1 - |a1|^2 - |b1|^2            (column 1 has unit norm)
+//   N = |a2|^2 + |a3|^2
+//   b2 = -(a3* c1* + a1* a2 b1)/N    b3 =  (a2* c1* - a1* a3 b1)/N
+//   c2 =  (a3* b1* - a1* a2 c1)/N    c3 = -(a2* b1* + a1* a3 c1)/N
+// (unitarity and det U = 1 solved for the four unknowns).  1/N amplifies rounding when the first
+// row is nearly (a1,0,0): that is the round-off the paper means, and N = 0 (unit links) has no
+// 8-parameter form at all; stag_links_create measures the rebuilt error and refuses such fields.
+// On entry m[0..3] hold the four slots; on exit m[0..8] the matrix M.
+// fp32: the hardware sine / cosine (arguments are in [-pi, pi], absolute error ~5e-7, the size
+// of an fp32 rounding of the stored phase itself) and reciprocal; the library sincosf with its
+// range reduction made the fp32 hop ALU-bound (94.8 us against 70.0 us for 12-real on 28^3 x 96).
+__device__ __forceinline__ void sincos_fast(float x, float *s, float *c) { __sincosf(x, s, c); }
+__device__ __forceinline__ void sincos_fast(double x, double *s, double *c) { sincos(x, s, c); }
+__device__ __forceinline__ float recip_fast(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ double recip_fast(double x) { return 1.0 / x; }
+
+template <typename T>
+__device__ __forceinline__ void rebuild_from8(cplx_t<T> *m, bool neg)
+{
+    using C = cplx_t<T>;
+    const C a2 = m[0], a3 = m[1], b1 = m[2];
+    T s1, c1r, s2, c2r;
+    sincos_fast(m[3].x, &s1, &c1r);
+    sincos_fast(m[3].y, &s2, &c2r);
+    const T n = a2.x * a2.x + a2.y * a2.y + a3.x * a3.x + a3.y * a3.y;
+    const T r1 = sqrt(fmax((T)0, (T)1 - n));
+    const C a1 = mk<T>(r1 * c1r, r1 * s1);
+    const T r2 = sqrt(fmax((T)0, (T)1 - r1 * r1 - (b1.x * b1.x + b1.y * b1.y)));
+    const C c1 = mk<T>(r2 * c2r, r2 * s2);
+    const T inv = recip_fast(n);
+    const C a1c = mk<T>(a1.x, -a1.y), a2c = mk<T>(a2.x, -a2.y), a3c = mk<T>(a3.x, -a3.y);
+    const C b1c = mk<T>(b1.x, -b1.y), c1c = mk<T>(c1.x, -c1.y);
+    const C a1c_a2 = cmul(a1c, a2), a1c_a3 = cmul(a1c, a3);
+    const C t1 = cmul(a3c, c1c), t2 = cmul(a1c_a2, b1);      // b2 = -(t1 + t2)/N
+    const C t3 = cmul(a2c, c1c), t4 = cmul(a1c_a3, b1);      // b3 =  (t3 - t4)/N
+    const C t5 = cmul(a3c, b1c), t6 = cmul(a1c_a2, c1);      // c2 =  (t5 - t6)/N
+    const C t7 = cmul(a2c, b1c), t8 = cmul(a1c_a3, c1);      // c3 = -(t7 + t8)/N
+    const T sg = neg ? (T)-1 : (T)1, si = sg * inv;
+    m[0] = mk<T>(sg * a1.x, sg * a1.y);
+    m[1] = mk<T>(sg * a2.x, sg * a2.y);
+    m[2] = mk<T>(sg * a3.x, sg * a3.y);
+    m[3] = mk<T>(sg * b1.x, sg * b1.y);
+    m[4] = mk<T>(-si * (t1.x + t2.x), -si * (t1.y + t2.y));
+    m[5] = mk<T>(si * (t3.x - t4.x), si * (t3.y - t4.y));
+    m[6] = mk<T>(sg * c1.x, sg * c1.y);
+    m[7] = mk<T>(si * (t5.x - t6.x), si * (t5.y - t6.y));
+    m[8] = mk<T>(-si * (t7.x + t8.x), -si * (t7.y + t8.y));
+}
+
+// complex numbers stored per link for NR: 3 = all nine, 2 = rows 0,1, 1 = the 8-parameter form
+__host__ __device__ constexpr int link_slots(int NR) { return NR == 1 ? 4 : 3 * NR; }
+
 // Launch shape per precision / storage / right-hand sides, from the sweeps on 28^3 x 96
 // (profiles/README.md): MINB = resident blocks per SM promised to ptxas, GM = directions' worth
 // of packets loaded ahead (group = K*GM packets).  With N > 1 right-hand sides the registers go
 // to the N accumulators and the N neighbour vectors of one group instead.
 template <typename T, int NR, int N> struct HopTune { static constexpr int MINB = 4, GM = 1; };
 template <> struct HopTune<float, 2, 1>            { static constexpr int MINB = 6, GM = 2; };
+// 8-parameter fp32: ALU-bound (two sincos, two sqrt, a reciprocal and eight complex products per
+// link); 4 blocks/SM with two directions in flight measured best (70.2 us; 6 blocks: 76.8 us)
+template <> struct HopTune<float, 1, 1>            { static constexpr int MINB = 4, GM = 2; };
 template <int N> struct HopTune<double, 3, N>      { static constexpr int MINB = (N == 1) ? 4 : 2, GM = 1; };
 template <int N> struct HopTune<double, 2, N>      { static constexpr int MINB = (N == 1) ? 4 : 2, GM = 1; };
 
@@ -91,7 +150,7 @@ __device__ __forceinline__ void wait_flag(const unsigned long long *f, unsigned 
     } while (v < epoch);
 }
 
-// T: float or double.  NR: rows of each link held in memory (3 = 18-real, 2 = 12-real).
+// T: float or double.  NR: storage of each link (3 = 18-real, 2 = 12-real rows 0,1, 1 = 8-parameter).
 // N: right-hand sides handled by one thread; spinor k of a batch starts rs complex numbers after
 // spinor k-1 (rs = 3*Vh_pad: the batch is N device spinors back to back).
 // links: the gathered field of the OUTPUT parity as packets, L[tile][j][lane], packet j holding
@@ -115,7 +174,7 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
     static_assert(!HALO || N == 1, "slab hops carry one right-hand side");
     using C = cplx_t<T>;
     using P = pkt_t<T>;
-    constexpr int K = 3 * NR;
+    constexpr int K = link_slots(NR);
     constexpr int GM = HopTune<T, NR, N>::GM;
     constexpr int DPG = Pkt<T>::CPP * GM;     // directions per group
     constexpr int NG = 8 / DPG;               // groups per site
@@ -141,7 +200,7 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
         const P *L = links + (size_t)(cb >> 5) * (size_t)(NG * KG * TILE) + (cb & 31);
 
         unsigned neg = 0;
-        if (NR == 2) neg = det_sign_mask(g, s);
+        if (NR != 3) neg = det_sign_mask(g, s);
 
         // one right-hand side: all 24 neighbour loads are issued before the link stream;
         // several: the neighbours of one group of directions at a time (register budget)
@@ -197,6 +256,7 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
 #pragma unroll
                 for (int k = 0; k < K; ++k) m[k] = pk_get(pk, dd * K + k);
                 if (NR == 2) rebuild_row2<T>(m, (neg >> d) & 1u);
+                if (NR == 1) rebuild_from8<T>(m, (neg >> d) & 1u);
 #pragma unroll
                 for (int k = 0; k < N; ++k)
 #pragma unroll

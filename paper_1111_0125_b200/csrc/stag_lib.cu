@@ -50,9 +50,15 @@ int cuda_fail(cudaError_t e, const char *what, int line)
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-inline bool prec_ok(int prec) { return prec >= 0 && prec <= 3; }
-inline bool prec_is_f32(int prec) { return prec == STAG_PREC_F32 || prec == STAG_PREC_F32_R12; }
-inline int prec_rows(int prec) { return (prec == STAG_PREC_F64_R12 || prec == STAG_PREC_F32_R12) ? 2 : 3; }
+constexpr int N_PREC = 6;
+inline bool prec_ok(int prec) { return prec >= 0 && prec < N_PREC; }
+inline bool prec_is_f32(int prec) { return prec == STAG_PREC_F32 || prec == STAG_PREC_F32_R12 || prec == STAG_PREC_F32_R8; }
+// storage of a link: 3 = 18-real, 2 = 12-real (rows 0,1), 1 = 8-parameter
+inline int prec_rows(int prec)
+{
+    if (prec == STAG_PREC_F64_R8 || prec == STAG_PREC_F32_R8) return 1;
+    return (prec == STAG_PREC_F64_R12 || prec == STAG_PREC_F32_R12) ? 2 : 3;
+}
 
 // Grid of the streaming vector kernels: 4 resident blocks of 256 threads per SM (a multiple of
 // the SM count) shared among the nrhs right-hand sides (grid.y = nrhs), fewer when the vector
@@ -89,7 +95,8 @@ struct stag_links {
     int rank, nranks;      // T-slab: time slices [rank*X3, (rank+1)*X3) of nranks*X3; else 0, 1
     int is_slab;           // made by stag_slab_create: operator calls go through stag_slab_*
     int ntiles;            // Vh_pad / TILE
-    void *L[4];            // gathered link fields by precision enum; L[STAG_PREC_F64] always set
+    void *L[6];            // gathered link fields by precision enum; L[STAG_PREC_F64] always set
+    double recon8_err[2];  // 8-parameter forms: largest rebuilt-entry error, [0] fp64, [1] fp32 (-1: not built)
     double recon_err;
     void *tmp_odd[2];      // scratch odd-parity spinors for stag_apply_A: [0] fp64, [1] fp32
     int tmp_odd_rhs[2];    // how many right-hand sides each holds
@@ -118,7 +125,7 @@ namespace {
 
 size_t links_elems(const stag_links *L, int rows)   // complex numbers in one gathered field
 {
-    return (size_t)2 * L->ntiles * 8 * (3 * rows) * TILE;
+    return (size_t)2 * L->ntiles * 8 * link_slots(rows) * TILE;
 }
 
 // ---- S0 kernels ----------------------------------------------------------------------
@@ -172,10 +179,12 @@ gather_links_kernel(double2 *__restrict__ L, const double *__restrict__ W, const
         double2 t[9];
         for (int k = 0; k < 6; ++k) t[k] = m[k];
         rebuild_row2<double>(t, (neg >> d) & 1u);
-        for (int j = 0; j < 3; ++j)
-            worst = fmax(worst, fmax(fabs(t[6 + j].x - m[6 + j].x), fabs(t[6 + j].y - m[6 + j].y)));
+        for (int j = 0; j < 3; ++j) {
+            const double ex = fabs(t[6 + j].x - m[6 + j].x), ey = fabs(t[6 + j].y - m[6 + j].y);
+            if (!(ex == ex) || !(ey == ey)) worst = 1e300;   // fmax would drop a NaN
+            else worst = fmax(worst, fmax(ex, ey));
+        }
     }
-    if (!(worst == worst)) worst = 1e300;
     atomicMax(err_bits, (unsigned long long)__double_as_longlong(worst));   // worst >= 0
 }
 
@@ -204,6 +213,55 @@ derive_links_kernel(pkt_t<TD> *__restrict__ dst, const double2 *__restrict__ src
         v[2 * h + 1] = (TD)w.y;
     }
     dst[i] = pack(v);
+}
+
+// fp64/18 gathered field -> the 8-parameter form in precision TD (stag_dslash.cuh, rebuild_from8):
+// one thread per (parity, site, direction) stores the four slots a2, a3, b1, (arg a1, arg c1) of
+// U = s*M (s = det M from the site's coordinates), then rebuilds M from what it stored, in TD
+// arithmetic, exactly as the hop will, and records the largest entry error against the fp64 M.
+template <typename TD>
+__global__ void __launch_bounds__(128)
+derive_links8_kernel(pkt_t<TD> *__restrict__ dst, const double2 *__restrict__ src, const Geom g,
+                     unsigned long long *__restrict__ err_bits)
+{
+    constexpr int CPP = Pkt<TD>::CPP;
+    constexpr int PPS = 8 * 4 / CPP;             // packets per site
+    const long idx = blockIdx.x * 128L + threadIdx.x;
+    if (idx >= 2L * g.Vh_pad * 8) return;
+    const int d = (int)(idx & 7);
+    const long site = idx >> 3;                  // p * Vh_pad + cb
+    const int p = (int)(site / g.Vh_pad);
+    const int cb = (int)(site % g.Vh_pad);
+    const long tile = site >> 5;
+    const int lane = cb & 31;
+    double2 M[9];
+    for (int k = 0; k < 9; ++k) M[k] = src[((tile * 8 + d) * 9 + k) * TILE + lane];
+    bool neg = false;
+    if (cb < g.Vh) {
+        Site s;
+        decode_site(g, p, cb, s);
+        neg = (det_sign_mask(g, s) >> d) & 1u;
+    }
+    const double sg = neg ? -1.0 : 1.0;
+    cplx_t<TD> slot[9];
+    slot[0] = mk<TD>((TD)(sg * M[1].x), (TD)(sg * M[1].y));      // a2
+    slot[1] = mk<TD>((TD)(sg * M[2].x), (TD)(sg * M[2].y));      // a3
+    slot[2] = mk<TD>((TD)(sg * M[3].x), (TD)(sg * M[3].y));      // b1
+    slot[3] = mk<TD>((TD)atan2(sg * M[0].y, sg * M[0].x), (TD)atan2(sg * M[6].y, sg * M[6].x));
+    TD v[2 * CPP];
+    for (int j = 0; j < 4 / CPP; ++j) {
+        for (int h = 0; h < CPP; ++h) { v[2 * h] = slot[CPP * j + h].x; v[2 * h + 1] = slot[CPP * j + h].y; }
+        dst[(tile * PPS + (d * 4 / CPP + j)) * TILE + lane] = pack(v);
+    }
+    if (cb >= g.Vh) return;                      // pad lanes hold zeros (atan2(0,0) = 0): no error to take
+    rebuild_from8<TD>(slot, neg);
+    double worst = 0.0;
+    for (int k = 0; k < 9; ++k) {
+        const double ex = fabs((double)slot[k].x - M[k].x), ey = fabs((double)slot[k].y - M[k].y);
+        if (!(ex == ex) || !(ey == ey)) worst = 1e300;       // fmax would drop a NaN (0 * 1/0 at N = 0)
+        else worst = fmax(worst, fmax(ex, ey));
+    }
+    atomicMax(err_bits, (unsigned long long)__double_as_longlong(worst));
 }
 
 template <typename T>
@@ -246,6 +304,44 @@ int ensure_links(stag_links *L, int prec)
     const size_t bytes = links_elems(L, rows) * (prec_is_f32(prec) ? sizeof(float2) : sizeof(double2));
     const size_t n = bytes / 16;                 // 16-byte packets
     void *dst = nullptr;
+    if (rows == 1) {
+        // the 8-parameter form has no representation for a first row (a1,0,0) and loses accuracy
+        // near it: build it, measure the rebuilt error in the arithmetic of the hop,
+        // and refuse the field if it is beyond what that precision can mean
+        const int f32 = prec_is_f32(prec) ? 1 : 0;
+        const double limit = f32 ? 1e-3 : 1e-9;
+        if (!(L->recon_err <= 1e-10)) {
+            snprintf(t_errbuf, sizeof(t_errbuf), "8-parameter links refused: the links are not +-SU(3) (max error %.3g)", L->recon_err);
+            t_errbuf_status = STAG_EINVAL;
+            return STAG_EINVAL;
+        }
+        unsigned long long *err = nullptr;
+        CU(cudaMalloc(&dst, bytes));
+        if (cudaMalloc(&err, sizeof(*err)) != cudaSuccess) { cudaFree(dst); return STAG_ENOMEM; }
+        cudaMemsetAsync(err, 0, sizeof(*err), t_stream);
+        const unsigned g8 = (unsigned)((2L * L->g.Vh_pad * 8 + 127) / 128);
+        const double2 *src8 = (const double2 *)L->L[STAG_PREC_F64];
+        if (f32) derive_links8_kernel<float><<<g8, 128, 0, t_stream>>>((float4 *)dst, src8, L->g, err);
+        else derive_links8_kernel<double><<<g8, 128, 0, t_stream>>>((double2 *)dst, src8, L->g, err);
+        count_launch();
+        unsigned long long bits = 0;
+        cudaError_t e8 = cudaGetLastError();
+        if (e8 == cudaSuccess) e8 = cudaMemcpyAsync(&bits, err, sizeof(bits), cudaMemcpyDeviceToHost, t_stream);
+        if (e8 == cudaSuccess) e8 = cudaStreamSynchronize(t_stream);
+        cudaFree(err);
+        if (e8 != cudaSuccess) { cudaFree(dst); return cuda_fail(e8, "derive_links8_kernel", __LINE__); }
+        memcpy(&L->recon8_err[f32], &bits, sizeof(double));
+        if (!(L->recon8_err[f32] <= limit)) {
+            cudaFree(dst);
+            snprintf(t_errbuf, sizeof(t_errbuf),
+                     "8-parameter links refused: rebuilt entries are off by up to %.3g (limit %.1g); a link with a first row near (a1,0,0) has no usable 8-parameter form",
+                     L->recon8_err[f32], limit);
+            t_errbuf_status = STAG_EINVAL;
+            return STAG_EINVAL;
+        }
+        L->L[prec] = dst;
+        return STAG_OK;
+    }
     CU(cudaMalloc(&dst, bytes));
     const unsigned grid = (unsigned)((n + 255) / 256);
     const double2 *src = (const double2 *)L->L[STAG_PREC_F64];
@@ -279,7 +375,7 @@ int launch_hop_n(const stag_links *L, int prec, int hop, cplx_t<T> *out, const c
 {
     const Geom &g = L->g;
     const pkt_t<T> *field = (const pkt_t<T> *)L->L[prec] +
-                            (size_t)parity * L->ntiles * (8 * (3 * NR) / Pkt<T>::CPP) * TILE;
+                            (size_t)parity * L->ntiles * (8 * link_slots(NR) / Pkt<T>::CPP) * TILE;
     const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
     switch (hop) {
     case HOP_PLAIN:
@@ -343,6 +439,10 @@ int launch_hop(const stag_links *L, int prec, int hop, void *out, const void *in
         return launch_hop_t<double, 2>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, cD, (const double2 *)own, partials, ctrl, nrhs, s);
     case STAG_PREC_F32_R12:
         return launch_hop_t<float, 2>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, cD, (const float2 *)own, partials, ctrl, nrhs, s);
+    case STAG_PREC_F64_R8:
+        return launch_hop_t<double, 1>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, cD, (const double2 *)own, partials, ctrl, nrhs, s);
+    case STAG_PREC_F32_R8:
+        return launch_hop_t<float, 1>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, cD, (const float2 *)own, partials, ctrl, nrhs, s);
     }
     return STAG_EINVAL;
 }
@@ -457,7 +557,7 @@ static void stag_slab_cg_free(struct stag_slab_cg *c);
 extern "C" void stag_links_destroy(stag_links_t *L)
 {
     if (!L) return;
-    for (int i = 0; i < 4; ++i) if (L->L[i]) cudaFree(L->L[i]);
+    for (int i = 0; i < N_PREC; ++i) if (L->L[i]) cudaFree(L->L[i]);
     for (int i = 0; i < 2; ++i) if (L->tmp_odd[i]) cudaFree(L->tmp_odd[i]);
     if (L->ws) cudaFree(L->ws);
     if (L->h_ctrl) cudaFreeHost(L->h_ctrl);
@@ -470,6 +570,15 @@ extern "C" void stag_links_destroy(stag_links_t *L)
     if (L->ev0) cudaEventDestroy(L->ev0);
     if (L->ev1) cudaEventDestroy(L->ev1);
     delete L;
+}
+
+extern "C" int stag_links_recon8_error(const stag_links_t *links, int prec, double *err_out)
+{
+    stag_links *L = const_cast<stag_links *>(links);
+    if (!L || !err_out || (prec != STAG_PREC_F64_R8 && prec != STAG_PREC_F32_R8)) return STAG_EINVAL;
+    const int rc = ensure_links(L, prec);        // builds (or refuses) and measures
+    *err_out = L->recon8_err[prec_is_f32(prec) ? 1 : 0];
+    return rc;
 }
 
 extern "C" int stag_links_recon_error(const stag_links_t *L, double *err_out)
@@ -694,8 +803,8 @@ int cg_solve_device(double *x, const double *b, stag_links *L, double mass, doub
     S.m2 = mass * mass;
     S.mode = mode;
     S.nrhs = nrhs;
-    S.prec_lo = (mode == STAG_CG_F64) ? (P.recon12 ? STAG_PREC_F64_R12 : STAG_PREC_F64)
-                                       : (P.recon12 ? STAG_PREC_F32_R12 : STAG_PREC_F32);
+    S.prec_lo = (mode == STAG_CG_F64) ? (P.recon8 ? STAG_PREC_F64_R8 : P.recon12 ? STAG_PREC_F64_R12 : STAG_PREC_F64)
+                                       : (P.recon8 ? STAG_PREC_F32_R8 : P.recon12 ? STAG_PREC_F32_R12 : STAG_PREC_F32);
     S.prec_hi = P.recon12_f64 ? STAG_PREC_F64_R12 : STAG_PREC_F64;
     S.n = (long)6 * L->g.Vh_pad;
     S.gb = blas_grid(S.n, nrhs);
@@ -1046,7 +1155,7 @@ int slab_hop_t(stag_links *L, int prec, cplx_t<T> *out, const cplx_t<T> *in, int
 {
     const Geom &g = L->g;
     const pkt_t<T> *field = (const pkt_t<T> *)L->L[prec] +
-                            (size_t)parity * L->ntiles * (8 * (3 * NR) / Pkt<T>::CPP) * TILE;
+                            (size_t)parity * L->ntiles * (8 * link_slots(NR) / Pkt<T>::CPP) * TILE;
     const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
     XchHeader *mine = (XchHeader *)L->xch;
     HaloArgs<T> h;
@@ -1086,6 +1195,7 @@ extern "C" int stag_slab_hop(void *out, const void *in, stag_links_t *L, int par
     case STAG_PREC_F32:     return slab_hop_t<float, 3>(L, prec, (float2 *)out, (const float2 *)in, parity, a, (const float2 *)own, t_stream);
     case STAG_PREC_F64_R12: return slab_hop_t<double, 2>(L, prec, (double2 *)out, (const double2 *)in, parity, a, (const double2 *)own, t_stream);
     case STAG_PREC_F32_R12: return slab_hop_t<float, 2>(L, prec, (float2 *)out, (const float2 *)in, parity, a, (const float2 *)own, t_stream);
+    default: break;       // the 8-parameter forms are whole-lattice only
     }
     return STAG_EINVAL;
 }
@@ -1152,7 +1262,7 @@ int slab_hop_mode_t(stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx
 {
     const Geom &g = L->g;
     const pkt_t<T> *field = (const pkt_t<T> *)L->L[prec] +
-                            (size_t)parity * L->ntiles * (8 * (3 * NR) / Pkt<T>::CPP) * TILE;
+                            (size_t)parity * L->ntiles * (8 * link_slots(NR) / Pkt<T>::CPP) * TILE;
     const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
     XchHeader *mine = (XchHeader *)L->xch;
     HaloArgs<T> h;
@@ -1185,6 +1295,7 @@ int slab_hop_mode(stag_links *L, int prec, int hop, void *out, const void *in, i
     case STAG_PREC_F32:     return slab_hop_mode_t<float, 3>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, (const float2 *)own, partials, ctrl, s);
     case STAG_PREC_F64_R12: return slab_hop_mode_t<double, 2>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, (const double2 *)own, partials, ctrl, s);
     case STAG_PREC_F32_R12: return slab_hop_mode_t<float, 2>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, (const float2 *)own, partials, ctrl, s);
+    default: break;
     }
     return STAG_EINVAL;
 }

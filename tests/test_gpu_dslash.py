@@ -183,3 +183,54 @@ def test_device_side_phase_folding_is_bit_identical_to_the_generator(dims, antip
             assert torch.equal(stag.dslash(v, La, parity, prec), stag.dslash(v, Lb, parity, prec))
         out = stag.spinor_unpack(stag.dslash(stag.spinor_pack(chi, dims, 0), Lb, parity, 0), dims, 0)
         assert rel_l2(out, oracle.dslash(chi, W, dims, parity)) <= 1e-13
+
+
+# ---- the 8-parameter link form ---------------------------------
+# Tolerances: fp64 keeps 1e-11 (the rebuild divides by N = |a2|^2+|a3|^2, which amplifies the
+# 1e-16 rounding of the stored slots by 1/N; measured <= 8e-14 down to eps = 0.05 smooth links);
+# fp32 gets 5e-6, NOT the 2e-6 of the other fp32 forms: measured 4.7e-7 (random SU(3)) to 1.9e-6
+# (smooth eps = 0.3), single rebuilt entries off by up to 4e-4 -- the round-off the paper rejects
+# the form for.
+TOL8 = {stag.PREC_F64_R8: 1e-11, stag.PREC_F32_R8: 5e-6}
+
+
+@pytest.mark.parametrize("kind,eps", [("random", 0.0), ("smooth", 0.5), ("smooth", 0.3)])
+@pytest.mark.parametrize("prec", [stag.PREC_F64_R8, stag.PREC_F32_R8])
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (6, 4, 2, 10)])
+def test_eight_parameter_hop_matches_oracle(dims, prec, kind, eps):
+    W = fieldgen.links(dims, kind, seed=5, eps=eps)
+    L = stag.Links(dims, W)
+    for parity in (0, 1):
+        chi = fieldgen.spinor_gaussian(dims, 1 - parity, seed=6 + parity)
+        out = stag.spinor_unpack(stag.dslash(stag.spinor_pack(chi, dims, prec), L, parity, prec), dims, prec)
+        assert rel_l2(out, oracle.dslash(chi, W, dims, parity)) <= TOL8[prec]
+    assert L.recon8_error(prec) <= (1e-9 if prec == stag.PREC_F64_R8 else 1e-3)
+
+
+def test_eight_parameter_periodic_boundary_and_apply_A():
+    dims = (4, 4, 2, 6)
+    W = fieldgen.links(dims, "random", seed=5, antiperiodic_t=False)
+    L = stag.Links(dims, W, antiperiodic_t=False)
+    chi = fieldgen.spinor_gaussian(dims, 0, seed=6)
+    for prec in (stag.PREC_F64_R8, stag.PREC_F32_R8):
+        out = stag.spinor_unpack(stag.apply_A(stag.spinor_pack(chi, dims, prec), L, 0.1, prec), dims, prec)
+        assert rel_l2(out, oracle.apply_A(chi, W, dims, 0.1)) <= TOL8[prec]
+
+
+def test_eight_parameter_form_refused_where_it_does_not_exist():
+    """Unit links have first row (1,0,0): N = 0, no 8-parameter form; nearly-unit links lose all
+    fp32 accuracy.  Both must be refused with STAG_EINVAL, never silently wrong."""
+    dims = (4, 4, 4, 4)
+    chi = fieldgen.spinor_gaussian(dims, 0, seed=2)
+    L = stag.Links(dims, fieldgen.links(dims, "unit"))
+    for prec in (stag.PREC_F64_R8, stag.PREC_F32_R8):
+        with pytest.raises(stag.StagError) as e:
+            stag.dslash(stag.spinor_pack(chi, dims, prec), L, 1, prec)
+        assert e.value.status == stag.EINVAL
+    L2 = stag.Links(dims, fieldgen.links(dims, "smooth", seed=3, eps=0.003))
+    with pytest.raises(stag.StagError):
+        stag.dslash(stag.spinor_pack(chi, dims, stag.PREC_F32_R8), L2, 1, stag.PREC_F32_R8)
+    rng = np.random.default_rng(0)
+    L3 = stag.Links(dims, rng.normal(size=(4, 2, 128, 3, 3)) + 1j * rng.normal(size=(4, 2, 128, 3, 3)))
+    with pytest.raises(stag.StagError):
+        stag.dslash(stag.spinor_pack(chi, dims, stag.PREC_F64_R8), L3, 1, stag.PREC_F64_R8)
