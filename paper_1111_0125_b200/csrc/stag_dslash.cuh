@@ -269,6 +269,14 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
             }
         }
 
+        if (NR == 1 && cb >= g.Vh) {
+            // a rebuilt 8-parameter matrix is unitary, never zero: pad lanes are zeroed here
+            // (the 18- and 12-real forms get their zeros from the zero links of the pad lanes)
+#pragma unroll
+            for (int k = 0; k < N; ++k)
+#pragma unroll
+                for (int i = 0; i < 3; ++i) acc[k][i] = mk<T>(0, 0);
+        }
 #pragma unroll
         for (int k = 0; k < N; ++k) {
             if (MODE == HOP_PLAIN) {

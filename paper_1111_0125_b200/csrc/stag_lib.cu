@@ -248,12 +248,16 @@ derive_links8_kernel(pkt_t<TD> *__restrict__ dst, const double2 *__restrict__ sr
     slot[1] = mk<TD>((TD)(sg * M[2].x), (TD)(sg * M[2].y));      // a3
     slot[2] = mk<TD>((TD)(sg * M[3].x), (TD)(sg * M[3].y));      // b1
     slot[3] = mk<TD>((TD)atan2(sg * M[0].y, sg * M[0].x), (TD)atan2(sg * M[6].y, sg * M[6].x));
+    if (cb >= g.Vh) {      // pad lanes: slots whose rebuild is finite (N = 1); the hop zeroes their output
+        slot[0] = mk<TD>((TD)1, (TD)0);
+        slot[1] = slot[2] = slot[3] = mk<TD>((TD)0, (TD)0);
+    }
     TD v[2 * CPP];
     for (int j = 0; j < 4 / CPP; ++j) {
         for (int h = 0; h < CPP; ++h) { v[2 * h] = slot[CPP * j + h].x; v[2 * h + 1] = slot[CPP * j + h].y; }
         dst[(tile * PPS + (d * 4 / CPP + j)) * TILE + lane] = pack(v);
     }
-    if (cb >= g.Vh) return;                      // pad lanes hold zeros (atan2(0,0) = 0): no error to take
+    if (cb >= g.Vh) return;                      // pad lanes: no error to take
     rebuild_from8<TD>(slot, neg);
     double worst = 0.0;
     for (int k = 0; k < 9; ++k) {
