@@ -310,7 +310,9 @@ int stag_cg_solve_host(double *x_host, const double *b_host, const stag_links_t 
  * the same phase, so slabs that share one device can instead be stepped rank after rank, phase
  * by phase (how the single-GPU tests run the multi-GPU data path).  x, b: fp64 device spinors of
  * the slab's local dims; x holds the initial guess.  Modes: STAG_CG_F64, STAG_CG_RELIABLE.
- * graph_chunk of the params = iterations per ACT_ITER (default 32; plain launches). */
+ * graph_chunk of the params = iterations per ACT_ITER (default 32): plain launches when stepped,
+ * one CUDA-graph launch per ACT_ITER inside stag_slab_cg_run (the exchange and reduction numbers
+ * live in device memory, so the captured chunk can be replayed). */
 enum {
     STAG_SLAB_ACT_DONE = 0, STAG_SLAB_ACT_NORM = 1, STAG_SLAB_ACT_INIT = 2, STAG_SLAB_ACT_ITER = 3,
     STAG_SLAB_ACT_UPDATE = 4, STAG_SLAB_ACT_VERIFY = 5, STAG_SLAB_ACT_FINAL = 6

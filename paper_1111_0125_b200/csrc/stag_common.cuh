@@ -170,6 +170,24 @@ struct CgCtrl {
 constexpr int CTRL_SLOT = 2048;   // bytes reserved for CgCtrl in the workspace
 static_assert(sizeof(CgCtrl) <= CTRL_SLOT, "CgCtrl must fit its workspace slot");
 
+// ---- T-slab exchange region header (stag_slab.cuh describes the protocol) ----------------------
+constexpr size_t XCH_HDR = 1024;    // bytes of header in front of the halo buffers
+constexpr size_t XCH_RED = 256;     // offset of the reduction slots inside the header area
+struct XchHeader {
+    unsigned long long flag_back;   // PEER-written: number of the last exchange pushed into my "back" halo
+    unsigned long long flag_fwd;    // PEER-written: ... into my "fwd" halo
+    // local only (never peer-written).  Kept in device memory, not in kernel arguments, so that a
+    // captured CUDA graph of iterations can be replayed: every kernel reads the current number.
+    unsigned long long epoch;       // exchanges I have started (face_push_kernel increments it)
+    unsigned long long red_seq;     // global sums I have published
+    unsigned ticket;                // last-block ticket of my face_push_kernel
+};
+static_assert(sizeof(XchHeader) <= XCH_RED, "exchange header must fit its slot");
+__host__ __device__ inline size_t xch_halo_offset(int s3, unsigned long long epoch, int dir)
+{
+    return XCH_HDR + ((size_t)((epoch & 1ull) * 2 + dir) * 3 * s3) * 16;
+}
+
 enum { CG_RUN = 0, CG_CONVERGED = 1, CG_UPDATE = 2, CG_MAXITER = 3, CG_BREAKDOWN = 4 };
 
 }  // namespace stag

@@ -136,10 +136,10 @@ template <> struct HopMaxRhs<double> { static constexpr int value = 2; };
 // x3 = -1 and x3 = X3 of the INPUT spinor live in two halo buffers, [colour][s3] complex each,
 // that the neighbouring GPUs fill with peer-to-peer stores (face_push_kernel) and then mark by
 // storing the exchange's epoch into flag_back / flag_fwd with system-scope release.
+// The kernel reads the number of the current exchange from the region's header (device memory,
+// so a graph replay sees the right one) and derives the halo buffers of that parity from it.
 template <typename T> struct HaloArgs {
-    const cplx_t<T> *back, *fwd;
-    const unsigned long long *flag_back, *flag_fwd;
-    unsigned long long epoch;
+    const char *xch;     // this slab's exchange region
 };
 
 __device__ __forceinline__ void wait_flag(const unsigned long long *f, unsigned long long epoch)
@@ -214,16 +214,21 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
             if constexpr (HALO) {
                 // decode_site wrapped the +-t neighbours of the boundary slices onto the slab's
                 // own other end; their in-slice index is what addresses the halo buffers
+                const XchHeader *hdr = (const XchHeader *)halo.xch;
                 if (s.x3 == g.X3 - 1) {
-                    wait_flag(halo.flag_fwd, halo.epoch);
+                    const unsigned long long e = __ldcg(&hdr->epoch);
+                    const C *fwd = (const C *)(halo.xch + xch_halo_offset(g.s3, e, 1));
+                    wait_flag(&hdr->flag_fwd, e);
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) v1[3][c] = __ldcg(halo.fwd + (size_t)c * g.s3 + s.nbr[3]);
+                    for (int c = 0; c < 3; ++c) v1[3][c] = __ldcg(fwd + (size_t)c * g.s3 + s.nbr[3]);
                 }
                 if (s.x3 == 0) {
-                    wait_flag(halo.flag_back, halo.epoch);
+                    const unsigned long long e = __ldcg(&hdr->epoch);
+                    const C *back = (const C *)(halo.xch + xch_halo_offset(g.s3, e, 0));
+                    wait_flag(&hdr->flag_back, e);
 #pragma unroll
                     for (int c = 0; c < 3; ++c)
-                        v1[7][c] = __ldcg(halo.back + (size_t)c * g.s3 + (s.nbr[7] - (g.X3 - 1) * g.s3));
+                        v1[7][c] = __ldcg(back + (size_t)c * g.s3 + (s.nbr[7] - (g.X3 - 1) * g.s3));
                 }
             }
         }

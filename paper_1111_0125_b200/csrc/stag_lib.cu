@@ -1141,13 +1141,9 @@ template <typename T>
 int slab_push_t(stag_links *L, const cplx_t<T> *in, cudaStream_t s)
 {
     const Geom &g = L->g;
-    const unsigned long long e = ++L->epoch;
-    XchHeader *mine = (XchHeader *)L->xch, *pf = (XchHeader *)L->peer_fwd, *pb = (XchHeader *)L->peer_bwd;
+    ++L->epoch;            // host mirror, only for "has anything been pushed yet"; the kernels count for themselves
     const unsigned grid = (unsigned)((2L * 3 * g.s3 + 255) / 256);
-    face_push_kernel<T><<<grid, 256, 0, s>>>(in, g.Vh, g.Vh_pad, g.s3,
-                                             (cplx_t<T> *)(L->peer_fwd + xch_halo_offset(g.s3, e, 0)),
-                                             (cplx_t<T> *)(L->peer_bwd + xch_halo_offset(g.s3, e, 1)),
-                                             &pf->flag_back, &pb->flag_fwd, e, &mine->ticket);
+    face_push_kernel<T><<<grid, 256, 0, s>>>(in, g.Vh, g.Vh_pad, g.s3, L->xch, L->peer_fwd, L->peer_bwd);
     count_launch();
     KCHECK();
     return STAG_OK;
@@ -1161,13 +1157,8 @@ int slab_hop_t(stag_links *L, int prec, cplx_t<T> *out, const cplx_t<T> *in, int
     const pkt_t<T> *field = (const pkt_t<T> *)L->L[prec] +
                             (size_t)parity * L->ntiles * (8 * link_slots(NR) / Pkt<T>::CPP) * TILE;
     const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
-    XchHeader *mine = (XchHeader *)L->xch;
     HaloArgs<T> h;
-    h.back = (const cplx_t<T> *)(L->xch + xch_halo_offset(g.s3, L->epoch, 0));
-    h.fwd = (const cplx_t<T> *)(L->xch + xch_halo_offset(g.s3, L->epoch, 1));
-    h.flag_back = &mine->flag_back;
-    h.flag_fwd = &mine->flag_fwd;
-    h.epoch = L->epoch;
+    h.xch = L->xch;
     if (own)
         dslash_kernel<T, NR, HOP_XPAY, 1, true><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)1, own, nullptr, nullptr, h);
     else
@@ -1225,8 +1216,8 @@ struct stag_slab_cg {
     long n;
     int gb;
     bool lo;
-    unsigned long long red_seq;      // global sums published so far (same on every rank)
-    unsigned long long seq_dAd, seq_rr, seq_res;
+    cudaGraphExec_t iter_graph;      // stag_slab_cg_run: one ACT_ITER (graph_chunk passes) captured
+    unsigned long long iter_graph_nodes;
     int stage;                       // 0: nothing done, 1: |b|^2 on its way, 2: in the loop, 3: done
     bool have_true, verifying;
     int n_restarts, applies_f64, final_state;
@@ -1249,14 +1240,13 @@ extern "C" int stag_slab_connect_all(stag_links_t *L, void *const *regions)
 
 namespace {
 
-Comm make_comm(const stag_links *L, unsigned long long seq)
+Comm make_comm(const stag_links *L)
 {
     Comm c;
     c.peers = L->peers_dev;
     c.mine = L->xch;
     c.nranks = L->nranks;
     c.myrank = L->rank;
-    c.seq = seq;
     return c;
 }
 
@@ -1268,13 +1258,8 @@ int slab_hop_mode_t(stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx
     const pkt_t<T> *field = (const pkt_t<T> *)L->L[prec] +
                             (size_t)parity * L->ntiles * (8 * link_slots(NR) / Pkt<T>::CPP) * TILE;
     const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
-    XchHeader *mine = (XchHeader *)L->xch;
     HaloArgs<T> h;
-    h.back = (const cplx_t<T> *)(L->xch + xch_halo_offset(g.s3, L->epoch, 0));
-    h.fwd = (const cplx_t<T> *)(L->xch + xch_halo_offset(g.s3, L->epoch, 1));
-    h.flag_back = &mine->flag_back;
-    h.flag_fwd = &mine->flag_fwd;
-    h.epoch = L->epoch;
+    h.xch = L->xch;
     switch (hop) {
     case HOP_PLAIN:
         dslash_kernel<T, NR, HOP_PLAIN, 1, true><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)0, (T)1, nullptr, nullptr, ctrl, h);
@@ -1312,10 +1297,9 @@ int slab_push_prec(stag_links *L, const void *in, int prec, cudaStream_t s)
 
 // r64 = b - A64 x and its global |r|^2 in four phases (0..3); WHAT selects the scalar step.
 template <int WHAT>
-int slab_residual_phase(stag_links *L, stag_slab_cg *C, int ph, bool accumulate_first, bool lo_copy, bool *more)
+int slab_residual_phase(stag_links *L, stag_slab_cg *C, int ph, bool accumulate_first, bool lo_copy, bool *more, cudaStream_t s)
 {
     Workspace &w = C->w;
-    cudaStream_t s = t_stream;
     int rc = STAG_OK;
     *more = ph < 3;
     switch (ph) {
@@ -1332,13 +1316,12 @@ int slab_residual_phase(stag_links *L, stag_slab_cg *C, int ph, bool accumulate_
         return slab_push_prec(L, w.tmp64, C->prec_hi, s);
     case 2:
         if ((rc = slab_hop_mode(L, C->prec_hi, HOP_XPAY, w.q64, w.tmp64, 0, C->m2, C->x, nullptr, nullptr, s))) return rc;
-        C->seq_res = ++C->red_seq;
-        slab_residual_kernel<float, WHAT><<<C->gb, BLAS_BLOCK, 0, s>>>(w.r64, C->b, w.q64, lo_copy ? w.r32 : nullptr, C->n, w.partials, w.ctrl, make_comm(L, C->seq_res));
+        slab_residual_kernel<float, WHAT><<<C->gb, BLAS_BLOCK, 0, s>>>(w.r64, C->b, w.q64, lo_copy ? w.r32 : nullptr, C->n, w.partials, w.ctrl, make_comm(L));
         count_launch();
         KCHECK();
         return STAG_OK;
     case 3:
-        slab_scalar_kernel<WHAT><<<1, 32, 0, s>>>(w.ctrl, make_comm(L, C->seq_res));
+        slab_scalar_kernel<WHAT><<<1, 32, 0, s>>>(w.ctrl, make_comm(L));
         count_launch();
         KCHECK();
         return STAG_OK;
@@ -1348,10 +1331,9 @@ int slab_residual_phase(stag_links *L, stag_slab_cg *C, int ph, bool accumulate_
 
 // phase ph of iteration chunk: five phases per pass of Fig. 1's loop
 template <typename T>
-int slab_iteration_phase(stag_links *L, stag_slab_cg *C, int sub, T *y, T *r, T *d, T *q, T *tmp)
+int slab_iteration_phase(stag_links *L, stag_slab_cg *C, int sub, T *y, T *r, T *d, T *q, T *tmp, cudaStream_t s)
 {
     Workspace &w = C->w;
-    cudaStream_t s = t_stream;
     int rc;
     switch (sub) {
     case 0:   // d = r + beta d ; its faces to the neighbours
@@ -1364,19 +1346,17 @@ int slab_iteration_phase(stag_links *L, stag_slab_cg *C, int sub, T *y, T *r, T 
         return slab_push_prec(L, tmp, C->prec_lo, s);
     case 2:   // q = m^2 d - D_eo tmp, local <d,q> published
         if ((rc = slab_hop_mode(L, C->prec_lo, HOP_XPAY_DOT, q, tmp, 0, C->m2, d, w.hop_partials, w.ctrl, s))) return rc;
-        C->seq_dAd = ++C->red_seq;
-        slab_publish_partials_kernel<<<1, BLAS_BLOCK, 0, s>>>(w.hop_partials, w.n_hop, make_comm(L, C->seq_dAd), w.ctrl);
+        slab_publish_partials_kernel<<<1, BLAS_BLOCK, 0, s>>>(w.hop_partials, w.n_hop, make_comm(L), w.ctrl);
         count_launch();
         KCHECK();
         return STAG_OK;
     case 3:   // alpha from the global <d,Ad>; y, r; local |r|^2 published
-        C->seq_rr = ++C->red_seq;
-        slab_update_kernel<T><<<C->gb, BLAS_BLOCK, 0, s>>>(y, r, d, q, C->n, w.partials, w.ctrl, make_comm(L, C->seq_dAd), make_comm(L, C->seq_rr));
+        slab_update_kernel<T><<<C->gb, BLAS_BLOCK, 0, s>>>(y, r, d, q, C->n, w.partials, w.ctrl, make_comm(L));
         count_launch();
         KCHECK();
         return STAG_OK;
     case 4:   // beta, stopping tests, trigger: the same epilogue on every rank
-        slab_scalar_kernel<SCALAR_ITER><<<1, 32, 0, s>>>(w.ctrl, make_comm(L, C->seq_rr));
+        slab_scalar_kernel<SCALAR_ITER><<<1, 32, 0, s>>>(w.ctrl, make_comm(L));
         count_launch();
         KCHECK();
         return STAG_OK;
@@ -1395,12 +1375,10 @@ extern "C" int stag_slab_cg_begin(stag_links_t *L, void *x_even, const void *b_e
     if (!L->cg) {
         L->cg = new (std::nothrow) stag_slab_cg();
         if (!L->cg) return STAG_ENOMEM;
-        L->cg->red_seq = 0;
     }
     stag_slab_cg *C = L->cg;
-    const unsigned long long keep_seq = C->red_seq;      // reduction numbers never restart
+    if (C->iter_graph) cudaGraphExecDestroy(C->iter_graph);
     memset(C, 0, sizeof(*C));
-    C->red_seq = keep_seq;
     if (params) C->P = *params;
     if (!(C->P.eps_in > 0.0)) C->P.eps_in = 0.1;
     if (C->P.graph_chunk <= 0) C->P.graph_chunk = 32;    // iterations between host checks (plain launches)
@@ -1507,7 +1485,14 @@ extern "C" int stag_slab_cg_control(stag_links_t *L, int *action_out)
 // Enqueue phase `phase` of `action`.  *more_out = 1 while the action has further phases.  Within a
 // phase no kernel waits for a peer's kernel of the SAME phase, so ranks that share a device may be
 // stepped one after the other, phase by phase.
+static int slab_cg_step_on(stag_links_t *L, int action, int phase, int *more_out, cudaStream_t t_stream);
+
 extern "C" int stag_slab_cg_step(stag_links_t *L, int action, int phase, int *more_out)
+{
+    return slab_cg_step_on(L, action, phase, more_out, t_stream);
+}
+
+static int slab_cg_step_on(stag_links_t *L, int action, int phase, int *more_out, cudaStream_t t_stream)
 {
     if (!L || !L->is_slab || !L->cg || phase < 0 || !more_out) return STAG_EINVAL;
     stag_slab_cg *C = L->cg;
@@ -1517,14 +1502,13 @@ extern "C" int stag_slab_cg_step(stag_links_t *L, int action, int phase, int *mo
     switch (action) {
     case STAG_SLAB_ACT_NORM:
         if (phase == 0) {
-            C->seq_res = ++C->red_seq;
-            slab_residual_kernel<float, RES_NORM><<<C->gb, BLAS_BLOCK, 0, t_stream>>>(nullptr, C->b, nullptr, nullptr, C->n, w.partials, w.ctrl, make_comm(L, C->seq_res));
+                slab_residual_kernel<float, RES_NORM><<<C->gb, BLAS_BLOCK, 0, t_stream>>>(nullptr, C->b, nullptr, nullptr, C->n, w.partials, w.ctrl, make_comm(L));
             count_launch();
             KCHECK();
             more = true;
             rc = STAG_OK;
         } else if (phase == 1) {
-            slab_scalar_kernel<RES_NORM><<<1, 32, 0, t_stream>>>(w.ctrl, make_comm(L, C->seq_res));
+            slab_scalar_kernel<RES_NORM><<<1, 32, 0, t_stream>>>(w.ctrl, make_comm(L));
             count_launch();
             KCHECK();
             rc = STAG_OK;
@@ -1532,23 +1516,23 @@ extern "C" int stag_slab_cg_step(stag_links_t *L, int action, int phase, int *mo
         break;
     case STAG_SLAB_ACT_INIT:
         if (phase == 0 && C->lo) CU(cudaMemsetAsync(w.y32, 0, (size_t)C->n * sizeof(float), t_stream));
-        rc = slab_residual_phase<RES_INIT>(L, C, phase, false, C->lo, &more);
+        rc = slab_residual_phase<RES_INIT>(L, C, phase, false, C->lo, &more, t_stream);
         break;
     case STAG_SLAB_ACT_VERIFY:
-        rc = slab_residual_phase<RES_INIT>(L, C, phase, false, false, &more);
+        rc = slab_residual_phase<RES_INIT>(L, C, phase, false, false, &more, t_stream);
         break;
     case STAG_SLAB_ACT_UPDATE:
-        rc = slab_residual_phase<RES_UPDATE>(L, C, phase, true, true, &more);
+        rc = slab_residual_phase<RES_UPDATE>(L, C, phase, true, true, &more, t_stream);
         break;
     case STAG_SLAB_ACT_FINAL:
-        rc = slab_residual_phase<RES_FINAL>(L, C, phase, C->lo, false, &more);
+        rc = slab_residual_phase<RES_FINAL>(L, C, phase, C->lo, false, &more, t_stream);
         break;
     case STAG_SLAB_ACT_ITER: {
         const int total = 5 * C->P.graph_chunk;
         if (phase >= total) return STAG_EINVAL;
         more = phase + 1 < total;
-        if (C->lo) rc = slab_iteration_phase<float>(L, C, phase % 5, w.y32, w.r32, w.d32, w.q32, w.tmp32);
-        else rc = slab_iteration_phase<double>(L, C, phase % 5, C->x, w.r64, w.d64, w.q64, w.tmp64);
+        if (C->lo) rc = slab_iteration_phase<float>(L, C, phase % 5, w.y32, w.r32, w.d32, w.q32, w.tmp32, t_stream);
+        else rc = slab_iteration_phase<double>(L, C, phase % 5, C->x, w.r64, w.d64, w.q64, w.tmp64, t_stream);
         break;
     }
     default:
@@ -1596,6 +1580,32 @@ extern "C" int stag_slab_cg_run(stag_links_t *L, void *x_even, const void *b_eve
         int act = STAG_SLAB_ACT_DONE;
         if ((rc = stag_slab_cg_control(L, &act))) return rc;
         if (act == STAG_SLAB_ACT_DONE) break;
+        if (act == STAG_SLAB_ACT_ITER) {
+            // the chunk of iterations as ONE graph launch: possible because the exchange and
+            // reduction numbers live in device memory, not in the kernels' arguments
+            stag_slab_cg *C = L->cg;
+            if (!C->iter_graph) {
+                cudaGraph_t graph = nullptr;
+                cudaError_t e = cudaStreamBeginCapture(L->cap_stream, cudaStreamCaptureModeThreadLocal);
+                if (e != cudaSuccess) return cuda_fail(e, "cudaStreamBeginCapture", __LINE__);
+                t_capturing = true;
+                t_captured_nodes = 0;
+                int more = 1;
+                rc = STAG_OK;
+                for (int ph = 0; more && rc == STAG_OK; ++ph) rc = slab_cg_step_on(L, act, ph, &more, L->cap_stream);
+                t_capturing = false;
+                C->iter_graph_nodes = t_captured_nodes;
+                e = cudaStreamEndCapture(L->cap_stream, &graph);
+                if (rc != STAG_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+                if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture", __LINE__);
+                e = cudaGraphInstantiate(&C->iter_graph, graph, 0);
+                cudaGraphDestroy(graph);
+                if (e != cudaSuccess) return cuda_fail(e, "cudaGraphInstantiate", __LINE__);
+            }
+            CU(cudaGraphLaunch(C->iter_graph, t_stream));
+            count_launch(C->iter_graph_nodes);
+            continue;
+        }
         int more = 1;
         for (int ph = 0; more; ++ph)
             if ((rc = stag_slab_cg_step(L, act, ph, &more))) return rc;
@@ -1603,4 +1613,8 @@ extern "C" int stag_slab_cg_run(stag_links_t *L, void *x_even, const void *b_eve
     return stag_slab_cg_finish(L, stats_out);
 }
 
-static void stag_slab_cg_free(struct stag_slab_cg *c) { delete c; }
+static void stag_slab_cg_free(struct stag_slab_cg *c)
+{
+    if (c && c->iter_graph) cudaGraphExecDestroy(c->iter_graph);
+    delete c;
+}

@@ -28,25 +28,12 @@
 
 namespace stag {
 
-constexpr size_t XCH_HDR = 1024;
-constexpr size_t XCH_RED = 256;     // offset of XchReduce inside the header area
 constexpr int MAX_RANKS = STAG_MAX_RANKS;
 struct XchReduce {
     unsigned long long flag[MAX_RANKS];   // flag[r]: last reduction number rank r has published here
     double slot[2][MAX_RANKS];            // slot[seq & 1][r]: rank r's local total of reduction seq
 };
 static_assert(XCH_RED + sizeof(XchReduce) <= XCH_HDR, "reduction slots must fit the header area");
-struct XchHeader {
-    unsigned long long flag_back;   // epoch of the last completed push into my "back" halo
-    unsigned long long flag_fwd;    // ... into my "fwd" halo
-    unsigned ticket;                // last-block ticket of MY face_push_kernel (never peer-written)
-};
-static_assert(sizeof(XchHeader) <= XCH_RED, "exchange header must fit its slot");
-
-inline size_t xch_halo_offset(int s3, unsigned long long epoch, int dir)
-{
-    return XCH_HDR + ((size_t)((epoch & 1ull) * 2 + dir) * 3 * s3) * 16;
-}
 inline size_t xch_bytes(int s3) { return XCH_HDR + (size_t)4 * 3 * s3 * 16; }
 
 // in: one parity's device spinor of the slab (planes of Vh_pad).  Stores its last time slice into
@@ -55,10 +42,13 @@ inline size_t xch_bytes(int s3) { return XCH_HDR + (size_t)4 * 3 * s3 * 16; }
 template <typename T>
 __global__ void __launch_bounds__(256)
 face_push_kernel(const cplx_t<T> *__restrict__ in, const int Vh, const int Vh_pad, const int s3,
-                 cplx_t<T> *__restrict__ fwd_back, cplx_t<T> *__restrict__ bwd_fwd,
-                 unsigned long long *fwd_flag_back, unsigned long long *bwd_flag_fwd,
-                 const unsigned long long epoch, unsigned *ticket)
+                 char *mine, char *peer_fwd, char *peer_bwd)
 {
+    XchHeader *hdr = (XchHeader *)mine;
+    // every block reads the count before it takes its ticket; the last block bumps it afterwards
+    const unsigned long long epoch = __ldcg(&hdr->epoch) + 1;
+    cplx_t<T> *fwd_back = (cplx_t<T> *)(peer_fwd + xch_halo_offset(s3, epoch, 0));
+    cplx_t<T> *bwd_fwd = (cplx_t<T> *)(peer_bwd + xch_halo_offset(s3, epoch, 1));
     const long i = blockIdx.x * 256L + threadIdx.x;
     const long face = 3L * s3;
     if (i < 2 * face) {
@@ -69,11 +59,12 @@ face_push_kernel(const cplx_t<T> *__restrict__ in, const int Vh, const int Vh_pa
     }
     __threadfence_system();       // my peer stores are ordered before what follows, system-wide
     __syncthreads();
-    if (threadIdx.x == 0 && atomicAdd(ticket, 1u) == gridDim.x - 1) {
-        *ticket = 0;
+    if (threadIdx.x == 0 && atomicAdd(&hdr->ticket, 1u) == gridDim.x - 1) {
+        hdr->ticket = 0;
+        hdr->epoch = epoch;
         __threadfence_system();   // cumulativity: every block's stores precede the flags
-        asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(fwd_flag_back), "l"(epoch) : "memory");
-        asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(bwd_flag_fwd), "l"(epoch) : "memory");
+        asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)peer_fwd)->flag_back), "l"(epoch) : "memory");
+        asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)peer_bwd)->flag_fwd), "l"(epoch) : "memory");
     }
 }
 
@@ -105,13 +96,29 @@ __device__ __forceinline__ double gather_total(const char *mine, int nranks, uns
     return t;
 }
 
-// Comm: what a kernel of the slab CG needs to publish / gather (passed by value)
+// Comm: what a kernel of the slab CG needs to publish / gather (passed by value).  The number of
+// a reduction is not an argument: the publisher takes red_seq + 1 from its own header and stores
+// it back, the gatherer (a LATER kernel on the same stream) reads red_seq, so a captured graph of
+// iterations can be replayed.
 struct Comm {
     char *const *peers;     // device array of nranks pointers to every rank's exchange region
-    const char *mine;
+    char *mine;
     int nranks, myrank;
-    unsigned long long seq; // number of THIS launch's reduction (publish) or of the one to gather
 };
+
+// one thread
+__device__ __forceinline__ void publish_next(const Comm &c, double value)
+{
+    XchHeader *hdr = (XchHeader *)c.mine;
+    const unsigned long long seq = __ldcg(&hdr->red_seq) + 1;
+    publish_total(c.peers, c.nranks, c.myrank, seq, value);
+    hdr->red_seq = seq;
+}
+// any thread of a kernel launched after the publishing one
+__device__ __forceinline__ double gather_current(const Comm &c)
+{
+    return gather_total(c.mine, c.nranks, __ldcg(&((const XchHeader *)c.mine)->red_seq));
+}
 
 // Local fixed-order sum of the second hop's per-block partials of <d,Ad>, published to all ranks.
 __global__ void __launch_bounds__(BLAS_BLOCK)
@@ -121,16 +128,16 @@ slab_publish_partials_kernel(const double *__restrict__ partials, int n, const C
     if (ctrl->state != CG_RUN) return;
     __shared__ double red[32];
     const double t = block_total_fixed(partials, n, red);
-    if (threadIdx.x == 0) publish_total(c.peers, c.nranks, c.myrank, c.seq, t);
+    if (threadIdx.x == 0) publish_next(c, t);
 }
 
 // update_kernel for one right-hand side of a slab: <d,Ad> is the all-rank sum of reduction
-// c_in.seq; the local |r|^2 is published as reduction c_out.seq instead of running the epilogue.
+// last published; the local |r|^2 is published as the next one instead of running the epilogue.
 template <typename T>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 slab_update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
                    const T *__restrict__ q, long n, double *__restrict__ partials,
-                   CgCtrl *__restrict__ ctrl, const Comm c_in, const Comm c_out)
+                   CgCtrl *__restrict__ ctrl, const Comm c)
 {
     if (ctrl->state != CG_RUN) return;
     using V = typename Vec4<T>::type;
@@ -138,7 +145,7 @@ slab_update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d
     __shared__ double red[32];
     __shared__ double totals[MAX_RHS];
     __shared__ double s_dAd;
-    if (threadIdx.x == 0) s_dAd = gather_total(c_in.mine, c_in.nranks, c_in.seq);
+    if (threadIdx.x == 0) s_dAd = gather_current(c);     // every block reads red_seq before the last one bumps it
     __syncthreads();
     const double dAd = s_dAd;
     const bool ok = dAd > 0.0;
@@ -168,7 +175,7 @@ slab_update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d
     }
     const double bs = block_sum(s, red);
     if (!finish_reduction(bs, partials, &ctrl->ticket[1], red, totals)) return;
-    if (threadIdx.x == 0) publish_total(c_out.peers, c_out.nranks, c_out.myrank, c_out.seq, totals[0]);
+    if (threadIdx.x == 0) publish_next(c, totals[0]);
 }
 
 // residual_kernel for one right-hand side of a slab: publishes the local |r|^2 (or |b|^2).
@@ -176,7 +183,7 @@ template <typename T, int WHAT>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 slab_residual_kernel(double *__restrict__ r, const double *__restrict__ b,
                      const double *__restrict__ q, T *__restrict__ r_lo, long n,
-                     double *__restrict__ partials, CgCtrl *__restrict__ ctrl, const Comm c_out)
+                     double *__restrict__ partials, CgCtrl *__restrict__ ctrl, const Comm c)
 {
     double s = 0.0;
     for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < n; i += (long)gridDim.x * BLAS_BLOCK) {
@@ -194,18 +201,18 @@ slab_residual_kernel(double *__restrict__ r, const double *__restrict__ b,
     __shared__ double totals[MAX_RHS];
     const double bs = block_sum(s, red);
     if (!finish_reduction(bs, partials, &ctrl->ticket[2], red, totals)) return;
-    if (threadIdx.x == 0) publish_total(c_out.peers, c_out.nranks, c_out.myrank, c_out.seq, totals[0]);
+    if (threadIdx.x == 0) publish_next(c, totals[0]);
 }
 
 // The scalar step that follows a published reduction: gather the all-rank sum and run the same
 // epilogue the one-GPU kernels run in their last block.  WHAT: RES_* or SCALAR_ITER.
 enum { SCALAR_ITER = 100 };
 template <int WHAT>
-__global__ void slab_scalar_kernel(CgCtrl *__restrict__ ctrl, const Comm c_in)
+__global__ void slab_scalar_kernel(CgCtrl *__restrict__ ctrl, const Comm c)
 {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     if (WHAT == SCALAR_ITER && ctrl->state != CG_RUN) return;
-    double total = gather_total(c_in.mine, c_in.nranks, c_in.seq);
+    double total = gather_current(c);
     if (WHAT == SCALAR_ITER) cg_iteration_epilogue(ctrl, &total);
     else residual_epilogue<WHAT>(ctrl, &total);
 }
