@@ -279,9 +279,13 @@ def run_ours(args):
         return 0
 
     # ---- rank 0, N = any: the per-kernel numbers and the CPU baseline ---------------------------
-    dsl = {stag.PREC_NAMES[p]: time_dslash(stag, torch, fieldgen, cfg, L, p) for p in range(6)}
-    dsl["fp32/8"]["rebuilt_entry_error"] = L.recon8_error(stag.PREC_F32_R8)
-    dsl["fp64/8"]["rebuilt_entry_error"] = L.recon8_error(stag.PREC_F64_R8)
+    dsl = {stag.PREC_NAMES[p]: time_dslash(stag, torch, fieldgen, cfg, L, p) for p in range(4)}
+    for p in (stag.PREC_F64_R8, stag.PREC_F32_R8):      # refused on fields with nearly-unit links
+        try:
+            dsl[stag.PREC_NAMES[p]] = time_dslash(stag, torch, fieldgen, cfg, L, p)
+            dsl[stag.PREC_NAMES[p]]["rebuilt_entry_error"] = L.recon8_error(p)
+        except stag.StagError as e:
+            dsl[stag.PREC_NAMES[p]] = {"refused": str(e)}
     dom = dsl["fp32/12"]
     roofline = {"bound": "hbm", "kernel": "dslash_kernel<float,2,*> (fp32, 12-real links: the hop of the timed solve)",
                 "achieved": dom["gbs"], "peak": peak, "unit": "GB/s", "frac": dom["gbs"] / peak,
