@@ -119,7 +119,7 @@ __host__ __device__ constexpr int link_slots(int NR) { return NR == 1 ? 4 : 3 * 
 // of packets loaded ahead (group = K*GM packets).  With N > 1 right-hand sides the registers go
 // to the N accumulators and the N neighbour vectors of one group instead.
 template <typename T, int NR, int N> struct HopTune { static constexpr int MINB = 4, GM = 1; };
-template <> struct HopTune<float, 2, 1>            { static constexpr int MINB = 6, GM = 2; };
+template <> struct HopTune<float, 2, 1>            { static constexpr int MINB = 4, GM = 2; };
 // 8-parameter fp32: ALU-bound (two sincos, two sqrt, a reciprocal and eight complex products per
 // link); 4 blocks/SM with two directions in flight measured best (70.2 us; 6 blocks: 76.8 us)
 template <> struct HopTune<float, 1, 1>            { static constexpr int MINB = 4, GM = 2; };

@@ -189,9 +189,10 @@ def test_gauge_covariance_of_the_gpu_solve():
 
 
 @pytest.mark.slow
-@pytest.mark.parametrize("name,recon12", [("c4_28^3x96", False), ("c4_28^3x96", True)])
+@pytest.mark.parametrize("name,recon12", [("c4_28^3x96", False), ("c4_28^3x96", True), ("c5_48^3x96", True)])
 def test_mixed_cg_full_size_true_residual_with_oracle_A(name, recon12):
-    """BASELINE configs[3] in the configuration bench.py times: the oracle cannot solve this in
+    """BASELINE configs[3] in the configuration bench.py times, and configs[4] (48^3 x 96, smooth
+    links, m = 0.005: the ill-conditioned one): the oracle cannot solve these in
     seconds, so the unique solution is checked through its defining property with the ORACLE's
     A: |b - A_oracle x| / |b| <= tol, which bounds |x - A^-1 b| <= |r| / m^2."""
     cfg = fieldgen.CONFIGS[name]
