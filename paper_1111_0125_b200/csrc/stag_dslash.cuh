@@ -139,7 +139,11 @@ template <> struct HopMaxRhs<double> { static constexpr int value = 2; };
 // The kernel reads the number of the current exchange from the region's header (device memory,
 // so a graph replay sees the right one) and derives the halo buffers of that parity from it.
 template <typename T> struct HaloArgs {
-    const char *xch;     // this slab's exchange region
+    char *xch;           // this slab's exchange region
+    // HOP_PLAIN only, may be null: push the faces of OUT as the next exchange while computing it
+    // (the hop that produces the second hop's input stores its first / last time slice straight
+    // into the neighbours' halo buffers; its last block then bumps the count and sets their flags)
+    char *peer_fwd, *peer_bwd;
 };
 
 __device__ __forceinline__ void wait_flag(const unsigned long long *f, unsigned long long epoch)
@@ -190,6 +194,13 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
         }
     }
     const size_t rs = (size_t)3 * g.Vh_pad;
+    bool pushing = false;
+    unsigned long long e_in = 0;
+    if constexpr (HALO && MODE == HOP_PLAIN) {
+        pushing = halo.peer_fwd != nullptr;
+        // every block reads the count before it takes its ticket; the last block bumps it afterwards
+        if (pushing) e_in = __ldcg(&((const XchHeader *)halo.xch)->epoch);
+    }
     double dot[N];
 #pragma unroll
     for (int k = 0; k < N; ++k) dot[k] = 0.0;
@@ -287,6 +298,18 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
             if (MODE == HOP_PLAIN) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) st_keep(out + k * rs + (size_t)c * g.Vh_pad + cb, acc[k][c]);
+                if constexpr (HALO) {
+                    if (pushing && cb < g.Vh && (s.x3 == 0 || s.x3 == g.X3 - 1)) {
+                        // first slice -> the backward neighbour's "fwd" halo, last slice -> the
+                        // forward neighbour's "back" halo, buffers of exchange e_in + 1
+                        C *dst = (s.x3 == 0)
+                            ? (C *)(halo.peer_bwd + xch_halo_offset(g.s3, e_in + 1, 1)) + cb
+                            : (C *)(halo.peer_fwd + xch_halo_offset(g.s3, e_in + 1, 0)) + (cb - (g.Vh - g.s3));
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) dst[(size_t)c * g.s3] = acc[k][c];
+                        __threadfence_system();
+                    }
+                }
             } else {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -303,6 +326,20 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
                     if (MODE == HOP_XPAY_DOT)
                         dot[k] += (double)o.x * (double)r.x + (double)o.y * (double)r.y;
                 }
+            }
+        }
+    }
+
+    if constexpr (HALO && MODE == HOP_PLAIN) {
+        if (pushing) {       // uniform over the grid
+            __syncthreads();
+            XchHeader *hdr = (XchHeader *)halo.xch;
+            if (threadIdx.x == 0 && atomicAdd(&hdr->ticket, 1u) == gridDim.x - 1) {
+                hdr->ticket = 0;
+                hdr->epoch = e_in + 1;
+                __threadfence_system();   // cumulativity: every block's peer stores precede the flags
+                asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)halo.peer_fwd)->flag_back), "l"(e_in + 1) : "memory");
+                asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)halo.peer_bwd)->flag_fwd), "l"(e_in + 1) : "memory");
             }
         }
     }

@@ -1159,6 +1159,7 @@ int slab_hop_t(stag_links *L, int prec, cplx_t<T> *out, const cplx_t<T> *in, int
     const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
     HaloArgs<T> h;
     h.xch = L->xch;
+    h.peer_fwd = h.peer_bwd = nullptr;
     if (own)
         dslash_kernel<T, NR, HOP_XPAY, 1, true><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)1, own, nullptr, nullptr, h);
     else
@@ -1252,7 +1253,8 @@ Comm make_comm(const stag_links *L)
 
 template <typename T, int NR>
 int slab_hop_mode_t(stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx_t<T> *in, int parity,
-                    double a, const cplx_t<T> *own, double *partials, const CgCtrl *ctrl, cudaStream_t s)
+                    double a, const cplx_t<T> *own, double *partials, const CgCtrl *ctrl, cudaStream_t s,
+                    bool push_out = false)
 {
     const Geom &g = L->g;
     const pkt_t<T> *field = (const pkt_t<T> *)L->L[prec] +
@@ -1260,6 +1262,12 @@ int slab_hop_mode_t(stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx
     const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
     HaloArgs<T> h;
     h.xch = L->xch;
+    h.peer_fwd = h.peer_bwd = nullptr;
+    if (push_out && hop == HOP_PLAIN) {      // the faces of out go to the neighbours as the next exchange
+        h.peer_fwd = L->peer_fwd;
+        h.peer_bwd = L->peer_bwd;
+        ++L->epoch;
+    }
     switch (hop) {
     case HOP_PLAIN:
         dslash_kernel<T, NR, HOP_PLAIN, 1, true><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)0, (T)1, nullptr, nullptr, ctrl, h);
@@ -1277,13 +1285,13 @@ int slab_hop_mode_t(stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx
 }
 
 int slab_hop_mode(stag_links *L, int prec, int hop, void *out, const void *in, int parity, double a,
-                  const void *own, double *partials, const CgCtrl *ctrl, cudaStream_t s)
+                  const void *own, double *partials, const CgCtrl *ctrl, cudaStream_t s, bool push_out = false)
 {
     switch (prec) {
-    case STAG_PREC_F64:     return slab_hop_mode_t<double, 3>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, (const double2 *)own, partials, ctrl, s);
-    case STAG_PREC_F32:     return slab_hop_mode_t<float, 3>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, (const float2 *)own, partials, ctrl, s);
-    case STAG_PREC_F64_R12: return slab_hop_mode_t<double, 2>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, (const double2 *)own, partials, ctrl, s);
-    case STAG_PREC_F32_R12: return slab_hop_mode_t<float, 2>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, (const float2 *)own, partials, ctrl, s);
+    case STAG_PREC_F64:     return slab_hop_mode_t<double, 3>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, (const double2 *)own, partials, ctrl, s, push_out);
+    case STAG_PREC_F32:     return slab_hop_mode_t<float, 3>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, (const float2 *)own, partials, ctrl, s, push_out);
+    case STAG_PREC_F64_R12: return slab_hop_mode_t<double, 2>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, (const double2 *)own, partials, ctrl, s, push_out);
+    case STAG_PREC_F32_R12: return slab_hop_mode_t<float, 2>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, (const float2 *)own, partials, ctrl, s, push_out);
     default: break;
     }
     return STAG_EINVAL;
@@ -1336,14 +1344,15 @@ int slab_iteration_phase(stag_links *L, stag_slab_cg *C, int sub, T *y, T *r, T 
     Workspace &w = C->w;
     int rc;
     switch (sub) {
-    case 0:   // d = r + beta d ; its faces to the neighbours
-        xpay_kernel<T><<<dim3(C->gb, 1), BLAS_BLOCK, 0, s>>>(d, r, C->n, w.ctrl);
+    case 0:   // d = r + beta d, its faces stored into the neighbours' halos by the same kernel
+        ++L->epoch;
+        slab_xpay_push_kernel<T><<<C->gb, BLAS_BLOCK, 0, s>>>(d, r, C->n, w.ctrl, L->g.Vh, L->g.Vh_pad, L->g.s3,
+                                                             L->xch, L->peer_fwd, L->peer_bwd);
         count_launch();
         KCHECK();
-        return slab_push_prec(L, d, C->prec_lo, s);
-    case 1:   // tmp = D_oe d ; its faces
-        if ((rc = slab_hop_mode(L, C->prec_lo, HOP_PLAIN, tmp, d, 1, 0.0, nullptr, nullptr, w.ctrl, s))) return rc;
-        return slab_push_prec(L, tmp, C->prec_lo, s);
+        return STAG_OK;
+    case 1:   // tmp = D_oe d, the faces of tmp pushed by the boundary-slice threads of the same kernel
+        return slab_hop_mode(L, C->prec_lo, HOP_PLAIN, tmp, d, 1, 0.0, nullptr, nullptr, w.ctrl, s, true);
     case 2:   // q = m^2 d - D_eo tmp, local <d,q> published
         if ((rc = slab_hop_mode(L, C->prec_lo, HOP_XPAY_DOT, q, tmp, 0, C->m2, d, w.hop_partials, w.ctrl, s))) return rc;
         slab_publish_partials_kernel<<<1, BLAS_BLOCK, 0, s>>>(w.hop_partials, w.n_hop, make_comm(L), w.ctrl);

@@ -68,6 +68,62 @@ face_push_kernel(const cplx_t<T> *__restrict__ in, const int Vh, const int Vh_pa
     }
 }
 
+// d = r + beta d (xpay_kernel) that also pushes the faces of the new d: the producer of the first
+// hop's input stores the packets of its first / last time slice straight into the neighbours'
+// halo buffers.  Vectors are flat (3 colour planes of Vh_pad complex); a 16-byte packet never
+// straddles a slice because s3 and Vh are even.
+template <typename T>
+__global__ void __launch_bounds__(BLAS_BLOCK)
+slab_xpay_push_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const CgCtrl *__restrict__ ctrl,
+                      const int Vh, const int Vh_pad, const int s3, char *mine, char *peer_fwd, char *peer_bwd)
+{
+    if (ctrl->state != CG_RUN || !ctrl->active[0]) return;     // the same in every block: no ticket taken
+    using V = typename Vec4<T>::type;
+    constexpr int N = Vec4<T>::N;
+    constexpr int CPK = N / 2;                                 // complex numbers per packet
+    XchHeader *hdr = (XchHeader *)mine;
+    const unsigned long long epoch = __ldcg(&hdr->epoch) + 1;
+    V *fwd_back = (V *)(peer_fwd + xch_halo_offset(s3, epoch, 0));
+    V *bwd_fwd = (V *)(peer_bwd + xch_halo_offset(s3, epoch, 1));
+    const T beta = (T)ctrl->beta[0];
+    const long nv = n / N;
+    V *dv = reinterpret_cast<V *>(d);
+    const V *rv = reinterpret_cast<const V *>(r);
+    bool stored = false;
+    for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)gridDim.x * BLAS_BLOCK) {
+        T a[N], b[N];
+        unpack<T>(ld_keep(rv + i), a);
+        unpack<T>(ld_keep(dv + i), b);
+        if (beta == (T)0) {
+#pragma unroll
+            for (int j = 0; j < N; ++j) b[j] = a[j];
+        } else {
+#pragma unroll
+            for (int j = 0; j < N; ++j) b[j] = fma(beta, b[j], a[j]);
+        }
+        const V pk = pack(b);
+        st_keep(dv + i, pk);
+        const long ci = i * CPK;                               // first complex number of the packet
+        const int c = (int)(ci / Vh_pad), cb = (int)(ci % Vh_pad);
+        if (cb < s3) {                                         // first time slice
+            bwd_fwd[((long)c * s3 + cb) / CPK] = pk;
+            stored = true;
+        } else if (cb >= Vh - s3 && cb < Vh) {                 // last time slice
+            fwd_back[((long)c * s3 + (cb - (Vh - s3))) / CPK] = pk;
+            stored = true;
+        }
+    }
+    if (stored) __threadfence_system();
+    __syncthreads();
+    if (threadIdx.x == 0 && atomicAdd(&hdr->ticket, 1u) == gridDim.x - 1) {
+        hdr->ticket = 0;
+        hdr->epoch = epoch;
+        __threadfence_system();
+        asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)peer_fwd)->flag_back), "l"(epoch) : "memory");
+        asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)peer_bwd)->flag_fwd), "l"(epoch) : "memory");
+    }
+}
+
 // ---- global sums of the slab CG ---------------------------------------------------------
 // One thread: store my local total of reduction seq into every rank's slots, then the flags.
 __device__ __forceinline__ void publish_total(char *const *peers, int nranks, int myrank,
