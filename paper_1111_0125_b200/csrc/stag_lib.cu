@@ -113,6 +113,7 @@ struct stag_links {
     char *xch;
     char *peer_bwd, *peer_fwd;
     unsigned long long epoch;
+    unsigned n_push_blocks; // blocks of a HALO hop that own boundary-slice sites (cached)
     char **peers_dev;      // device array: every rank's exchange region (stag_slab_connect_all)
     int all_connected;
     struct stag_slab_cg *cg;   // state of the slab CG in progress (stag_slab_cg_*)
@@ -1160,6 +1161,7 @@ int slab_hop_t(stag_links *L, int prec, cplx_t<T> *out, const cplx_t<T> *in, int
     HaloArgs<T> h;
     h.xch = L->xch;
     h.peer_fwd = h.peer_bwd = nullptr;
+    h.n_push_blocks = 0;
     if (own)
         dslash_kernel<T, NR, HOP_XPAY, 1, true><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)1, own, nullptr, nullptr, h);
     else
@@ -1251,6 +1253,29 @@ Comm make_comm(const stag_links *L)
     return c;
 }
 
+// Blocks of a HALO hop launch that own at least one site of the first or last time slice (the hop
+// visits sites rotated by one slice: thread t of block b owns cb = (b*128 + t + s3) mod Vh_pad).
+unsigned push_block_count(const Geom &g)
+{
+    const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
+    unsigned n = 0;
+    for (unsigned b = 0; b < grid; ++b) {
+        bool any = false;
+        for (int t = 0; t < DSLASH_BLOCK && !any; ++t) {
+            int cb = (int)b * DSLASH_BLOCK + t;
+            if (cb >= g.Vh_pad) break;
+            cb += g.s3;
+            if (cb >= g.Vh_pad) cb -= g.Vh_pad;
+            if (cb < g.Vh) {
+                const int x3 = cb / g.s3;
+                any = (x3 == 0 || x3 == g.X3 - 1);
+            }
+        }
+        n += any ? 1u : 0u;
+    }
+    return n;
+}
+
 template <typename T, int NR>
 int slab_hop_mode_t(stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx_t<T> *in, int parity,
                     double a, const cplx_t<T> *own, double *partials, const CgCtrl *ctrl, cudaStream_t s,
@@ -1263,9 +1288,12 @@ int slab_hop_mode_t(stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx
     HaloArgs<T> h;
     h.xch = L->xch;
     h.peer_fwd = h.peer_bwd = nullptr;
+    h.n_push_blocks = 0;
     if (push_out && hop == HOP_PLAIN) {      // the faces of out go to the neighbours as the next exchange
         h.peer_fwd = L->peer_fwd;
         h.peer_bwd = L->peer_bwd;
+        if (L->n_push_blocks == 0) L->n_push_blocks = push_block_count(g);    // once per handle
+        h.n_push_blocks = L->n_push_blocks;
         ++L->epoch;
     }
     switch (hop) {
@@ -1355,7 +1383,7 @@ int slab_iteration_phase(stag_links *L, stag_slab_cg *C, int sub, T *y, T *r, T 
         return slab_hop_mode(L, C->prec_lo, HOP_PLAIN, tmp, d, 1, 0.0, nullptr, nullptr, w.ctrl, s, true);
     case 2:   // q = m^2 d - D_eo tmp, local <d,q> published
         if ((rc = slab_hop_mode(L, C->prec_lo, HOP_XPAY_DOT, q, tmp, 0, C->m2, d, w.hop_partials, w.ctrl, s))) return rc;
-        slab_publish_partials_kernel<<<1, BLAS_BLOCK, 0, s>>>(w.hop_partials, w.n_hop, make_comm(L), w.ctrl);
+        slab_publish_partials_kernel<<<1, 1024, 0, s>>>(w.hop_partials, w.n_hop, make_comm(L), w.ctrl);
         count_launch();
         KCHECK();
         return STAG_OK;

@@ -19,6 +19,11 @@
 // halo buffers [epoch & 1][dir][colour][s3] of 16-byte complex slots (fp32 uses the front half):
 //   dir 0 = "back":  the neighbour slice x3 = -1,  written by rank-1 from its LAST slice
 //   dir 1 = "fwd":   the neighbour slice x3 = X3,  written by rank+1 from its FIRST slice
+// Ordering of a push: every storing block's thread 0, after the block barrier, fences at gpu scope and
+// takes a ticket; the ticket's last holder has thereby observed all of them, fences at SYSTEM scope
+// (cumulative over everything that happens-before it, i.e. every block's peer stores) and only then
+// release-stores the flags.  One system-scope fence per launch instead of one per storing block:
+// those sat at the tail of the kernel and cost ~8 us.
 // Double buffering by epoch parity is enough: a rank cannot start exchange e+2 before both its
 // neighbours have finished consuming exchange e (its own hop e+1 waits for their push e+1, which
 // follows their hop e in stream order).
@@ -57,8 +62,8 @@ face_push_kernel(const cplx_t<T> *__restrict__ in, const int Vh, const int Vh_pa
         if (i < face) fwd_back[(size_t)c * s3 + j] = in[(size_t)c * Vh_pad + (Vh - s3) + j];
         else          bwd_fwd[(size_t)c * s3 + j] = in[(size_t)c * Vh_pad + j];
     }
-    __threadfence_system();       // my peer stores are ordered before what follows, system-wide
     __syncthreads();
+    if (threadIdx.x == 0) __threadfence();    // gpu-scope release of the block's peer stores (after the block barrier)
     if (threadIdx.x == 0 && atomicAdd(&hdr->ticket, 1u) == gridDim.x - 1) {
         hdr->ticket = 0;
         hdr->epoch = epoch;
@@ -104,7 +109,8 @@ slab_xpay_push_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const 
         const V pk = pack(b);
         st_keep(dv + i, pk);
         const long ci = i * CPK;                               // first complex number of the packet
-        const int c = (int)(ci / Vh_pad), cb = (int)(ci % Vh_pad);
+        const int c = (ci >= 2L * Vh_pad) ? 2 : (ci >= Vh_pad ? 1 : 0);      // colour plane, no division
+        const int cb = (int)(ci - (long)c * Vh_pad);
         if (cb < s3) {                                         // first time slice
             bwd_fwd[((long)c * s3 + cb) / CPK] = pk;
             stored = true;
@@ -113,8 +119,8 @@ slab_xpay_push_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const 
             stored = true;
         }
     }
-    if (stored) __threadfence_system();
-    __syncthreads();
+    const int any = __syncthreads_or(stored ? 1 : 0);
+    if (threadIdx.x == 0 && any) __threadfence();      // gpu-scope release of the block's peer stores (after the block barrier)
     if (threadIdx.x == 0 && atomicAdd(&hdr->ticket, 1u) == gridDim.x - 1) {
         hdr->ticket = 0;
         hdr->epoch = epoch;
@@ -129,13 +135,10 @@ slab_xpay_push_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const 
 __device__ __forceinline__ void publish_total(char *const *peers, int nranks, int myrank,
                                               unsigned long long seq, double value)
 {
+    // the release store of the flag orders this thread's slot store before it: no separate fence
     for (int r = 0; r < nranks; ++r) {
         XchReduce *R = (XchReduce *)(peers[r] + XCH_RED);
         *(volatile double *)&R->slot[seq & 1ull][myrank] = value;
-    }
-    __threadfence_system();
-    for (int r = 0; r < nranks; ++r) {
-        XchReduce *R = (XchReduce *)(peers[r] + XCH_RED);
         asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&R->flag[myrank]), "l"(seq) : "memory");
     }
 }
@@ -177,7 +180,7 @@ __device__ __forceinline__ double gather_current(const Comm &c)
 }
 
 // Local fixed-order sum of the second hop's per-block partials of <d,Ad>, published to all ranks.
-__global__ void __launch_bounds__(BLAS_BLOCK)
+__global__ void __launch_bounds__(1024)
 slab_publish_partials_kernel(const double *__restrict__ partials, int n, const Comm c,
                              const CgCtrl *__restrict__ ctrl)
 {
