@@ -1,0 +1,402 @@
+// stag_host_cg.cuh -- the CG drivers of one GPU (Fig. 1, Fig. 2, section 3.2; several right-hand sides; the (D+m) wrapper) and their C ABI
+//
+// A section of libstag's single translation unit: included by stag_lib.cu, which holds the
+// per-thread state, the error / launch-count helpers and the link handle these sections share.
+// Not a stand-alone header.
+
+// ------------------------------------------------------------------------------------
+// the CG drivers
+// ------------------------------------------------------------------------------------
+namespace {
+
+struct Workspace {
+    CgCtrl *ctrl;
+    double *partials;       // block partials of the vector kernels' reductions, [rhs][block]
+    double *hop_partials;   // block partials of <d,Ad> written by the second hop, [rhs][block]
+    int n_hop;              // = grid of the hop
+    double *r64, *q64, *tmp64, *d64;          // nrhs spinors each
+    float *y32, *r32, *d32, *q32, *tmp32;
+};
+
+// One allocation on the handle, sized for nrhs right-hand sides (grown when a later solve
+// carries more).  Right-hand side k of every vector starts k*n reals in (n = 6*Vh_pad).
+int ensure_workspace(stag_links *L, Workspace &w, int nrhs)
+{
+    const size_t n = (size_t)6 * L->g.Vh_pad;
+    if (L->ws && L->ws_rhs < nrhs) { CU(cudaFree(L->ws)); L->ws = nullptr; }
+    const int cap = L->ws ? L->ws_rhs : nrhs;
+    const size_t nb64 = align_up(cap * n * sizeof(double), 256), nb32 = align_up(cap * n * sizeof(float), 256);
+    const size_t n_hop = ((size_t)L->g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK;
+    const size_t pb = align_up((size_t)MAX_RHS * blas_full_grid() * sizeof(double), 256);
+    const size_t hb = align_up((size_t)cap * n_hop * sizeof(double), 256);
+    const size_t total = CTRL_SLOT + pb + hb + 4 * nb64 + 5 * nb32;
+    if (!L->ws) {
+        CU(cudaMalloc((void **)&L->ws, total));
+        L->ws_bytes = total;
+        L->ws_rhs = cap;
+    }
+    if (!L->h_ctrl) CU(cudaMallocHost((void **)&L->h_ctrl, sizeof(CgCtrl)));
+    char *p = L->ws;
+    w.ctrl = (CgCtrl *)p; p += CTRL_SLOT;
+    w.partials = (double *)p; p += pb;
+    w.hop_partials = (double *)p; p += hb;
+    w.n_hop = (int)n_hop;
+    w.r64 = (double *)p; p += nb64;
+    w.q64 = (double *)p; p += nb64;
+    w.tmp64 = (double *)p; p += nb64;
+    w.d64 = (double *)p; p += nb64;
+    w.y32 = (float *)p; p += nb32;
+    w.r32 = (float *)p; p += nb32;
+    w.d32 = (float *)p; p += nb32;
+    w.q32 = (float *)p; p += nb32;
+    w.tmp32 = (float *)p; p += nb32;
+    return STAG_OK;
+}
+
+struct Solver {
+    stag_links *L;
+    Workspace w;
+    cudaStream_t s;
+    double m2;
+    int mode;
+    int nrhs;
+    int prec_lo;     // precision enum of the iteration's Dslash
+    int prec_hi;     // precision enum of the fp64 corrections
+    long n;          // reals per spinor
+    int gb;          // blas grid.x (blocks per right-hand side)
+    int applies_f64;
+
+    dim3 grid2() const { return dim3((unsigned)gb, (unsigned)nrhs); }
+
+    // q64 = A x  in fp64 (two hops), outside the iteration
+    int apply_A64(const double *x)
+    {
+        int rc = launch_hop(L, prec_hi, HOP_PLAIN, w.tmp64, x, 1, 0.0, 1.0, nullptr, nullptr, nullptr, nrhs, s);
+        if (rc) return rc;
+        ++applies_f64;
+        return launch_hop(L, prec_hi, HOP_XPAY, w.q64, w.tmp64, 0, m2, 1.0, x, nullptr, nullptr, nrhs, s);
+    }
+
+    template <int WHAT>
+    int residual(const double *b, bool lo_copy)
+    {
+        residual_kernel<float, WHAT><<<grid2(), BLAS_BLOCK, 0, s>>>(w.r64, b, w.q64, lo_copy ? w.r32 : nullptr, n, w.partials, w.ctrl);
+        count_launch();
+        KCHECK();
+        return STAG_OK;
+    }
+
+    int accumulate(double *x)
+    {
+        accumulate_kernel<float><<<blas_grid(n * nrhs, 1), BLAS_BLOCK, 0, s>>>(x, w.y32, n * nrhs);
+        count_launch();
+        KCHECK();
+        return STAG_OK;
+    }
+
+    // one pass of the loop body of Fig. 1, four launches (the hops: one launch per
+    // chunk of right-hand sides)
+    template <typename T>
+    int iteration(T *y, T *r, T *d, T *q, T *tmp, cudaStream_t st)
+    {
+        xpay_kernel<T><<<grid2(), BLAS_BLOCK, 0, st>>>(d, r, n, w.ctrl);                     // d = r + beta d
+        count_launch();
+        KCHECK();
+        int rc = launch_hop(L, prec_lo, HOP_PLAIN, tmp, d, 1, 0.0, 1.0, nullptr, nullptr, w.ctrl, nrhs, st);   // D_oe d
+        if (rc) return rc;
+        rc = launch_hop(L, prec_lo, HOP_XPAY_DOT, q, tmp, 0, m2, 1.0, d, w.hop_partials, w.ctrl, nrhs, st);  // q = A d, <d,q>
+        if (rc) return rc;
+        update_kernel<T><<<grid2(), BLAS_BLOCK, 0, st>>>(y, r, d, q, n, w.hop_partials, w.n_hop, w.partials, w.ctrl);  // alpha, y, r, delta, beta
+        count_launch();
+        KCHECK();
+        return STAG_OK;
+    }
+
+    int iteration_mode(double *x, cudaStream_t st)
+    {
+        if (mode == STAG_CG_F64) return iteration<double>(x, w.r64, w.d64, w.q64, w.tmp64, st);
+        return iteration<float>(w.y32, w.r32, w.d32, w.q32, w.tmp32, st);
+    }
+
+    int read_ctrl()
+    {
+        CU(cudaMemcpyAsync(L->h_ctrl, w.ctrl, sizeof(CgCtrl), cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+        return STAG_OK;
+    }
+};
+
+// nrhs right-hand sides in lockstep.  x, b: nrhs fp64 device spinors
+// back to back.  stats: nrhs entries, or null.
+int cg_solve_device(double *x, const double *b, stag_links *L, double mass, double tol, int maxiter,
+                    int mode, int nrhs, const stag_cg_params_t *prm, stag_cg_stats_t *stats)
+{
+    stag_cg_params_t P;
+    memset(&P, 0, sizeof(P));
+    if (prm) P = *prm;
+    if (!(P.eps_in > 0.0)) P.eps_in = (mode == STAG_CG_DEFECT) ? 1e-2 : 0.1;
+    if (P.graph_chunk == 0) P.graph_chunk = 32;
+
+    Solver S;
+    S.L = L;
+    S.s = t_stream;
+    S.m2 = mass * mass;
+    S.mode = mode;
+    S.nrhs = nrhs;
+    S.prec_lo = (mode == STAG_CG_F64) ? (P.recon8 ? STAG_PREC_F64_R8 : P.recon12 ? STAG_PREC_F64_R12 : STAG_PREC_F64)
+                                       : (P.recon8 ? STAG_PREC_F32_R8 : P.recon12 ? STAG_PREC_F32_R12 : STAG_PREC_F32);
+    S.prec_hi = P.recon12_f64 ? STAG_PREC_F64_R12 : STAG_PREC_F64;
+    S.n = (long)6 * L->g.Vh_pad;
+    S.gb = blas_grid(S.n, nrhs);
+    S.applies_f64 = 0;
+    int rc;
+    if ((rc = ensure_links(L, S.prec_lo))) return rc;
+    if ((rc = ensure_links(L, S.prec_hi))) return rc;
+    if ((rc = ensure_workspace(L, S.w, nrhs))) return rc;
+    Workspace &w = S.w;
+    cudaStream_t s = S.s;
+    const bool lo = (mode != STAG_CG_F64);
+    const size_t vec_bytes = (size_t)S.n * sizeof(double);
+
+    CU(cudaEventRecord(L->ev0, s));
+
+    // ---- |b_k|^2 and the solver scalars ---------------------------------------------------
+    CgCtrl *h = L->h_ctrl;
+    memset(h, 0, sizeof(*h));
+    h->mode = mode;
+    h->maxiter = maxiter;
+    h->eps_in = P.eps_in;
+    h->nrhs = nrhs;
+    CU(cudaMemcpyAsync(w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, s));
+    residual_kernel<float, RES_NORM><<<S.grid2(), BLAS_BLOCK, 0, s>>>(nullptr, b, nullptr, nullptr, S.n, w.partials, w.ctrl);
+    count_launch();
+    KCHECK();
+    if ((rc = S.read_ctrl())) return rc;
+    double bnorm2[MAX_RHS];
+    bool all_zero = true, bad = false;
+    for (int k = 0; k < nrhs; ++k) {
+        bnorm2[k] = h->bnorm2[k];
+        if (bnorm2[k] != 0.0) all_zero = false;
+        if (!(bnorm2[k] == bnorm2[k]) || std::isinf(bnorm2[k])) bad = true;
+    }
+
+    stag_cg_stats_t zero;
+    memset(&zero, 0, sizeof(zero));
+    if (bad) {
+        for (int k = 0; stats && k < nrhs; ++k) { stats[k] = zero; stats[k].true_resid = NAN; }
+        return STAG_EBREAKDOWN;
+    }
+    // b_k = 0  =>  x_k = 0 exactly, nothing to iterate for k (no 0/0)
+    for (int k = 0; k < nrhs; ++k)
+        if (bnorm2[k] == 0.0) CU(cudaMemsetAsync(x + (size_t)k * S.n, 0, vec_bytes, s));
+    if (all_zero) {
+        CU(cudaEventRecord(L->ev1, s));
+        CU(cudaStreamSynchronize(s));
+        for (int k = 0; stats && k < nrhs; ++k) stats[k] = zero;
+        return STAG_OK;
+    }
+    for (int k = 0; k < nrhs; ++k) h->tol2b[k] = tol * tol * bnorm2[k];
+    CU(cudaMemcpyAsync(w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, s));
+
+    // ---- r = b - A x0 (P:L46 / Fig. 2), in fp64 -------------------------------------
+    if ((rc = S.apply_A64(x))) return rc;
+    if ((rc = S.residual<RES_INIT>(b, lo))) return rc;
+    if (lo) CU(cudaMemsetAsync(w.y32, 0, (size_t)nrhs * S.n * sizeof(float), s));
+    // beta = 0 makes the first xpay d = r without reading d, so d needs no initial value
+
+    // ---- the iteration as a CUDA graph of `chunk` passes ----------------------------------
+    const int chunk = P.graph_chunk;
+    cudaGraphExec_t gexec = nullptr;
+    unsigned long long graph_nodes = 0;
+    if (chunk > 0) {
+        cudaGraph_t graph = nullptr;
+        cudaError_t e = cudaStreamBeginCapture(L->cap_stream, cudaStreamCaptureModeThreadLocal);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaStreamBeginCapture", __LINE__);
+        t_capturing = true;
+        t_captured_nodes = 0;
+        rc = STAG_OK;
+        for (int i = 0; i < chunk && rc == STAG_OK; ++i) rc = S.iteration_mode(x, L->cap_stream);
+        t_capturing = false;
+        graph_nodes = t_captured_nodes;
+        e = cudaStreamEndCapture(L->cap_stream, &graph);
+        if (rc != STAG_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture", __LINE__);
+        e = cudaGraphInstantiate(&gexec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaGraphInstantiate", __LINE__);
+    }
+    struct GraphGuard { cudaGraphExec_t g; ~GraphGuard() { if (g) cudaGraphExecDestroy(g); } } guard{gexec};
+
+    int n_restarts = 0, n_outer = 0;
+    int final_state = CG_RUN;
+    bool have_true = true;      // ctrl->sum0[k] holds |b_k - A x_k|^2 for the current x
+    bool verifying = false;     // mode 0: the last launch was the true-residual check of Q6b
+    for (;;) {
+        if ((rc = S.read_ctrl())) return rc;
+        const int state = h->state;
+        if (state == CG_RUN) {
+            if (verifying) ++n_restarts;
+            verifying = false;
+            if (gexec) {
+                CU(cudaGraphLaunch(gexec, s));
+                count_launch(graph_nodes);
+            } else {
+                for (int i = 0; i < 8; ++i) if ((rc = S.iteration_mode(x, s))) return rc;
+            }
+            have_true = false;
+            continue;
+        }
+        if (state == CG_UPDATE) {                      // section 3.2: mode 3 only
+            if ((rc = S.accumulate(x))) return rc;                 // x += y ; y = 0
+            if ((rc = S.apply_A64(x))) return rc;
+            if ((rc = S.residual<RES_UPDATE>(b, true))) return rc; // r = b - A x -> r32, beta
+            have_true = true;
+            continue;
+        }
+        if (state == CG_CONVERGED && !have_true) {
+            if (mode == STAG_CG_F64) {                 // Q6b: verify on the true residual
+                if ((rc = S.apply_A64(x))) return rc;
+                if ((rc = S.residual<RES_INIT>(b, false))) return rc;
+                have_true = true;
+                verifying = true;
+                continue;
+            }
+            if (mode == STAG_CG_DEFECT) {              // Fig. 2 outer step
+                if ((rc = S.accumulate(x))) return rc;
+                if ((rc = S.apply_A64(x))) return rc;
+                if ((rc = S.residual<RES_INIT>(b, true))) return rc;
+                have_true = true;
+                ++n_outer;
+                continue;
+            }
+            if (mode == STAG_CG_F32) {
+                if ((rc = S.accumulate(x))) return rc;
+                if ((rc = S.apply_A64(x))) return rc;
+                if ((rc = S.residual<RES_FINAL>(b, false))) return rc;
+                have_true = true;
+                final_state = CG_CONVERGED;
+                if ((rc = S.read_ctrl())) return rc;
+                break;
+            }
+        }
+        if (state == CG_CONVERGED) { final_state = CG_CONVERGED; break; }
+        // CG_MAXITER or CG_BREAKDOWN: fold y into x, report the true residual
+        final_state = state;
+        if (!have_true) {
+            if (lo && (rc = S.accumulate(x))) return rc;
+            if ((rc = S.apply_A64(x))) return rc;
+            if ((rc = S.residual<RES_FINAL>(b, false))) return rc;
+            if ((rc = S.read_ctrl())) return rc;
+        }
+        break;
+    }
+    CU(cudaEventRecord(L->ev1, s));
+    CU(cudaStreamSynchronize(s));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, L->ev0, L->ev1));
+
+    bool all_met = true;
+    for (int k = 0; k < nrhs; ++k) {
+        stag_cg_stats_t st = zero;
+        st.iters = h->iters[k];
+        st.n_updates = (mode == STAG_CG_DEFECT) ? n_outer : h->n_updates;
+        st.n_restarts = n_restarts;
+        st.iters_f32 = lo ? h->iters[k] : 0;
+        st.applies_f64 = S.applies_f64;
+        st.true_resid = bnorm2[k] > 0.0 ? sqrt(h->sum0[k] / bnorm2[k]) : 0.0;
+        st.iter_resid = bnorm2[k] > 0.0 ? sqrt(h->sum1[k] / bnorm2[k]) : 0.0;
+        st.seconds = ms * 1e-3;
+        if (!(st.true_resid <= tol)) all_met = false;
+        if (stats) stats[k] = st;
+    }
+    if (final_state == CG_BREAKDOWN) return STAG_EBREAKDOWN;
+    if (!all_met) return STAG_ENOCONV;
+    return STAG_OK;
+}
+
+}  // namespace
+
+extern "C" int stag_cg_solve_mrhs(void *x_even, const void *b_even, const stag_links_t *links,
+                                  double mass, double tol, int maxiter, int mode, int nrhs,
+                                  const stag_cg_params_t *params, stag_cg_stats_t *stats_out)
+{
+    stag_links *L = const_cast<stag_links *>(links);
+    if (!x_even || !b_even || !L || x_even == b_even || !(tol > 0.0) || maxiter < 0 || mode < 0 ||
+        mode > 3 || nrhs < 1 || nrhs > MAX_RHS || L->is_slab)
+        return STAG_EINVAL;
+    return cg_solve_device((double *)x_even, (const double *)b_even, L, mass, tol, maxiter, mode,
+                           nrhs, params, stats_out);
+}
+
+extern "C" int stag_cg_solve_ex(void *x_even, const void *b_even, const stag_links_t *links,
+                                double mass, double tol, int maxiter, int mode,
+                                const stag_cg_params_t *params, stag_cg_stats_t *stats_out)
+{
+    return stag_cg_solve_mrhs(x_even, b_even, links, mass, tol, maxiter, mode, 1, params, stats_out);
+}
+
+extern "C" int stag_cg_solve(void *x_even, const void *b_even, const stag_links_t *links,
+                             double mass, double tol, int maxiter, int mode, int *iters_out,
+                             double *true_resid_out)
+{
+    stag_cg_stats_t st;
+    memset(&st, 0, sizeof(st));
+    int rc = stag_cg_solve_ex(x_even, b_even, links, mass, tol, maxiter, mode, nullptr, &st);
+    if (rc < 0) return rc;
+    if (iters_out) *iters_out = st.iters;
+    if (true_resid_out) *true_resid_out = st.true_resid;
+    return rc;
+}
+
+extern "C" int stag_cg_solve_host(double *x_host, const double *b_host, const stag_links_t *links,
+                                  double mass, double tol, int maxiter, int mode,
+                                  const stag_cg_params_t *params, stag_cg_stats_t *stats_out)
+{
+    stag_links *L = const_cast<stag_links *>(links);
+    if (!x_host || !b_host || !L || x_host == b_host) return STAG_EINVAL;
+    const size_t nc = (size_t)L->g.Vh * 6;         // canonical doubles
+    const size_t nd = (size_t)L->g.Vh_pad * 6;     // device-layout doubles
+    if (!L->stage_dev) CU(cudaMalloc((void **)&L->stage_dev, (2 * nc + 2 * nd) * sizeof(double)));
+    double *cx = L->stage_dev, *cb = cx + nc, *dx = cb + nc, *db = dx + nd;
+    CU(cudaMemcpyAsync(cb, b_host, nc * sizeof(double), cudaMemcpyHostToDevice, t_stream));
+    CU(cudaMemcpyAsync(cx, x_host, nc * sizeof(double), cudaMemcpyHostToDevice, t_stream));
+    int rc;
+    if ((rc = stag_spinor_pack(db, cb, L->dims, STAG_PREC_F64))) return rc;
+    if ((rc = stag_spinor_pack(dx, cx, L->dims, STAG_PREC_F64))) return rc;
+    const int solve_rc = stag_cg_solve_ex(dx, db, L, mass, tol, maxiter, mode, params, stats_out);
+    if (solve_rc < 0) return solve_rc;
+    if ((rc = stag_spinor_unpack(cx, dx, L->dims, STAG_PREC_F64))) return rc;
+    CU(cudaMemcpyAsync(x_host, cx, nc * sizeof(double), cudaMemcpyDeviceToHost, t_stream));
+    CU(cudaStreamSynchronize(t_stream));
+    return solve_rc;
+}
+
+// (D + m) psi = h on the whole lattice through the even-site solve (Q23):
+//   b_e = m h_e - D_eo h_o ;  A psi_e = b_e ;  psi_o = (h_o - D_oe psi_e) / m
+// The two extra hops run in fp64 on the 18-real links; b_e lives in scratch on the handle.
+extern "C" int stag_solve_M(void *psi_even, void *psi_odd, const void *h_even, const void *h_odd,
+                            const stag_links_t *links, double mass, double tol, int maxiter,
+                            int mode, int nrhs, const stag_cg_params_t *params,
+                            stag_cg_stats_t *stats_out)
+{
+    stag_links *L = const_cast<stag_links *>(links);
+    if (!psi_even || !psi_odd || !h_even || !h_odd || !L || psi_even == h_even ||
+        psi_odd == h_odd || !(tol > 0.0) || maxiter < 0 || mode < 0 || mode > 3 || nrhs < 1 ||
+        nrhs > MAX_RHS || mass == 0.0 || L->is_slab)
+        return STAG_EINVAL;
+    int rc;
+    if ((rc = ensure_links(L, STAG_PREC_F64))) return rc;
+    const size_t bytes = (size_t)nrhs * 6 * L->g.Vh_pad * sizeof(double);
+    if (L->wrap_b && L->wrap_b_rhs < nrhs) { CU(cudaFree(L->wrap_b)); L->wrap_b = nullptr; }
+    if (!L->wrap_b) { CU(cudaMalloc(&L->wrap_b, bytes)); L->wrap_b_rhs = nrhs; }
+    // step 1: b_e = m h_e - D_eo h_o
+    if ((rc = launch_hop(L, STAG_PREC_F64, HOP_XPAY, L->wrap_b, h_odd, 0, mass, 1.0, h_even, nullptr, nullptr, nrhs, t_stream))) return rc;
+    // step 2: A psi_e = b_e (psi_even holds the initial guess on entry)
+    const int solve_rc = cg_solve_device((double *)psi_even, (const double *)L->wrap_b, L, mass, tol,
+                                         maxiter, mode, nrhs, params, stats_out);
+    if (solve_rc < 0) return solve_rc;
+    // step 3: psi_o = (1/m) h_o - (1/m) D_oe psi_e
+    if ((rc = launch_hop(L, STAG_PREC_F64, HOP_AXPBY, psi_odd, psi_even, 1, 1.0 / mass, 1.0 / mass, h_odd, nullptr, nullptr, nrhs, t_stream))) return rc;
+    return solve_rc;
+}
+
