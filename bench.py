@@ -290,7 +290,7 @@ def run_ours(args):
     roofline = {"bound": "hbm", "kernel": "dslash_kernel<float,2,*> (fp32, 12-real links: the hop of the timed solve)",
                 "achieved": dom["gbs"], "peak": peak, "unit": "GB/s", "frac": dom["gbs"] / peak,
                 "peak_source": peak_src, "traffic": args.traffic if cfg.name == "c4_28^3x96" else None,
-                "traffic_source": "profiles/r1d_dslash_fp32r12_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum, one launch)",
+                "traffic_source": "profiles/r1e_dslash_fp32r12_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum, one launch)",
                 "algorithmic_bytes_per_launch": dom["algorithmic_bytes_per_site"] * cfg.vh,
                 "us_per_launch": dom["us"], "frac_of_nominal_8TBs": dom["gbs"] / 8000.0}
     x64, st64 = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_F64)
@@ -461,9 +461,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--decomp", choices=["replicas", "slabs"], default="replicas",
                     help="N > 1: independent replicas (weak scaling, default) or one lattice in T-slabs (strong)")
-    ap.add_argument("--traffic", type=float, default=436.3e6,
+    ap.add_argument("--traffic", type=float, default=436.2e6,
                     help="dram bytes (read + write) per launch of the dominant kernel from the ncu --set full "
-                         "capture profiles/r1d_dslash_fp32r12_ncu_full.md (28^3x96, fp32/12 plain hop)")
+                         "capture profiles/r1e_dslash_fp32r12_ncu_full.md (28^3x96, fp32/12 plain hop)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
