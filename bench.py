@@ -295,6 +295,7 @@ def run_ours(args):
                 "us_per_launch": dom["us"], "frac_of_nominal_8TBs": dom["gbs"] / 8000.0}
     x64, st64 = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_F64)
     x18, st18 = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE)
+    x64c, st64c = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_F64, recon12=True)
 
     # several right-hand sides sharing each pass over the links: three
     # Gaussian sources in lockstep, and the batch hop alone
@@ -334,6 +335,7 @@ def run_ours(args):
                "true_resid": st["true_resid"], "time_to_solution_s": st["seconds"],
                "ms_per_iteration": st["seconds"] / max(1, st["iters"]) * 1e3,
                "fp64_cg": {"iters": st64["iters"], "time_to_solution_s": st64["seconds"], "true_resid": st64["true_resid"]},
+               "fp64_cg_12real_links": {"iters": st64c["iters"], "time_to_solution_s": st64c["seconds"], "true_resid": st64c["true_resid"]},
                "mixed_18real_links": {"iters": st18["iters"], "time_to_solution_s": st18["seconds"], "true_resid": st18["true_resid"],
                                       "ms_per_iteration": st18["seconds"] / max(1, st18["iters"]) * 1e3},
                "speedup_mixed_vs_fp64": st64["seconds"] / st["seconds"]},

@@ -208,3 +208,28 @@ def test_slab_cg_run_single_call_on_one_rank():
     xs, sts = slab.cg_solve_in_process(S, [bd], cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE)
     x, st = S[0].cg_solve(bd, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE)
     assert st["iters"] == sts[0]["iters"] and torch.equal(x, xs[0])
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("nranks", [2, 4, 8])
+def test_slab_hop_full_size_bitwise_against_whole_lattice(nranks):
+    """bench configuration (28^3 x 96) split into 2, 4, 8 slabs on one device: both hops in the
+    precisions of the timed solve must reproduce the whole-lattice kernel bit for bit."""
+    import torch
+    cfg = fieldgen.CONFIGS["c4_28^3x96"]
+    W = cfg.links()
+    L = stag.Links(cfg.dims, W)
+    slabs = make_slabs(cfg.dims, W, nranks)
+    del W
+    chi = cfg.source()
+    for prec in (stag.PREC_F32_R12, stag.PREC_F64):
+        whole1 = stag.dslash(stag.spinor_pack(chi, cfg.dims, prec), L, 1, prec)
+        w1 = stag.spinor_unpack(whole1, cfg.dims, prec)
+        outs, got = slab_hop_all(slabs, chi, cfg.dims, 1, prec)
+        assert np.array_equal(got, w1)
+        whole0 = stag.spinor_unpack(stag.dslash(whole1, L, 0, prec), cfg.dims, prec)
+        _, got0 = slab_hop_all(slabs, w1, cfg.dims, 0, prec)
+        assert np.array_equal(got0, whole0)
+    for s in slabs:
+        s.close()
+    L.close()
