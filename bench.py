@@ -114,7 +114,7 @@ def oracle_sample(cfg, W, b, target_seconds: float):
     t0 = time.perf_counter()
     oracle.apply_A(b, W, cfg.dims, cfg.mass)
     t_a = time.perf_counter() - t0
-    iters = int(max(3, min(400, target_seconds / max(t_a * 1.15, 1e-6))))
+    iters = int(max(3, min(1000, target_seconds / max(t_a * 1.15, 1e-6))))
     t0 = time.perf_counter()
     _, it, _, _, _ = oracle.cg(b, W, cfg.dims, cfg.mass, 1e-30, iters)
     dt = time.perf_counter() - t0
