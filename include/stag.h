@@ -57,6 +57,8 @@ enum {
                               tol <= 0, maxiter < 0, out aliases in, 12-real unavailable     */
     STAG_ECUDA      = -2,  /* a CUDA call failed; text via stag_strerror(STAG_ECUDA)         */
     STAG_ENOMEM     = -3,  /* device or host allocation failed                               */
+    STAG_ETIMEOUT   = -4,  /* T-slabs: a kernel gave up waiting for a neighbour's exchange or global
+                              sum (missing, mis-ordered or dead peer); results are not valid     */
     STAG_ENOCONV    = 1,   /* maxiter reached; x, iters and the true residual ARE written    */
     STAG_EBREAKDOWN = 2    /* NaN or <d,Ad> <= 0; x, iters and the true residual ARE written */
 };
@@ -221,6 +223,14 @@ int stag_slab_hop(void *out, const void *in, stag_links_t *slab, int parity, int
                   const void *own);
 /* push + hop: what each rank of a real multi-GPU run calls. */
 int stag_slab_dslash(void *out, const void *in, stag_links_t *slab, int parity, int prec);
+
+/* Watchdog.  A kernel that waits for a neighbour's flag polls it at most `polls` times (about a
+ * microsecond each; 0 restores the default of 2^23, roughly ten seconds), then gives up, marks the
+ * slab and finishes on stale data instead of spinning for ever.  stag_slab_status synchronises
+ * the stream and returns STAG_ETIMEOUT if that has happened since the slab was made (also reported
+ * by stag_slab_cg_control / _finish), STAG_OK otherwise. */
+int stag_slab_set_wait_limit(stag_links_t *slab, unsigned long long polls);
+int stag_slab_status(stag_links_t *slab);
 
 /* ---- the solver -------------------------------------------------------- */
 

@@ -36,7 +36,7 @@ _HEADER = os.path.join(os.path.dirname(_HERE), "include", "stag.h")
 
 PREC_F64, PREC_F32, PREC_F64_R12, PREC_F32_R12, PREC_F64_R8, PREC_F32_R8 = 0, 1, 2, 3, 4, 5
 CG_F64, CG_F32, CG_DEFECT, CG_RELIABLE = 0, 1, 2, 3
-OK, EINVAL, ECUDA, ENOMEM, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, 1, 2
+OK, EINVAL, ECUDA, ENOMEM, ETIMEOUT, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, 1, 2
 
 MAX_RHS = 12
 
@@ -126,6 +126,8 @@ SIGNATURES = {
     "stag_slab_push": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
     "stag_slab_hop": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, ctypes.c_int, ctypes.c_double, _vp]),
     "stag_slab_dslash": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, ctypes.c_int]),
+    "stag_slab_set_wait_limit": (ctypes.c_int, [_vp, ctypes.c_ulonglong]),
+    "stag_slab_status": (ctypes.c_int, [_vp]),
     "stag_slab_connect_all": (ctypes.c_int, [_vp, ctypes.POINTER(_vp)]),
     "stag_slab_cg_begin": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                           ctypes.c_int, ctypes.POINTER(_Params)]),

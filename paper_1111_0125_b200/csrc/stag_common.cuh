@@ -181,7 +181,13 @@ struct XchHeader {
     unsigned long long epoch;       // exchanges I have started (face_push_kernel increments it)
     unsigned long long red_seq;     // global sums I have published
     unsigned ticket;                // last-block ticket of my face_push_kernel
+    // watchdog of the acquire-waits: a wait that polls wait_limit times without seeing its flag gives
+    // up, sets timed_out and lets the kernel finish on stale data, so a missing or mis-ordered peer
+    // shows up as an error from the next host call instead of a GPU that spins for ever
+    unsigned timed_out;
+    unsigned long long wait_limit;  // polls (~1 us each); 0 = the default below
 };
+constexpr unsigned long long XCH_DEFAULT_WAIT_POLLS = 1ull << 23;     // roughly ten seconds
 static_assert(sizeof(XchHeader) <= XCH_RED, "exchange header must fit its slot");
 __host__ __device__ inline size_t xch_halo_offset(int s3, unsigned long long epoch, int dir)
 {

@@ -147,12 +147,18 @@ template <typename T> struct HaloArgs {
     unsigned n_push_blocks;   // blocks of this launch that own boundary-slice sites (they alone take the ticket)
 };
 
-__device__ __forceinline__ void wait_flag(const unsigned long long *f, unsigned long long epoch)
+// hdr: the header of the slab whose flag f belongs to (for the watchdog, stag_common.cuh)
+__device__ __forceinline__ void wait_flag(const unsigned long long *f, unsigned long long epoch, XchHeader *hdr)
 {
-    unsigned long long v;
-    do {
+    unsigned long long v, polls = 0;
+    unsigned long long limit = __ldcg(&hdr->wait_limit);
+    if (limit == 0) limit = XCH_DEFAULT_WAIT_POLLS;
+    for (;;) {
         asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(f) : "memory");
-    } while (v < epoch);
+        if (v >= epoch) return;
+        if (++polls >= limit) { hdr->timed_out = 1u; return; }
+        __nanosleep(200);
+    }
 }
 
 // T: float or double.  NR: storage of each link (3 = 18-real, 2 = 12-real rows 0,1, 1 = 8-parameter).
@@ -224,18 +230,18 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
             if constexpr (HALO) {
                 // decode_site wrapped the +-t neighbours of the boundary slices onto the slab's
                 // own other end; their in-slice index is what addresses the halo buffers
-                const XchHeader *hdr = (const XchHeader *)halo.xch;
+                XchHeader *hdr = (XchHeader *)halo.xch;
                 if (s.x3 == g.X3 - 1) {
                     const unsigned long long e = __ldcg(&hdr->epoch);
                     const C *fwd = (const C *)(halo.xch + xch_halo_offset(g.s3, e, 1));
-                    wait_flag(&hdr->flag_fwd, e);
+                    wait_flag(&hdr->flag_fwd, e, hdr);
 #pragma unroll
                     for (int c = 0; c < 3; ++c) v1[3][c] = __ldcg(fwd + (size_t)c * g.s3 + s.nbr[3]);
                 }
                 if (s.x3 == 0) {
                     const unsigned long long e = __ldcg(&hdr->epoch);
                     const C *back = (const C *)(halo.xch + xch_halo_offset(g.s3, e, 0));
-                    wait_flag(&hdr->flag_back, e);
+                    wait_flag(&hdr->flag_back, e, hdr);
 #pragma unroll
                     for (int c = 0; c < 3; ++c)
                         v1[7][c] = __ldcg(back + (size_t)c * g.s3 + (s.nbr[7] - (g.X3 - 1) * g.s3));

@@ -358,6 +358,7 @@ extern "C" const char *stag_strerror(int status)
     case STAG_EINVAL: return (t_errbuf_status == STAG_EINVAL) ? t_errbuf : "invalid argument";
     case STAG_ECUDA: return t_errbuf;
     case STAG_ENOMEM: return (t_errbuf_status == STAG_ENOMEM) ? t_errbuf : "out of memory";
+    case STAG_ETIMEOUT: return "a T-slab kernel gave up waiting for a neighbour's exchange or global sum";
     case STAG_ENOCONV: return "maxiter reached before the true residual met tol";
     case STAG_EBREAKDOWN: return "CG breakdown (NaN or <d,Ad> <= 0)";
     }

@@ -188,6 +188,23 @@ extern "C" int stag_slab_hop(void *out, const void *in, stag_links_t *L, int par
     return slab_hop_mode(L, prec, own ? HOP_XPAY : HOP_PLAIN, out, in, parity, a, own, nullptr, nullptr, t_stream);
 }
 
+extern "C" int stag_slab_set_wait_limit(stag_links_t *L, unsigned long long polls)
+{
+    if (!L || !L->is_slab) return STAG_EINVAL;
+    CU(cudaMemcpyAsync(&((XchHeader *)L->xch)->wait_limit, &polls, sizeof(polls), cudaMemcpyHostToDevice, t_stream));
+    CU(cudaStreamSynchronize(t_stream));
+    return STAG_OK;
+}
+
+extern "C" int stag_slab_status(stag_links_t *L)
+{
+    if (!L || !L->is_slab) return STAG_EINVAL;
+    unsigned flag = 0;
+    CU(cudaMemcpyAsync(&flag, &((XchHeader *)L->xch)->timed_out, sizeof(flag), cudaMemcpyDeviceToHost, t_stream));
+    CU(cudaStreamSynchronize(t_stream));
+    return flag ? STAG_ETIMEOUT : STAG_OK;
+}
+
 extern "C" int stag_slab_dslash(void *out, const void *in, stag_links_t *L, int parity, int prec)
 {
     int rc = stag_slab_push(in, L, prec);
@@ -371,6 +388,7 @@ extern "C" int stag_slab_cg_control(stag_links_t *L, int *action_out)
     if (C->stage == 3) { *action_out = STAG_SLAB_ACT_DONE; return STAG_OK; }
     CU(cudaMemcpyAsync(h, C->w.ctrl, sizeof(CgCtrl), cudaMemcpyDeviceToHost, t_stream));
     CU(cudaStreamSynchronize(t_stream));
+    { const int ws = stag_slab_status(L); if (ws != STAG_OK) return ws; }      // a wait gave up: nothing below is valid
     if (C->stage == 1) {                       // |b|^2 (global) has arrived
         C->bnorm2 = h->bnorm2[0];
         if (C->bnorm2 == 0.0) {                // b = 0  =>  x = 0, nothing to iterate
@@ -498,6 +516,7 @@ extern "C" int stag_slab_cg_finish(stag_links_t *L, stag_cg_stats_t *stats_out)
     CgCtrl *h = L->h_ctrl;
     CU(cudaEventRecord(L->ev1, t_stream));
     CU(cudaStreamSynchronize(t_stream));
+    { const int ws = stag_slab_status(L); if (ws != STAG_OK) return ws; }
     float ms = 0.f;
     CU(cudaEventElapsedTime(&ms, L->ev0, L->ev1));
     stag_cg_stats_t st;

@@ -144,12 +144,12 @@ __device__ __forceinline__ void publish_total(char *const *peers, int nranks, in
 }
 
 // Any thread: the sum over ranks of reduction seq, added in rank order (same bits on every rank).
-__device__ __forceinline__ double gather_total(const char *mine, int nranks, unsigned long long seq)
+__device__ __forceinline__ double gather_total(char *mine, int nranks, unsigned long long seq)
 {
     const XchReduce *R = (const XchReduce *)(mine + XCH_RED);
     double t = 0.0;
     for (int r = 0; r < nranks; ++r) {
-        wait_flag(&R->flag[r], seq);
+        wait_flag(&R->flag[r], seq, (XchHeader *)mine);
         t += __ldcg(&R->slot[seq & 1ull][r]);
     }
     return t;

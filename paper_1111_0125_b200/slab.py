@@ -210,6 +210,16 @@ class SlabLinks:
                 ph += 1
         return x, self.cg_finish()
 
+    def set_wait_limit(self, polls: int):
+        """Watchdog of the acquire-waits (stag_slab_set_wait_limit); 0 = the default (~10 s)."""
+        stag.use_current_stream()
+        stag._check(stag.lib().stag_slab_set_wait_limit(self._h, int(polls)))
+
+    def status(self) -> int:
+        """stag.OK, or stag.ETIMEOUT once a kernel of this slab gave up waiting for a peer."""
+        stag.use_current_stream()
+        return int(stag.lib().stag_slab_status(self._h))
+
     # -- the operator; spinors are device spinors of the LOCAL dims -------------------------
     def push(self, v, prec):
         stag.use_current_stream()

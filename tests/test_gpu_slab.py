@@ -233,3 +233,34 @@ def test_slab_hop_full_size_bitwise_against_whole_lattice(nranks):
     for s in slabs:
         s.close()
     L.close()
+
+
+def test_watchdog_turns_a_missing_push_into_an_error_instead_of_a_hang():
+    """Two slabs; only rank 0 pushes, then rank 0 hops: its boundary threads wait for flags rank 1
+    never sets.  With the wait limit lowered the kernel must give up, the slab must report
+    STAG_ETIMEOUT, and the interior of the result (which needs no neighbour) must still be right."""
+    dims = (4, 4, 4, 8)
+    W = fieldgen.links(dims, "random", seed=61)
+    slabs = make_slabs(dims, W, 2)
+    chi = fieldgen.spinor_gaussian(dims, 0, seed=62)
+    prec = stag.PREC_F64
+    v0 = stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(chi, dims, 0, 2)), slabs[0].dims, prec)
+    slabs[0].set_wait_limit(2000)                      # ~ a millisecond
+    assert slabs[0].status() == stag.OK
+    slabs[0].push(v0, prec)                            # rank 1 never pushes
+    out = stag.spinor_unpack(slabs[0].hop(v0, 1, prec), slabs[0].dims, prec)
+    assert slabs[0].status() == stag.ETIMEOUT
+    ref = slab.scatter_spinor(oracle.dslash(chi, W, dims, 1), dims, 0, 2)
+    s3 = slab.slice_sites(dims)
+    assert rel_l2(out[s3:-s3], ref[s3:-s3]) <= 1e-13   # slices 1 .. Tl-2 need no halo
+    # the CG entry points report it too
+    import torch
+    x = torch.zeros_like(v0)
+    slabs[0].cg_begin(x, v0, 0.1, 1e-10, 10, stag.CG_F64)
+    with pytest.raises(stag.StagError) as e:
+        slabs[0].cg_control()      # ACT_NORM needs no status read; the next control call does
+        ph = 0
+        while slabs[0].cg_step(slab.ACT_NORM, ph):
+            ph += 1
+        slabs[0].cg_control()
+    assert e.value.status == stag.ETIMEOUT
