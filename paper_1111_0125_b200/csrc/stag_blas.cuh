@@ -292,13 +292,4 @@ residual_kernel(double *__restrict__ r, const double *__restrict__ b,
     residual_epilogue<WHAT>(ctrl, totals);
 }
 
-// dst = (T) src, elementwise (precision change of a device spinor)
-template <typename TD, typename TS>
-__global__ void __launch_bounds__(BLAS_BLOCK)
-convert_kernel(TD *__restrict__ dst, const TS *__restrict__ src, long n)
-{
-    for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < n; i += (long)gridDim.x * BLAS_BLOCK)
-        dst[i] = (TD)src[i];
-}
-
 }  // namespace stag

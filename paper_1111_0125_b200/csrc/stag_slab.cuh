@@ -3,10 +3,12 @@
 // The paper's multi-GPU Dirac operation is kernel -> boundary collect -> memcpy to host -> MPI ->
 // memcpy to device (Table 1), and it plans peer-to-peer copies.  Here a
 // slab's two boundary time slices of the hop's INPUT spinor are stored straight into the
-// neighbouring GPUs' halo buffers by face_push_kernel (peer-to-peer stores over NVLink; the
-// buffers are ordinary device memory mapped into this process with CUDA IPC or, for slabs that
-// share a process, used directly), followed by one system-scope release store of the exchange's
-// epoch into each neighbour's flag.  The consuming hop (dslash_kernel<..., HALO = true>) waits on
+// neighbouring GPUs' halo buffers (peer-to-peer stores over NVLink; the buffers are ordinary device
+// memory mapped into this process with CUDA IPC or, for slabs that share a process, used directly)
+// by the kernel that PRODUCES that spinor -- slab_xpay_push_kernel for the direction d, the
+// boundary-slice threads of hop 1 for its output (stag_dslash.cuh) -- or, stand-alone, by
+// face_push_kernel; a system-scope release store of the exchange's number into each neighbour's
+// flag follows.  The consuming hop (dslash_kernel<..., HALO = true>) waits on
 // its own two flags only in the threads of the first and last time slice, which it visits last.
 //
 // The slab CG's global sums go through the same region: a rank stores its local total into slot
