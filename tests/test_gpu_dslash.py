@@ -234,3 +234,32 @@ def test_eight_parameter_form_refused_where_it_does_not_exist():
     L3 = stag.Links(dims, rng.normal(size=(4, 2, 128, 3, 3)) + 1j * rng.normal(size=(4, 2, 128, 3, 3)))
     with pytest.raises(stag.StagError):
         stag.dslash(stag.spinor_pack(chi, dims, stag.PREC_F64_R8), L3, 1, stag.PREC_F64_R8)
+
+
+def _random_cases(n, seed):
+    rng = np.random.default_rng(seed)
+    cases = []
+    while len(cases) < n:
+        dims = tuple(int(v) for v in rng.choice([2, 4, 6, 8, 10, 12], size=4))
+        if np.prod(dims) <= 6000:
+            cases.append((dims, int(rng.integers(0, 2)), bool(rng.integers(0, 2)), int(rng.integers(1, 10**6))))
+    return cases
+
+
+@pytest.mark.parametrize("dims,parity,antiperiodic,seed", _random_cases(24, 20111125))
+def test_hop_on_randomly_drawn_small_lattices(dims, parity, antiperiodic, seed):
+    """Two dozen lattices drawn from even extents 2..12 (fixed seed): every mixture of extents of 2
+    (coinciding neighbours), ragged volumes and boundary conditions, all storage forms, single and
+    batch entry, against the oracle."""
+    W = fieldgen.links(dims, "random", seed=seed, antiperiodic_t=antiperiodic)
+    L = stag.Links(dims, W, antiperiodic_t=antiperiodic)
+    chis = [fieldgen.spinor_gaussian(dims, 1 - parity, seed=seed + 1 + k) for k in range(3)]
+    refs = [oracle.dslash(c, W, dims, parity) for c in chis]
+    for prec in ALL_PREC + [stag.PREC_F64_R8, stag.PREC_F32_R8]:
+        tol = TOL.get(prec) or TOL8[prec]
+        out = stag.spinor_unpack(stag.dslash(stag.spinor_pack(chis[0], dims, prec), L, parity, prec), dims, prec)
+        assert rel_l2(out, refs[0]) <= tol, (prec, dims)
+        if prec in ALL_PREC:
+            outs = stag.dslash_mrhs(stag.spinor_pack_mrhs(chis, dims, prec), L, parity, prec)
+            for k, o in enumerate(stag.spinor_unpack_mrhs(outs, dims, prec)):
+                assert rel_l2(o, refs[k]) <= tol, (prec, dims, k)
