@@ -223,3 +223,31 @@ def test_mixed_cg_on_eight_parameter_links_still_meets_the_target():
     res = np.linalg.norm((b - oracle.apply_A(xs, W, cfg.dims, cfg.mass)).ravel()) / np.linalg.norm(b.ravel())
     assert res <= cfg.tol * (1 + 1e-3)
     assert np.linalg.norm((xs - x_ref).ravel()) / np.linalg.norm(x_ref.ravel()) <= 1e-8
+
+
+def _random_cg_cases(n, seed):
+    rng = np.random.default_rng(seed)
+    cases = []
+    while len(cases) < n:
+        dims = tuple(int(v) for v in rng.choice([2, 4, 6, 8], size=4))
+        if 64 <= np.prod(dims) <= 3000:
+            cases.append((dims, float(rng.choice([0.05, 0.1, 0.3])), str(rng.choice(["random", "smooth"])), int(rng.integers(1, 10**6))))
+    return cases
+
+
+@pytest.mark.parametrize("dims,mass,kind,seed", _random_cg_cases(10, 1111))
+def test_cg_on_randomly_drawn_small_lattices(dims, mass, kind, seed):
+    """Ten lattices / masses / link kinds drawn with a fixed seed: fp64 and mixed solves against
+    the oracle's solution (to 1e-12) and the oracle's A."""
+    W = fieldgen.links(dims, kind, seed=seed, eps=0.4)
+    b = fieldgen.spinor_gaussian(dims, 0, seed=seed + 1)
+    x_ref, _, _, _, rc = oracle.cg(b, W, dims, mass, 1e-12, 50000)
+    assert rc == 0
+    L = stag.Links(dims, W)
+    bd = stag.spinor_pack(b, dims, 0)
+    for mode, kw in ((stag.CG_F64, {}), (stag.CG_RELIABLE, {}), (stag.CG_RELIABLE, {"recon12": True}), (stag.CG_DEFECT, {})):
+        x, st = stag.cg_solve(bd, L, mass, 1e-10, 20000, mode, **kw)
+        xs = stag.spinor_unpack(x, dims, 0)
+        assert st["status"] == stag.OK and st["true_resid"] <= 1e-10, (mode, st)
+        assert oracle_true_resid(xs, b, W, dims, mass) <= 1e-10 * (1 + 1e-3)
+        assert rel_l2(xs, x_ref) <= 1e-8

@@ -264,3 +264,36 @@ def test_watchdog_turns_a_missing_push_into_an_error_instead_of_a_hang():
             ph += 1
         slabs[0].cg_control()
     assert e.value.status == stag.ETIMEOUT
+
+
+def _random_slab_cases(n, seed):
+    rng = np.random.default_rng(seed)
+    cases = []
+    while len(cases) < n:
+        dims = tuple(int(v) for v in rng.choice([2, 4, 6], size=3)) + (int(rng.choice([4, 8, 12, 16, 24])),)
+        nranks = int(rng.choice([r for r in (1, 2, 3, 4, 6) if dims[3] % r == 0 and (dims[3] // r) % 2 == 0]))
+        if np.prod(dims) <= 5000:
+            cases.append((dims, nranks, int(rng.integers(1, 10**6))))
+    return cases
+
+
+@pytest.mark.parametrize("dims,nranks,seed", _random_slab_cases(12, 2011))
+def test_slab_hop_and_cg_on_randomly_drawn_decompositions(dims, nranks, seed):
+    """A dozen lattices and slab counts drawn with a fixed seed: both hops bitwise against the
+    whole-lattice kernel, and the mixed slab CG against the oracle's A."""
+    W = fieldgen.links(dims, "random", seed=seed)
+    L = stag.Links(dims, W)
+    slabs = make_slabs(dims, W, nranks)
+    for parity in (0, 1):
+        chi = fieldgen.spinor_gaussian(dims, 1 - parity, seed=seed + parity)
+        for prec in (stag.PREC_F64, stag.PREC_F32_R12):
+            _, got = slab_hop_all(slabs, chi, dims, parity, prec)
+            whole = stag.spinor_unpack(stag.dslash(stag.spinor_pack(chi, dims, prec), L, parity, prec), dims, prec)
+            assert np.array_equal(got, whole)
+    b = fieldgen.spinor_gaussian(dims, 0, seed=seed + 7)
+    bs = [stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(b, dims, r, nranks)), slabs[r].dims, 0) for r in range(nranks)]
+    xs, sts = slab.cg_solve_in_process(slabs, bs, 0.2, 1e-10, 5000, stag.CG_RELIABLE, recon12=True)
+    x = slab.gather_spinor([stag.spinor_unpack(xs[r], slabs[r].dims, 0) for r in range(nranks)], dims)
+    assert all(st["status"] == stag.OK for st in sts)
+    res = np.linalg.norm((b - oracle.apply_A(x, W, dims, 0.2)).ravel()) / np.linalg.norm(b.ravel())
+    assert res <= 1e-10 * (1 + 1e-3)
