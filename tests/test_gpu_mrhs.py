@@ -200,3 +200,37 @@ def test_mrhs_full_size_hop_matches_oracle():
         outs = stag.dslash_mrhs(stag.spinor_pack_mrhs(chis, cfg.dims, prec), L, 1, prec)
         for k, o in enumerate(stag.spinor_unpack_mrhs(outs, cfg.dims, prec)):
             assert rel_l2(o, refs[k]) <= TOL[prec]
+
+
+@pytest.mark.slow
+def test_batched_solve_and_propagator_full_size_with_oracle_operators():
+    """bench configuration (28^3 x 96): three sources in lockstep (mode 3, 12-real fp32 links), each
+    solution checked through the ORACLE's A; then the propagator wrapper for a point source in the
+    three colours, checked through the oracle's M = D + m on the whole lattice."""
+    cfg = fieldgen.CONFIGS["c4_28^3x96"]
+    W = cfg.links()
+    L = stag.Links(cfg.dims, W)
+    bs = [fieldgen.spinor_gaussian(cfg.dims, 0, seed=500 + k) for k in range(3)]
+    xs, sts = stag.cg_solve_mrhs(stag.spinor_pack_mrhs(bs, cfg.dims, 0), L, cfg.mass, cfg.tol, cfg.maxiter,
+                                 stag.CG_RELIABLE, recon12=True)
+    for k, x in enumerate(stag.spinor_unpack_mrhs(xs, cfg.dims, 0)):
+        assert sts[k]["status"] == stag.OK and sts[k]["true_resid"] <= cfg.tol
+        res = np.linalg.norm((bs[k] - oracle.apply_A(x, W, cfg.dims, cfg.mass)).ravel()) / np.linalg.norm(bs[k].ravel())
+        assert res <= cfg.tol * (1 + 1e-3), (k, res)
+    del xs
+    hs = []
+    for c in range(3):
+        h = np.zeros((2, cfg.vh, 3), dtype=np.complex128)
+        h[1, 12345, c] = 1.0
+        hs.append(h)
+    he = stag.spinor_pack_mrhs([np.ascontiguousarray(h[0]) for h in hs], cfg.dims, 0)
+    ho = stag.spinor_pack_mrhs([np.ascontiguousarray(h[1]) for h in hs], cfg.dims, 0)
+    pe, po, sts = stag.solve_M(he, ho, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True)
+    pe, po = stag.spinor_unpack_mrhs(pe, cfg.dims, 0), stag.spinor_unpack_mrhs(po, cfg.dims, 0)
+    for c in range(3):
+        assert sts[c]["status"] == stag.OK
+        psi = np.ascontiguousarray(np.stack([pe[c], po[c]]))
+        b_e = cfg.mass * hs[c][0] - oracle.dslash(np.ascontiguousarray(hs[c][1]), W, cfg.dims, 0)
+        res = rel_l2(oracle.apply_M(psi, W, cfg.dims, cfg.mass), hs[c])
+        assert res <= cfg.tol * np.linalg.norm(b_e) / (cfg.mass * np.linalg.norm(hs[c])) * (1 + 1e-3), (c, res)
+    L.close()
