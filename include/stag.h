@@ -35,11 +35,21 @@
  *
  * Pointers: every `void *` / `const void *` spinor argument is DEVICE memory
  * in the device layout unless the name ends in `_host`.  The caller owns all
- * spinor buffers; the library owns only what hangs off a stag_links_t.
+ * spinor buffers and, once it has called stag_set_workspace(), the solver's
+ * workspace; the library owns only what hangs off a stag_links_t.
  * All calls are asynchronous on the stream set by stag_set_stream() except
  * where stated.  No call throws or aborts; every `int` return is a
  * stag_status (0 = OK, < 0 = failure, > 0 = solver outcome that still wrote
  * its results).
+ *
+ * Threads: the stream, the workspace and the error text are PER HOST THREAD.
+ * A `const stag_links_t *` is immutable to its callers: any number of host
+ * threads, each with its own stream and its own workspace, may apply the
+ * operator and solve on one handle at the same time (the production pattern:
+ * many sources per gauge field).  A thread that has set no workspace
+ * uses one owned by the handle, under the handle's mutex: such calls are safe
+ * from any thread but run one after the other.  Slab handles (stag_slab_*) are
+ * not const and belong to one host thread.
  */
 #ifndef STAG_H
 #define STAG_H
@@ -97,6 +107,32 @@ typedef struct stag_links stag_links_t;
 /* Stream (a cudaStream_t cast to void*) every later call enqueues on; NULL = the legacy
  * default stream.  Per host thread. */
 int stag_set_stream(void *cuda_stream);
+
+/* ---- workspace ("the caller owns every spinor buffer and the
+ * workspace") ----------------------------------------------------------------------------
+ *
+ * What lives there: Fig. 1's vectors other than x and b -- r, d and q = A d and the
+ * odd-site intermediate of A (eq. 2.3) in fp64 -- the fp32 iteration's y, r, d, q, tmp of the
+ * mixed modes (section 3.2), the device-resident scalars alpha, beta, delta, the
+ * partial sums of the inner products, b_e of stag_solve_M and the two device-layout
+ * spinors stag_cg_solve_host stages x and b in.
+ *
+ * stag_cg_workspace_bytes: bytes a workspace needs for any of stag_cg_solve*, stag_solve_M,
+ * stag_cg_solve_host, stag_apply_A* on a lattice `dims` in CG mode `mode` with up to `nrhs`
+ * right-hand sides (mode < 0: only stag_apply_A*).  Pure arithmetic, no device needed; 0 on bad
+ * arguments.  A workspace sized for (mode, nrhs) also serves fewer right-hand sides; sizes for
+ * different modes differ, take the largest of the modes you use.
+ *
+ * stag_set_workspace: from now on THIS host thread's calls keep every intermediate in
+ * ws[0 .. bytes) (device memory, 256-byte aligned, caller-owned, must stay valid until replaced)
+ * and write nothing to the link handle.  A call that needs more than `bytes` fails with
+ * STAG_EINVAL (stag_strerror says how much).  Calls sharing a workspace must be issued from the
+ * thread that set it; they are ordered on the device even if that thread changes its stream in
+ * between.  The instantiated CUDA graph of the iteration is cached with the workspace per
+ * (handle, mode, link form, nrhs, chunk, mass), so repeated solves do not re-capture.
+ * ws = NULL, bytes = 0 returns to the handle-owned default.  Not asynchronous; no device work. */
+size_t stag_cg_workspace_bytes(const int dims[4], int mode, int nrhs);
+int stag_set_workspace(void *ws, size_t bytes);
 
 /* Text for a status; for STAG_ECUDA, the text of the last CUDA error seen by this thread.
  * The pointer stays valid until the next failing call on this thread. */
@@ -163,7 +199,7 @@ int stag_dslash(void *out, const void *in, const stag_links_t *links, int parity
 
 /* A = -D^2 + m^2 on the even sites (eq. 2.3):
  *   out_even = mass^2 * in_even - D_eo ( D_oe in_even ).
- * The odd-parity intermediate lives in scratch owned by the handle.  out must not alias in. */
+ * The odd-parity intermediate lives in the workspace.  out must not alias in. */
 int stag_apply_A(void *out_even, const void *in_even, const stag_links_t *links, double mass,
                  int prec);
 
@@ -261,7 +297,8 @@ typedef struct stag_cg_stats {
  * the initial guess on entry and the solution on exit; b is fp64 device layout.  Convergence:
  * |r| <= tol * |b| (Q6), checked on the fp64 true residual before returning.  Synchronises
  * the stream before returning iterations and true residual.  b = 0 gives x = 0, 0 iterations,
- * residual 0.  Returns STAG_OK, STAG_ENOCONV, STAG_EBREAKDOWN or an error < 0. */
+ * residual 0.  Pad lanes of x are zeroed on entry, pad lanes of b are read as zero whatever
+ * they hold.  Returns STAG_OK, STAG_ENOCONV, STAG_EBREAKDOWN or an error < 0. */
 int stag_cg_solve(void *x_even, const void *b_even, const stag_links_t *links, double mass,
                   double tol, int maxiter, int mode, int *iters_out, double *true_resid_out);
 

@@ -92,6 +92,8 @@ _vp, _ip, _dp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ct
 SIGNATURES = {
     "stag_set_stream": (ctypes.c_int, [_vp]),
     "stag_strerror": (ctypes.c_char_p, [ctypes.c_int]),
+    "stag_cg_workspace_bytes": (ctypes.c_size_t, [_ip, ctypes.c_int, ctypes.c_int]),
+    "stag_set_workspace": (ctypes.c_int, [_vp, ctypes.c_size_t]),
     "stag_launch_count": (ctypes.c_ulonglong, []),
     "stag_reset_launch_count": (None, []),
     "stag_links_create": (ctypes.c_int, [ctypes.POINTER(_vp), _ip, ctypes.c_int, _vp, ctypes.c_int]),
@@ -185,6 +187,24 @@ def use_current_stream():
     """Point the library at torch's current CUDA stream."""
     torch = _require_cuda()
     _check(lib().stag_set_stream(ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)))
+
+
+def cg_workspace_bytes(dims, mode: int, nrhs: int = 1) -> int:
+    """stag_cg_workspace_bytes: pure arithmetic, works without a device."""
+    return int(lib().stag_cg_workspace_bytes(_cdims(dims), int(mode), int(nrhs)))
+
+
+def set_workspace(ws=None):
+    """stag_set_workspace for the calling host thread.  ws: a CUDA uint8 tensor the caller keeps
+    alive (e.g. torch.empty(cg_workspace_bytes(...), dtype=torch.uint8, device="cuda")), or None
+    to return to the handle-owned default."""
+    if ws is None:
+        _check(lib().stag_set_workspace(None, 0))
+        return
+    _require_cuda()
+    if not ws.is_cuda or not ws.is_contiguous():
+        raise ValueError("the workspace must be a contiguous CUDA tensor")
+    _check(lib().stag_set_workspace(ctypes.c_void_p(ws.data_ptr()), ws.numel() * ws.element_size()))
 
 
 def launch_count() -> int:

@@ -218,6 +218,18 @@ accumulate_kernel(double *__restrict__ x, T *__restrict__ y, long n)
     }
 }
 
+// Zero the pad lanes cb in [Vh, Vh_pad) of the three colour planes of spinor blockIdx.y of a batch.
+template <typename C>
+__global__ void zero_pads_kernel(C *__restrict__ v, int Vh, int Vh_pad)
+{
+    C *vk = v + (size_t)blockIdx.y * 3 * Vh_pad;
+    const int npad = Vh_pad - Vh;
+    for (int i = threadIdx.x; i < 3 * npad; i += blockDim.x) {
+        C z; z.x = 0; z.y = 0;
+        vk[(size_t)(i / npad) * Vh_pad + Vh + i % npad] = z;
+    }
+}
+
 enum { RES_INIT = 0, RES_UPDATE = 1, RES_FINAL = 2, RES_NORM = 3 };
 
 // Scalar part of residual_kernel (see there), given totals[k] = |r_k|^2 (or |b_k|^2).  One thread.
@@ -264,20 +276,24 @@ __device__ __forceinline__ void residual_epilogue(CgCtrl *__restrict__ ctrl, con
 //   RES_UPDATE after x += y (eq. 3.1): beta = |r|^2 / delta_old, delta = |r|^2;
 //              an active k whose true residual meets the target is frozen
 //   RES_FINAL  exit: only report |r|^2
+// b is the caller's and read-only: its pad lanes (reals [n_valid, n_plane) of each colour plane,
+// n_plane = 2 Vh_pad, n_valid = 2 Vh) are taken as zero whatever they hold, so no stray value can
+// enter |b|^2, |r|^2 or the stopping tests.
 template <typename T, int WHAT>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 residual_kernel(double *__restrict__ r, const double *__restrict__ b,
-                const double *__restrict__ q, T *__restrict__ r_lo, long n,
+                const double *__restrict__ q, T *__restrict__ r_lo, long n, long n_plane, long n_valid,
                 double *__restrict__ partials, CgCtrl *__restrict__ ctrl)
 {
     const size_t off = (size_t)blockIdx.y * n;
     double s = 0.0;
     for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < n; i += (long)gridDim.x * BLAS_BLOCK) {
+        const double bi = (n_valid == n_plane || i % n_plane < n_valid) ? b[off + i] : 0.0;
         if (WHAT == RES_NORM) {
-            const double v = b[off + i];
+            const double v = bi;
             s += v * v;
         } else {
-            const double v = b[off + i] - q[off + i];
+            const double v = bi - q[off + i];
             r[off + i] = v;
             if (r_lo != nullptr) r_lo[off + i] = (T)v;
             s += v * v;

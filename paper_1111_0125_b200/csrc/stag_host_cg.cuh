@@ -9,52 +9,9 @@
 // ------------------------------------------------------------------------------------
 namespace {
 
-struct Workspace {
-    CgCtrl *ctrl;
-    double *partials;       // block partials of the vector kernels' reductions, [rhs][block]
-    double *hop_partials;   // block partials of <d,Ad> written by the second hop, [rhs][block]
-    int n_hop;              // = grid of the hop
-    double *r64, *q64, *tmp64, *d64;          // nrhs spinors each
-    float *y32, *r32, *d32, *q32, *tmp32;
-};
-
-// One allocation on the handle, sized for nrhs right-hand sides (grown when a later solve
-// carries more).  Right-hand side k of every vector starts k*n reals in (n = 6*Vh_pad).
-int ensure_workspace(stag_links *L, Workspace &w, int nrhs)
-{
-    const size_t n = (size_t)6 * L->g.Vh_pad;
-    if (L->ws && L->ws_rhs < nrhs) { CU(cudaFree(L->ws)); L->ws = nullptr; }
-    const int cap = L->ws ? L->ws_rhs : nrhs;
-    const size_t nb64 = align_up(cap * n * sizeof(double), 256), nb32 = align_up(cap * n * sizeof(float), 256);
-    const size_t n_hop = ((size_t)L->g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK;
-    const size_t pb = align_up((size_t)MAX_RHS * blas_full_grid() * sizeof(double), 256);
-    const size_t hb = align_up((size_t)cap * n_hop * sizeof(double), 256);
-    const size_t total = CTRL_SLOT + pb + hb + 4 * nb64 + 5 * nb32;
-    if (!L->ws) {
-        CU(cudaMalloc((void **)&L->ws, total));
-        L->ws_bytes = total;
-        L->ws_rhs = cap;
-    }
-    if (!L->h_ctrl) CU(cudaMallocHost((void **)&L->h_ctrl, sizeof(CgCtrl)));
-    char *p = L->ws;
-    w.ctrl = (CgCtrl *)p; p += CTRL_SLOT;
-    w.partials = (double *)p; p += pb;
-    w.hop_partials = (double *)p; p += hb;
-    w.n_hop = (int)n_hop;
-    w.r64 = (double *)p; p += nb64;
-    w.q64 = (double *)p; p += nb64;
-    w.tmp64 = (double *)p; p += nb64;
-    w.d64 = (double *)p; p += nb64;
-    w.y32 = (float *)p; p += nb32;
-    w.r32 = (float *)p; p += nb32;
-    w.d32 = (float *)p; p += nb32;
-    w.q32 = (float *)p; p += nb32;
-    w.tmp32 = (float *)p; p += nb32;
-    return STAG_OK;
-}
-
 struct Solver {
-    stag_links *L;
+    const stag_links *L;
+    WsHost *ws;
     Workspace w;
     cudaStream_t s;
     double m2;
@@ -80,7 +37,7 @@ struct Solver {
     template <int WHAT>
     int residual(const double *b, bool lo_copy)
     {
-        residual_kernel<float, WHAT><<<grid2(), BLAS_BLOCK, 0, s>>>(w.r64, b, w.q64, lo_copy ? w.r32 : nullptr, n, w.partials, w.ctrl);
+        residual_kernel<float, WHAT><<<grid2(), BLAS_BLOCK, 0, s>>>(w.r64, b, w.q64, lo_copy ? w.r32 : nullptr, n, 2L * L->g.Vh_pad, 2L * L->g.Vh, w.partials, w.ctrl);
         count_launch();
         KCHECK();
         return STAG_OK;
@@ -120,7 +77,7 @@ struct Solver {
 
     int read_ctrl()
     {
-        CU(cudaMemcpyAsync(L->h_ctrl, w.ctrl, sizeof(CgCtrl), cudaMemcpyDeviceToHost, s));
+        CU(cudaMemcpyAsync(ws->h_ctrl, w.ctrl, sizeof(CgCtrl), cudaMemcpyDeviceToHost, s));
         CU(cudaStreamSynchronize(s));
         return STAG_OK;
     }
@@ -128,8 +85,9 @@ struct Solver {
 
 // nrhs right-hand sides in lockstep.  x, b: nrhs fp64 device spinors
 // back to back.  stats: nrhs entries, or null.
-int cg_solve_device(double *x, const double *b, stag_links *L, double mass, double tol, int maxiter,
-                    int mode, int nrhs, const stag_cg_params_t *prm, stag_cg_stats_t *stats)
+// ws: the leased workspace (at least ws_layout(g, mode, nrhs).total bytes).
+int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws, double mass, double tol,
+                    int maxiter, int mode, int nrhs, const stag_cg_params_t *prm, stag_cg_stats_t *stats)
 {
     stag_cg_params_t P;
     memset(&P, 0, sizeof(P));
@@ -139,6 +97,7 @@ int cg_solve_device(double *x, const double *b, stag_links *L, double mass, doub
 
     Solver S;
     S.L = L;
+    S.ws = ws;
     S.s = t_stream;
     S.m2 = mass * mass;
     S.mode = mode;
@@ -152,23 +111,32 @@ int cg_solve_device(double *x, const double *b, stag_links *L, double mass, doub
     int rc;
     if ((rc = ensure_links(L, S.prec_lo))) return rc;
     if ((rc = ensure_links(L, S.prec_hi))) return rc;
-    if ((rc = ensure_workspace(L, S.w, nrhs))) return rc;
+    carve(ws->base, ws_layout(L->g, mode, nrhs), S.w);
     Workspace &w = S.w;
     cudaStream_t s = S.s;
     const bool lo = (mode != STAG_CG_F64);
     const size_t vec_bytes = (size_t)S.n * sizeof(double);
 
-    CU(cudaEventRecord(L->ev0, s));
+    CU(cudaEventRecord(ws->ev0, s));
+
+    // Pad lanes (Vh not a multiple of 32) must be zero in every vector that enters a reduction:
+    // x is the caller's to overwrite, so its pads are zeroed here; b is read-only, its pads are
+    // masked where b is read (residual_kernel).
+    if (L->g.Vh_pad != L->g.Vh) {
+        zero_pads_kernel<<<dim3(1, (unsigned)nrhs), 128, 0, s>>>((double2 *)x, L->g.Vh, L->g.Vh_pad);
+        count_launch();
+        KCHECK();
+    }
 
     // ---- |b_k|^2 and the solver scalars ---------------------------------------------------
-    CgCtrl *h = L->h_ctrl;
+    CgCtrl *h = ws->h_ctrl;
     memset(h, 0, sizeof(*h));
     h->mode = mode;
     h->maxiter = maxiter;
     h->eps_in = P.eps_in;
     h->nrhs = nrhs;
     CU(cudaMemcpyAsync(w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, s));
-    residual_kernel<float, RES_NORM><<<S.grid2(), BLAS_BLOCK, 0, s>>>(nullptr, b, nullptr, nullptr, S.n, w.partials, w.ctrl);
+    residual_kernel<float, RES_NORM><<<S.grid2(), BLAS_BLOCK, 0, s>>>(nullptr, b, nullptr, nullptr, S.n, 2L * L->g.Vh_pad, 2L * L->g.Vh, w.partials, w.ctrl);
     count_launch();
     KCHECK();
     if ((rc = S.read_ctrl())) return rc;
@@ -190,7 +158,7 @@ int cg_solve_device(double *x, const double *b, stag_links *L, double mass, doub
     for (int k = 0; k < nrhs; ++k)
         if (bnorm2[k] == 0.0) CU(cudaMemsetAsync(x + (size_t)k * S.n, 0, vec_bytes, s));
     if (all_zero) {
-        CU(cudaEventRecord(L->ev1, s));
+        CU(cudaEventRecord(ws->ev1, s));
         CU(cudaStreamSynchronize(s));
         for (int k = 0; stats && k < nrhs; ++k) stats[k] = zero;
         return STAG_OK;
@@ -205,27 +173,44 @@ int cg_solve_device(double *x, const double *b, stag_links *L, double mass, doub
     // beta = 0 makes the first xpay d = r without reading d, so d needs no initial value
 
     // ---- the iteration as a CUDA graph of `chunk` passes ----------------------------------
+    // Instantiated once per (handle, mode, link form, nrhs, chunk, mass[, x]) and kept with the
+    // workspace: everything else the nodes bake in (vector addresses, control block) is a
+    // function of the workspace's base address and those.
     const int chunk = P.graph_chunk;
     cudaGraphExec_t gexec = nullptr;
     unsigned long long graph_nodes = 0;
     if (chunk > 0) {
-        cudaGraph_t graph = nullptr;
-        cudaError_t e = cudaStreamBeginCapture(L->cap_stream, cudaStreamCaptureModeThreadLocal);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaStreamBeginCapture", __LINE__);
-        t_capturing = true;
-        t_captured_nodes = 0;
-        rc = STAG_OK;
-        for (int i = 0; i < chunk && rc == STAG_OK; ++i) rc = S.iteration_mode(x, L->cap_stream);
-        t_capturing = false;
-        graph_nodes = t_captured_nodes;
-        e = cudaStreamEndCapture(L->cap_stream, &graph);
-        if (rc != STAG_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
-        if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture", __LINE__);
-        e = cudaGraphInstantiate(&gexec, graph, 0);
-        cudaGraphDestroy(graph);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaGraphInstantiate", __LINE__);
+        const void *xkey = (mode == STAG_CG_F64) ? (const void *)x : nullptr;
+        GraphSlot *slot = nullptr, *victim = &ws->graphs[0];
+        for (GraphSlot &gs : ws->graphs) {
+            if (gs.exec && gs.uid == L->uid && gs.mode == mode && gs.prec_lo == S.prec_lo && gs.nrhs == nrhs &&
+                gs.chunk == chunk && gs.m2 == S.m2 && gs.x == xkey) { slot = &gs; break; }
+            if (!gs.exec || (victim->exec && gs.stamp < victim->stamp)) victim = &gs;
+        }
+        if (!slot) {
+            cudaGraph_t graph = nullptr;
+            cudaError_t e = cudaStreamBeginCapture(ws->cap_stream, cudaStreamCaptureModeThreadLocal);
+            if (e != cudaSuccess) return cuda_fail(e, "cudaStreamBeginCapture", __LINE__);
+            t_capturing = true;
+            t_captured_nodes = 0;
+            rc = STAG_OK;
+            for (int i = 0; i < chunk && rc == STAG_OK; ++i) rc = S.iteration_mode(x, ws->cap_stream);
+            t_capturing = false;
+            e = cudaStreamEndCapture(ws->cap_stream, &graph);
+            if (rc != STAG_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+            if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture", __LINE__);
+            cudaGraphExec_t ge = nullptr;
+            e = cudaGraphInstantiate(&ge, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) return cuda_fail(e, "cudaGraphInstantiate", __LINE__);
+            if (victim->exec) cudaGraphExecDestroy(victim->exec);
+            *victim = GraphSlot{L->uid, mode, S.prec_lo, nrhs, chunk, S.m2, xkey, ge, t_captured_nodes, 0};
+            slot = victim;
+        }
+        slot->stamp = ++ws->stamp;
+        gexec = slot->exec;
+        graph_nodes = slot->nodes;
     }
-    struct GraphGuard { cudaGraphExec_t g; ~GraphGuard() { if (g) cudaGraphExecDestroy(g); } } guard{gexec};
 
     int n_restarts = 0, n_outer = 0;
     int final_state = CG_RUN;
@@ -290,10 +275,10 @@ int cg_solve_device(double *x, const double *b, stag_links *L, double mass, doub
         }
         break;
     }
-    CU(cudaEventRecord(L->ev1, s));
+    CU(cudaEventRecord(ws->ev1, s));
     CU(cudaStreamSynchronize(s));
     float ms = 0.f;
-    CU(cudaEventElapsedTime(&ms, L->ev0, L->ev1));
+    CU(cudaEventElapsedTime(&ms, ws->ev0, ws->ev1));
 
     bool all_met = true;
     for (int k = 0; k < nrhs; ++k) {
@@ -316,15 +301,17 @@ int cg_solve_device(double *x, const double *b, stag_links *L, double mass, doub
 
 }  // namespace
 
-extern "C" int stag_cg_solve_mrhs(void *x_even, const void *b_even, const stag_links_t *links,
+extern "C" int stag_cg_solve_mrhs(void *x_even, const void *b_even, const stag_links_t *L,
                                   double mass, double tol, int maxiter, int mode, int nrhs,
                                   const stag_cg_params_t *params, stag_cg_stats_t *stats_out)
 {
-    stag_links *L = const_cast<stag_links *>(links);
     if (!x_even || !b_even || !L || x_even == b_even || !(tol > 0.0) || maxiter < 0 || mode < 0 ||
         mode > 3 || nrhs < 1 || nrhs > MAX_RHS || L->is_slab)
         return STAG_EINVAL;
-    return cg_solve_device((double *)x_even, (const double *)b_even, L, mass, tol, maxiter, mode,
+    WsLease lease;
+    int rc = lease_workspace(L, ws_layout(L->g, mode, nrhs).total, lease);
+    if (rc) return rc;
+    return cg_solve_device((double *)x_even, (const double *)b_even, L, lease.ws, mass, tol, maxiter, mode,
                            nrhs, params, stats_out);
 }
 
@@ -348,22 +335,29 @@ extern "C" int stag_cg_solve(void *x_even, const void *b_even, const stag_links_
     return rc;
 }
 
-extern "C" int stag_cg_solve_host(double *x_host, const double *b_host, const stag_links_t *links,
+// The canonical copies of b and x0 pass through the workspace's r64 / q64 (dead until the solve
+// starts, and again once it has finished); x and b in the device layout have their own two slots.
+extern "C" int stag_cg_solve_host(double *x_host, const double *b_host, const stag_links_t *L,
                                   double mass, double tol, int maxiter, int mode,
                                   const stag_cg_params_t *params, stag_cg_stats_t *stats_out)
 {
-    stag_links *L = const_cast<stag_links *>(links);
-    if (!x_host || !b_host || !L || x_host == b_host) return STAG_EINVAL;
+    if (!x_host || !b_host || !L || x_host == b_host || !(tol > 0.0) || maxiter < 0 || mode < 0 ||
+        mode > 3 || L->is_slab)
+        return STAG_EINVAL;
     const size_t nc = (size_t)L->g.Vh * 6;         // canonical doubles
     const size_t nd = (size_t)L->g.Vh_pad * 6;     // device-layout doubles
-    if (!L->stage_dev) CU(cudaMalloc((void **)&L->stage_dev, (2 * nc + 2 * nd) * sizeof(double)));
-    double *cx = L->stage_dev, *cb = cx + nc, *dx = cb + nc, *db = dx + nd;
+    const WsLayout lay = ws_layout(L->g, mode, 1);
+    WsLease lease;
+    int rc = lease_workspace(L, lay.total, lease);
+    if (rc) return rc;
+    Workspace w;
+    carve(lease.ws->base, lay, w);
+    double *cb = w.r64, *cx = w.q64, *dx = w.stage, *db = w.stage + nd;
     CU(cudaMemcpyAsync(cb, b_host, nc * sizeof(double), cudaMemcpyHostToDevice, t_stream));
     CU(cudaMemcpyAsync(cx, x_host, nc * sizeof(double), cudaMemcpyHostToDevice, t_stream));
-    int rc;
     if ((rc = stag_spinor_pack(db, cb, L->dims, STAG_PREC_F64))) return rc;
     if ((rc = stag_spinor_pack(dx, cx, L->dims, STAG_PREC_F64))) return rc;
-    const int solve_rc = stag_cg_solve_ex(dx, db, L, mass, tol, maxiter, mode, params, stats_out);
+    const int solve_rc = cg_solve_device(dx, db, L, lease.ws, mass, tol, maxiter, mode, 1, params, stats_out);
     if (solve_rc < 0) return solve_rc;
     if ((rc = stag_spinor_unpack(cx, dx, L->dims, STAG_PREC_F64))) return rc;
     CU(cudaMemcpyAsync(x_host, cx, nc * sizeof(double), cudaMemcpyDeviceToHost, t_stream));
@@ -373,30 +367,35 @@ extern "C" int stag_cg_solve_host(double *x_host, const double *b_host, const st
 
 // (D + m) psi = h on the whole lattice through the even-site solve (Q23):
 //   b_e = m h_e - D_eo h_o ;  A psi_e = b_e ;  psi_o = (h_o - D_oe psi_e) / m
-// The two extra hops run in fp64 on the 18-real links; b_e lives in scratch on the handle.
+// The two extra hops run in fp64 on the 18-real links; b_e lives in the workspace.
 extern "C" int stag_solve_M(void *psi_even, void *psi_odd, const void *h_even, const void *h_odd,
-                            const stag_links_t *links, double mass, double tol, int maxiter,
+                            const stag_links_t *L, double mass, double tol, int maxiter,
                             int mode, int nrhs, const stag_cg_params_t *params,
                             stag_cg_stats_t *stats_out)
 {
-    stag_links *L = const_cast<stag_links *>(links);
     if (!psi_even || !psi_odd || !h_even || !h_odd || !L || psi_even == h_even ||
         psi_odd == h_odd || !(tol > 0.0) || maxiter < 0 || mode < 0 || mode > 3 || nrhs < 1 ||
         nrhs > MAX_RHS || mass == 0.0 || L->is_slab)
         return STAG_EINVAL;
     int rc;
     if ((rc = ensure_links(L, STAG_PREC_F64))) return rc;
-    const size_t bytes = (size_t)nrhs * 6 * L->g.Vh_pad * sizeof(double);
-    if (L->wrap_b && L->wrap_b_rhs < nrhs) { CU(cudaFree(L->wrap_b)); L->wrap_b = nullptr; }
-    if (!L->wrap_b) { CU(cudaMalloc(&L->wrap_b, bytes)); L->wrap_b_rhs = nrhs; }
+    const WsLayout lay = ws_layout(L->g, mode, nrhs);
+    WsLease lease;
+    if ((rc = lease_workspace(L, lay.total, lease))) return rc;
+    Workspace w;
+    carve(lease.ws->base, lay, w);
     // step 1: b_e = m h_e - D_eo h_o
-    if ((rc = launch_hop(L, STAG_PREC_F64, HOP_XPAY, L->wrap_b, h_odd, 0, mass, 1.0, h_even, nullptr, nullptr, nrhs, t_stream))) return rc;
+    if ((rc = launch_hop(L, STAG_PREC_F64, HOP_XPAY, w.wrap_b, h_odd, 0, mass, 1.0, h_even, nullptr, nullptr, nrhs, t_stream))) return rc;
     // step 2: A psi_e = b_e (psi_even holds the initial guess on entry)
-    const int solve_rc = cg_solve_device((double *)psi_even, (const double *)L->wrap_b, L, mass, tol,
+    const int solve_rc = cg_solve_device((double *)psi_even, w.wrap_b, L, lease.ws, mass, tol,
                                          maxiter, mode, nrhs, params, stats_out);
     if (solve_rc < 0) return solve_rc;
     // step 3: psi_o = (1/m) h_o - (1/m) D_oe psi_e
     if ((rc = launch_hop(L, STAG_PREC_F64, HOP_AXPBY, psi_odd, psi_even, 1, 1.0 / mass, 1.0 / mass, h_odd, nullptr, nullptr, nrhs, t_stream))) return rc;
+    if (L->g.Vh_pad != L->g.Vh) {       // psi_o's pad lanes hold h_o's / m: zero them (every output keeps zero pads)
+        zero_pads_kernel<<<dim3(1, (unsigned)nrhs), 128, 0, t_stream>>>((double2 *)psi_odd, L->g.Vh, L->g.Vh_pad);
+        count_launch();
+        KCHECK();
+    }
     return solve_rc;
 }
-

@@ -177,10 +177,23 @@ spinor_unpack_kernel(double *__restrict__ dst, const cplx_t<T> *__restrict__ src
     }
 }
 
-// Build (once) the gathered field of precision `prec` from the fp64/18 one.
-int ensure_links(stag_links *L, int prec)
+// Build (once) the gathered field of precision `prec` from the fp64/18 one.  Thread-safe: the
+// first caller builds under the handle's mutex and synchronises its stream before the pointer is
+// published, so a second thread (on another stream) never sees a field still being written.
+int ensure_links_locked(const stag_links *L, int prec);
+int ensure_links(const stag_links *L, int prec)
 {
-    if (L->L[prec]) return STAG_OK;
+    if (!prec_ok(prec)) return STAG_EINVAL;
+    if (L->L_ready[prec].load(std::memory_order_acquire)) return STAG_OK;
+    std::lock_guard<std::mutex> lk(L->mu_links);
+    if (L->L_ready[prec].load(std::memory_order_relaxed)) return STAG_OK;
+    const int rc = ensure_links_locked(L, prec);
+    if (rc == STAG_OK) L->L_ready[prec].store(1, std::memory_order_release);
+    return rc;
+}
+
+int ensure_links_locked(const stag_links *L, int prec)
+{
     const int rows = prec_rows(prec);
     if (rows == 2 && !(L->recon_err <= 1e-10)) {
         snprintf(t_errbuf, sizeof(t_errbuf),
@@ -199,6 +212,13 @@ int ensure_links(stag_links *L, int prec)
         const double limit = f32 ? 1e-3 : 1e-9;
         if (!(L->recon_err <= 1e-10)) {
             snprintf(t_errbuf, sizeof(t_errbuf), "8-parameter links refused: the links are not +-SU(3) (max error %.3g)", L->recon_err);
+            t_errbuf_status = STAG_EINVAL;
+            return STAG_EINVAL;
+        }
+        if (L->recon8_err[f32] >= 0.0 && !(L->recon8_err[f32] <= limit)) {     // refused before: same answer, no rebuild
+            snprintf(t_errbuf, sizeof(t_errbuf),
+                     "8-parameter links refused: rebuilt entries are off by up to %.3g (limit %.1g); a link with a first row near (a1,0,0) has no usable 8-parameter form",
+                     L->recon8_err[f32], limit);
             t_errbuf_status = STAG_EINVAL;
             return STAG_EINVAL;
         }
@@ -240,17 +260,9 @@ int ensure_links(stag_links *L, int prec)
     }
     count_launch();
     cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(t_stream);     // published only once it is complete
     if (e != cudaSuccess) { cudaFree(dst); return cuda_fail(e, "derive_links_kernel", __LINE__); }
     L->L[prec] = dst;
-    return STAG_OK;
-}
-
-int ensure_tmp(stag_links *L, int f32, int nrhs)
-{
-    if (L->tmp_odd[f32] && L->tmp_odd_rhs[f32] >= nrhs) return STAG_OK;
-    if (L->tmp_odd[f32]) { CU(cudaFree(L->tmp_odd[f32])); L->tmp_odd[f32] = nullptr; }
-    CU(cudaMalloc(&L->tmp_odd[f32], (size_t)nrhs * 3 * L->g.Vh_pad * (f32 ? sizeof(float2) : sizeof(double2))));
-    L->tmp_odd_rhs[f32] = nrhs;
     return STAG_OK;
 }
 
@@ -402,7 +414,7 @@ static int links_create(stag_links_t **links_out, const int dims[4], int antiper
     g.X3g = dims[3];
     stag_links *L = new (std::nothrow) stag_links();
     if (!L) return STAG_ENOMEM;
-    memset(L, 0, sizeof(*L));
+    L->uid = g_next_uid.fetch_add(1, std::memory_order_relaxed);
     L->g = g;
     for (int m = 0; m < 4; ++m) { L->dims[m] = ldims[m]; L->gdims[m] = dims[m]; }
     L->rank = rank;
@@ -430,8 +442,7 @@ static int links_create(stag_links_t **links_out, const int dims[4], int antiper
         if ((e = cudaMemcpyAsync(&bits, err, sizeof(bits), cudaMemcpyDeviceToHost, t_stream)) != cudaSuccess) { rc = cuda_fail(e, "cudaMemcpyAsync(err)", __LINE__); break; }
         if ((e = cudaStreamSynchronize(t_stream)) != cudaSuccess) { rc = cuda_fail(e, "cudaStreamSynchronize", __LINE__); break; }
         memcpy(&L->recon_err, &bits, sizeof(double));
-        if ((e = cudaStreamCreateWithFlags(&L->cap_stream, cudaStreamNonBlocking)) != cudaSuccess) { rc = cuda_fail(e, "cudaStreamCreate", __LINE__); break; }
-        if ((e = cudaEventCreate(&L->ev0)) != cudaSuccess || (e = cudaEventCreate(&L->ev1)) != cudaSuccess) { rc = cuda_fail(e, "cudaEventCreate", __LINE__); break; }
+        L->L_ready[STAG_PREC_F64].store(1, std::memory_order_release);
     } while (0);
     if (Wd) cudaFree(Wd);
     if (err) cudaFree(err);
@@ -446,23 +457,15 @@ extern "C" void stag_links_destroy(stag_links_t *L)
 {
     if (!L) return;
     for (int i = 0; i < N_PREC; ++i) if (L->L[i]) cudaFree(L->L[i]);
-    for (int i = 0; i < 2; ++i) if (L->tmp_odd[i]) cudaFree(L->tmp_odd[i]);
-    if (L->ws) cudaFree(L->ws);
-    if (L->h_ctrl) cudaFreeHost(L->h_ctrl);
-    if (L->stage_dev) cudaFree(L->stage_dev);
-    if (L->wrap_b) cudaFree(L->wrap_b);
+    L->own.release();
     if (L->xch) cudaFree(L->xch);
     if (L->peers_dev) cudaFree(L->peers_dev);
     stag_slab_cg_free(L->cg);
-    if (L->cap_stream) cudaStreamDestroy(L->cap_stream);
-    if (L->ev0) cudaEventDestroy(L->ev0);
-    if (L->ev1) cudaEventDestroy(L->ev1);
     delete L;
 }
 
-extern "C" int stag_links_recon8_error(const stag_links_t *links, int prec, double *err_out)
+extern "C" int stag_links_recon8_error(const stag_links_t *L, int prec, double *err_out)
 {
-    stag_links *L = const_cast<stag_links *>(links);
     if (!L || !err_out || (prec != STAG_PREC_F64_R8 && prec != STAG_PREC_F32_R8)) return STAG_EINVAL;
     const int rc = ensure_links(L, prec);        // builds (or refuses) and measures
     *err_out = L->recon8_err[prec_is_f32(prec) ? 1 : 0];
@@ -516,7 +519,7 @@ extern "C" int stag_spinor_unpack(double *dst, const void *src, const int dims[4
 extern "C" int stag_dslash_mrhs(void *out, const void *in, const stag_links_t *links, int parity,
                                 const int dims[4], int prec, int nrhs)
 {
-    stag_links *L = const_cast<stag_links *>(links);
+    const stag_links *L = links;
     if (!out || !in || !L || out == in || (parity & ~1) || !prec_ok(prec) || !same_dims(L, dims) ||
         nrhs < 1 || L->is_slab)      // a slab's hop needs its halo: stag_slab_hop
         return STAG_EINVAL;
@@ -534,16 +537,19 @@ extern "C" int stag_dslash(void *out, const void *in, const stag_links_t *links,
 extern "C" int stag_apply_A_mrhs(void *out_even, const void *in_even, const stag_links_t *links,
                                  double mass, int prec, int nrhs)
 {
-    stag_links *L = const_cast<stag_links *>(links);
-    if (!out_even || !in_even || !L || out_even == in_even || !prec_ok(prec) || nrhs < 1 || L->is_slab)
+    const stag_links *L = links;
+    if (!out_even || !in_even || !L || out_even == in_even || !prec_ok(prec) || nrhs < 1 || nrhs > MAX_RHS || L->is_slab)
         return STAG_EINVAL;
     int rc = ensure_links(L, prec);
     if (rc) return rc;
-    const int f32 = prec_is_f32(prec) ? 1 : 0;
-    if ((rc = ensure_tmp(L, f32, nrhs))) return rc;
+    // the odd-site intermediate lives in the workspace (the caller's, or the handle's own)
+    const WsLayout lay = ws_layout(L->g, -1, nrhs);
+    WsLease lease;
+    if ((rc = lease_workspace(L, lay.total, lease))) return rc;
+    void *tmp_odd = lease.ws->base + lay.scratch;
     // tmp_o = D_oe in_e ;  out_e = m^2 in_e - D_eo tmp_o      (eq. 2.3)
-    if ((rc = launch_hop(L, prec, HOP_PLAIN, L->tmp_odd[f32], in_even, 1, 0.0, 1.0, nullptr, nullptr, nullptr, nrhs, t_stream))) return rc;
-    return launch_hop(L, prec, HOP_XPAY, out_even, L->tmp_odd[f32], 0, mass * mass, 1.0, in_even, nullptr, nullptr, nrhs, t_stream);
+    if ((rc = launch_hop(L, prec, HOP_PLAIN, tmp_odd, in_even, 1, 0.0, 1.0, nullptr, nullptr, nullptr, nrhs, t_stream))) return rc;
+    return launch_hop(L, prec, HOP_XPAY, out_even, tmp_odd, 0, mass * mass, 1.0, in_even, nullptr, nullptr, nrhs, t_stream);
 }
 
 extern "C" int stag_apply_A(void *out_even, const void *in_even, const stag_links_t *links,

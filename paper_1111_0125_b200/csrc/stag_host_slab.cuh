@@ -281,7 +281,7 @@ int slab_residual_phase(stag_links *L, stag_slab_cg *C, int ph, bool accumulate_
         return slab_push_prec(L, w.tmp64, C->prec_hi, s);
     case 2:
         if ((rc = slab_hop_mode(L, C->prec_hi, HOP_XPAY, w.q64, w.tmp64, 0, C->m2, C->x, nullptr, nullptr, s))) return rc;
-        slab_residual_kernel<float, WHAT><<<C->gb, BLAS_BLOCK, 0, s>>>(w.r64, C->b, w.q64, lo_copy ? w.r32 : nullptr, C->n, w.partials, w.ctrl, make_comm(L));
+        slab_residual_kernel<float, WHAT><<<C->gb, BLAS_BLOCK, 0, s>>>(w.r64, C->b, w.q64, lo_copy ? w.r32 : nullptr, C->n, 2L * L->g.Vh_pad, 2L * L->g.Vh, w.partials, w.ctrl, make_comm(L));
         count_launch();
         KCHECK();
         return STAG_OK;
@@ -364,15 +364,29 @@ extern "C" int stag_slab_cg_begin(stag_links_t *L, void *x_even, const void *b_e
     int rc;
     if ((rc = ensure_links(L, C->prec_lo))) return rc;
     if ((rc = ensure_links(L, C->prec_hi))) return rc;
-    if ((rc = ensure_workspace(L, C->w, 1))) return rc;
-    CgCtrl *h = L->h_ctrl;
+    {   // a slab handle belongs to one host thread and owns its workspace
+        const WsLayout lay = ws_layout(L->g, mode, 1);
+        WsLease lease;
+        WsHost *saved = t_ws.p;
+        t_ws.p = nullptr;                           // never the caller's: the solve spans several calls
+        rc = lease_workspace(L, lay.total, lease);
+        t_ws.p = saved;
+        if (rc) return rc;
+        carve(L->own.base, lay, C->w);
+    }
+    if (L->g.Vh_pad != L->g.Vh) {
+        zero_pads_kernel<<<dim3(1, 1), 128, 0, t_stream>>>((double2 *)x_even, L->g.Vh, L->g.Vh_pad);
+        count_launch();
+        KCHECK();
+    }
+    CgCtrl *h = L->own.h_ctrl;
     memset(h, 0, sizeof(*h));
     h->mode = mode;
     h->maxiter = maxiter;
     h->eps_in = C->P.eps_in;
     h->nrhs = 1;
     CU(cudaMemcpyAsync(C->w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, t_stream));
-    CU(cudaEventRecord(L->ev0, t_stream));
+    CU(cudaEventRecord(L->own.ev0, t_stream));
     C->stage = 0;
     return STAG_OK;
 }
@@ -383,7 +397,7 @@ extern "C" int stag_slab_cg_control(stag_links_t *L, int *action_out)
 {
     if (!L || !L->is_slab || !L->cg || !action_out) return STAG_EINVAL;
     stag_slab_cg *C = L->cg;
-    CgCtrl *h = L->h_ctrl;
+    CgCtrl *h = L->own.h_ctrl;
     if (C->stage == 0) { C->stage = 1; *action_out = STAG_SLAB_ACT_NORM; return STAG_OK; }
     if (C->stage == 3) { *action_out = STAG_SLAB_ACT_DONE; return STAG_OK; }
     CU(cudaMemcpyAsync(h, C->w.ctrl, sizeof(CgCtrl), cudaMemcpyDeviceToHost, t_stream));
@@ -469,7 +483,7 @@ static int slab_cg_step_on(stag_links_t *L, int action, int phase, int *more_out
     switch (action) {
     case STAG_SLAB_ACT_NORM:
         if (phase == 0) {
-                slab_residual_kernel<float, RES_NORM><<<C->gb, BLAS_BLOCK, 0, t_stream>>>(nullptr, C->b, nullptr, nullptr, C->n, w.partials, w.ctrl, make_comm(L));
+            slab_residual_kernel<float, RES_NORM><<<C->gb, BLAS_BLOCK, 0, t_stream>>>(nullptr, C->b, nullptr, nullptr, C->n, 2L * L->g.Vh_pad, 2L * L->g.Vh, w.partials, w.ctrl, make_comm(L));
             count_launch();
             KCHECK();
             more = true;
@@ -513,12 +527,12 @@ extern "C" int stag_slab_cg_finish(stag_links_t *L, stag_cg_stats_t *stats_out)
 {
     if (!L || !L->is_slab || !L->cg || L->cg->stage != 3) return STAG_EINVAL;
     stag_slab_cg *C = L->cg;
-    CgCtrl *h = L->h_ctrl;
-    CU(cudaEventRecord(L->ev1, t_stream));
+    CgCtrl *h = L->own.h_ctrl;
+    CU(cudaEventRecord(L->own.ev1, t_stream));
     CU(cudaStreamSynchronize(t_stream));
     { const int ws = stag_slab_status(L); if (ws != STAG_OK) return ws; }
     float ms = 0.f;
-    CU(cudaEventElapsedTime(&ms, L->ev0, L->ev1));
+    CU(cudaEventElapsedTime(&ms, L->own.ev0, L->own.ev1));
     stag_cg_stats_t st;
     memset(&st, 0, sizeof(st));
     st.iters = h->iters[0];
@@ -554,16 +568,16 @@ extern "C" int stag_slab_cg_run(stag_links_t *L, void *x_even, const void *b_eve
             stag_slab_cg *C = L->cg;
             if (!C->iter_graph) {
                 cudaGraph_t graph = nullptr;
-                cudaError_t e = cudaStreamBeginCapture(L->cap_stream, cudaStreamCaptureModeThreadLocal);
+                cudaError_t e = cudaStreamBeginCapture(L->own.cap_stream, cudaStreamCaptureModeThreadLocal);
                 if (e != cudaSuccess) return cuda_fail(e, "cudaStreamBeginCapture", __LINE__);
                 t_capturing = true;
                 t_captured_nodes = 0;
                 int more = 1;
                 rc = STAG_OK;
-                for (int ph = 0; more && rc == STAG_OK; ++ph) rc = slab_cg_step_on(L, act, ph, &more, L->cap_stream);
+                for (int ph = 0; more && rc == STAG_OK; ++ph) rc = slab_cg_step_on(L, act, ph, &more, L->own.cap_stream);
                 t_capturing = false;
                 C->iter_graph_nodes = t_captured_nodes;
-                e = cudaStreamEndCapture(L->cap_stream, &graph);
+                e = cudaStreamEndCapture(L->own.cap_stream, &graph);
                 if (rc != STAG_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
                 if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture", __LINE__);
                 e = cudaGraphInstantiate(&C->iter_graph, graph, 0);

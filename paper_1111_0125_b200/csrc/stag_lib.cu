@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <type_traits>
 
@@ -62,17 +63,23 @@ inline int prec_rows(int prec)
 
 // Grid of the streaming vector kernels: 4 resident blocks of 256 threads per SM (a multiple of
 // the SM count) shared among the nrhs right-hand sides (grid.y = nrhs), fewer when the vector
-// is too short to feed them.  Returns grid.x, the blocks per right-hand side.
+// is too short to feed them.  Returns grid.x, the blocks per right-hand side.  Never more than
+// MAX_BLAS_GRID, which is what a workspace reserves partial-sum slots for.
+constexpr int MAX_BLAS_GRID = 1024;
 int blas_full_grid()
 {
-    static int full = 0;
-    if (full == 0) {
+    static std::atomic<int> full{0};
+    int f = full.load(std::memory_order_relaxed);
+    if (f == 0) {
         int dev = 0, sms = 148;
         if (cudaGetDevice(&dev) == cudaSuccess)
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        full = sms * 4;
+        f = sms * 4;
+        if (f > MAX_BLAS_GRID) f = MAX_BLAS_GRID;
+        if (f < 1) f = 1;
+        full.store(f, std::memory_order_relaxed);
     }
-    return full;
+    return f;
 }
 int blas_grid(long n_reals, int nrhs)
 {
@@ -85,44 +92,116 @@ int blas_grid(long n_reals, int nrhs)
 }  // namespace
 
 // ------------------------------------------------------------------------------------
-// the link handle
+// CG workspace: device memory for Fig. 1's vectors r, d, Ad and the mixed driver's
+// y, fp32 copies and scalars, plus the host-side objects that go with one solve in flight.
+// Either caller-owned (stag_set_workspace, one per host thread) or owned by a link handle and
+// shared, behind the handle's mutex, by every call that finds no caller workspace.
 // ------------------------------------------------------------------------------------
-struct stag_slab_cg;
-struct stag_links {
-    Geom g;
-    int dims[4];           // extents of the lattice this handle covers (the slab's, for a slab)
-    int gdims[4];          // extents of the whole lattice
-    int rank, nranks;      // T-slab: time slices [rank*X3, (rank+1)*X3) of nranks*X3; else 0, 1
-    int is_slab;           // made by stag_slab_create: operator calls go through stag_slab_*
-    int ntiles;            // Vh_pad / TILE
-    void *L[6];            // gathered link fields by precision enum; L[STAG_PREC_F64] always set
-    double recon8_err[2];  // 8-parameter forms: largest rebuilt-entry error, [0] fp64, [1] fp32 (-1: not built)
-    double recon_err;
-    void *tmp_odd[2];      // scratch odd-parity spinors for stag_apply_A: [0] fp64, [1] fp32
-    int tmp_odd_rhs[2];    // how many right-hand sides each holds
-    // CG workspace (lazy)
-    char *ws;
-    size_t ws_bytes;
-    int ws_rhs;            // right-hand sides the workspace was sized for
-    CgCtrl *h_ctrl;        // pinned mirror
-    cudaStream_t cap_stream;
-    // staging for stag_cg_solve_host (lazy)
-    double *stage_dev;     // 2 canonical spinors + 2 device-layout fp64 spinors
-    // T-slab exchange (stag_slab_*): my exchange region, the neighbours' (peer memory), and the
-    // number of exchanges started so far
-    char *xch;
-    char *peer_bwd, *peer_fwd;
-    unsigned long long epoch;
-    unsigned n_push_blocks; // blocks of a HALO hop that own boundary-slice sites (cached)
-    char **peers_dev;      // device array: every rank's exchange region (stag_slab_connect_all)
-    int all_connected;
-    struct stag_slab_cg *cg;   // state of the slab CG in progress (stag_slab_cg_*)
-    void *wrap_b;          // stag_solve_M: b_e of the even-site system, wrap_b_rhs spinors (lazy)
-    int wrap_b_rhs;
-    cudaEvent_t ev0, ev1;
+struct GraphSlot {           // one instantiated CUDA graph of `chunk` CG iterations, and what it baked in
+    unsigned long long uid;  // the link handle's unique id (not its address: handles come and go)
+    int mode, prec_lo, nrhs, chunk;
+    double m2;
+    const void *x;           // mode 0 iterates on the caller's x itself; null for the fp32 modes
+    cudaGraphExec_t exec;
+    unsigned long long nodes, stamp;
+};
+constexpr int N_GRAPH_SLOTS = 4;
+
+struct WsHost {
+    char *base = nullptr;
+    size_t bytes = 0;
+    bool owned = false;          // base was cudaMalloc'ed by the library (handle-owned workspace)
+    bool in_use = false;         // a call is running on it (re-entry guard)
+    CgCtrl *h_ctrl = nullptr;    // pinned mirror of the control block
+    cudaStream_t cap_stream = nullptr;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr, busy = nullptr;
+    cudaStream_t last_stream = nullptr;
+    bool busy_recorded = false;
+    GraphSlot graphs[N_GRAPH_SLOTS] = {};
+    unsigned long long stamp = 0;
+
+    int init_host_objects()
+    {
+        if (h_ctrl) return STAG_OK;
+        CU(cudaMallocHost((void **)&h_ctrl, sizeof(CgCtrl)));
+        CU(cudaStreamCreateWithFlags(&cap_stream, cudaStreamNonBlocking));
+        CU(cudaEventCreate(&ev0));
+        CU(cudaEventCreate(&ev1));
+        CU(cudaEventCreateWithFlags(&busy, cudaEventDisableTiming));
+        return STAG_OK;
+    }
+    void drop_graphs()
+    {
+        for (GraphSlot &g : graphs) {
+            if (g.exec) cudaGraphExecDestroy(g.exec);
+            g = GraphSlot{};
+        }
+    }
+    void release()
+    {
+        drop_graphs();
+        if (owned && base) cudaFree(base);
+        base = nullptr; bytes = 0; owned = false;
+        if (h_ctrl) cudaFreeHost(h_ctrl);
+        if (cap_stream) cudaStreamDestroy(cap_stream);
+        if (ev0) cudaEventDestroy(ev0);
+        if (ev1) cudaEventDestroy(ev1);
+        if (busy) cudaEventDestroy(busy);
+        h_ctrl = nullptr; cap_stream = nullptr; ev0 = ev1 = busy = nullptr;
+        busy_recorded = false;
+    }
 };
 
-// The rest of the translation unit, in three sections (they see everything above):
+namespace {
+// the caller-owned workspace of this host thread (stag_set_workspace), if any
+struct ThreadWs {
+    WsHost *p = nullptr;
+    ~ThreadWs() { if (p) { p->release(); delete p; p = nullptr; } }
+};
+thread_local ThreadWs t_ws;
+std::atomic<unsigned long long> g_next_uid{1};
+}  // namespace
+
+// ------------------------------------------------------------------------------------
+// the link handle
+// ------------------------------------------------------------------------------------
+// Immutable after creation for every caller of the `const stag_links_t *` entry points, with two
+// exceptions that are invisible to them and internally synchronised (hence `mutable`):
+//   * the derived link forms (fp32, 12-real, 8-parameter), built once on first use under mu_links
+//     and published only after the building stream has been synchronised;
+//   * the handle-owned workspace `own`, used only when the calling thread has set none, under mu_ws
+//     for the whole call.
+struct stag_slab_cg;
+struct stag_links {
+    Geom g{};
+    int dims[4] = {0, 0, 0, 0};    // extents of the lattice this handle covers (the slab's, for a slab)
+    int gdims[4] = {0, 0, 0, 0};   // extents of the whole lattice
+    int rank = 0, nranks = 1;      // T-slab: time slices [rank*X3, (rank+1)*X3) of nranks*X3; else 0, 1
+    int is_slab = 0;               // made by stag_slab_create: operator calls go through stag_slab_*
+    int ntiles = 0;                // Vh_pad / TILE
+    unsigned long long uid = 0;
+    double recon_err = 0.0;
+    mutable std::mutex mu_links;
+    mutable void *L[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // gathered link fields by precision enum
+    mutable std::atomic<int> L_ready[6];
+    mutable double recon8_err[2] = {-1.0, -1.0};   // 8-parameter forms: largest rebuilt-entry error, [0] fp64, [1] fp32
+    mutable std::mutex mu_ws;
+    mutable WsHost own;
+    // T-slab exchange (stag_slab_*; slab handles are not const in the ABI and belong to one host
+    // thread): my exchange region, the neighbours' (peer memory), exchanges started so far
+    char *xch = nullptr;
+    char *peer_bwd = nullptr, *peer_fwd = nullptr;
+    unsigned long long epoch = 0;
+    unsigned n_push_blocks = 0;    // blocks of a HALO hop that own boundary-slice sites (cached)
+    char **peers_dev = nullptr;    // device array: every rank's exchange region (stag_slab_connect_all)
+    int all_connected = 0;
+    struct stag_slab_cg *cg = nullptr;   // state of the slab CG in progress (stag_slab_cg_*)
+
+    stag_links() { for (auto &r : L_ready) r.store(0, std::memory_order_relaxed); }
+};
+
+// The rest of the translation unit, in four sections (they see everything above):
+#include "stag_host_ws.cuh"      // the CG workspace: layout, lease; C ABI: stag_cg_workspace_bytes, stag_set_workspace
 #include "stag_host_links.cuh"   // S0 kernels, hop launchers; C ABI: state, links, spinors, operator
 #include "stag_host_cg.cuh"      // one-GPU CG drivers; C ABI: stag_cg_solve*, stag_solve_M
 #include "stag_host_slab.cuh"    // T-slabs: wiring, push / hop, CG over slabs; C ABI: stag_slab_*

@@ -243,16 +243,17 @@ slab_update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d
 template <typename T, int WHAT>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 slab_residual_kernel(double *__restrict__ r, const double *__restrict__ b,
-                     const double *__restrict__ q, T *__restrict__ r_lo, long n,
+                     const double *__restrict__ q, T *__restrict__ r_lo, long n, long n_plane, long n_valid,
                      double *__restrict__ partials, CgCtrl *__restrict__ ctrl, const Comm c)
 {
     double s = 0.0;
     for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < n; i += (long)gridDim.x * BLAS_BLOCK) {
+        const double bi = (n_valid == n_plane || i % n_plane < n_valid) ? b[i] : 0.0;   // b's pad lanes count as zero
         if (WHAT == RES_NORM) {
-            const double v = b[i];
+            const double v = bi;
             s += v * v;
         } else {
-            const double v = b[i] - q[i];
+            const double v = bi - q[i];
             r[i] = v;
             if (r_lo != nullptr) r_lo[i] = (T)v;
             s += v * v;

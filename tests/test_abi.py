@@ -53,6 +53,29 @@ def test_spinor_bytes_and_argument_checks_on_host():
     assert stag.spinor_bytes((4, 4, 4, 4), 7) == 0                  # bad enum
 
 
+def test_workspace_bytes_is_pure_arithmetic_on_host():
+    """stag_cg_workspace_bytes needs no device: control block + partial-sum
+    slots + the vectors of Fig. 1 the mode needs."""
+    d = (28, 28, 28, 96)
+    sp64, sp32 = stag.spinor_bytes(d, stag.PREC_F64), stag.spinor_bytes(d, stag.PREC_F32)
+    w0, w1, w3 = (stag.cg_workspace_bytes(d, m) for m in (stag.CG_F64, stag.CG_F32, stag.CG_RELIABLE))
+    fixed = w0 - 7 * sp64           # b_e, 2 staging, r, q, tmp, d in fp64
+    assert 0 < fixed < (1 << 20)
+    assert w3 == w1 == fixed + 6 * sp64 + 5 * sp32      # no fp64 d; y, r, d, q, tmp in fp32
+    assert stag.cg_workspace_bytes(d, stag.CG_DEFECT) == w3
+    op = stag.cg_workspace_bytes(d, -1)
+    assert fixed - 2 * 256 <= op - sp64 <= fixed        # operator only: one odd-site intermediate
+    # right-hand sides scale the vectors, not the fixed part
+    w3_4 = stag.cg_workspace_bytes(d, stag.CG_RELIABLE, 4)
+    assert 4 * (4 * sp64 + 5 * sp32) + 2 * sp64 <= w3_4 <= 4 * (4 * sp64 + 5 * sp32) + 2 * sp64 + (1 << 20)
+    assert stag.cg_workspace_bytes(d, 4) == 0 and stag.cg_workspace_bytes(d, 0, 0) == 0
+    assert stag.cg_workspace_bytes(d, 0, stag.MAX_RHS + 1) == 0
+    assert stag.cg_workspace_bytes((28, 28, 28, 95), 0) == 0
+    # the setter checks its arguments before it touches the device
+    assert stag.lib().stag_set_workspace(None, 0) == stag.OK
+    assert stag.lib().stag_set_workspace(None, 64) == stag.EINVAL
+
+
 def test_strerror_and_null_arguments():
     lib = stag.lib()
     assert lib.stag_strerror(0) == b"ok"

@@ -1,0 +1,57 @@
+"""The compact oracle records tests/golden/refsol_*.npz (written by make_reference_solutions.py
+from oracle/ + fieldgen/ only) and the sketch that scores a full-size solution against them,
+checked WITHOUT a GPU on the config the oracle solves in seconds (16^3 x 32): the record is what
+the oracle computes today, the sketch's estimate of |x - x_ref|_2 agrees with the true norm of a
+known perturbation, and a single corrupted site is visible in it."""
+import numpy as np
+import pytest
+
+import fieldgen
+import oracle
+from tests import refsol
+
+
+@pytest.fixture(scope="module")
+def c3():
+    cfg = fieldgen.CONFIGS["c3_16^3x32"]
+    W, b = cfg.links(), cfg.source()
+    x, it, rho, _, rc = oracle.cg(b, W, cfg.dims, cfg.mass, 1e-12, 10 * cfg.maxiter)
+    assert rc == 0 and rho <= 1e-12
+    return cfg, refsol.load(cfg.name), x, it
+
+
+def test_record_is_what_the_oracle_computes(c3):
+    cfg, rec, x, it = c3
+    assert int(rec["iters"]) == it
+    s = refsol.score(x, rec, cfg)
+    # same solver, same inputs: equal up to the thread count's summation order (~1e-13)
+    assert s["l2_sketch"] <= 1e-11 and s["l2_sites"] <= 1e-11 and s["max_site"] <= 1e-11 and s["norm"] <= 1e-12
+
+
+def test_sketch_estimates_the_norm_of_a_known_error(c3):
+    cfg, rec, x, _ = c3
+    for seed, size in ((5, 1e-6), (6, 1e-9)):
+        e = fieldgen.spinor_gaussian(cfg.dims, 0, seed) * size
+        true = np.linalg.norm(e.ravel()) / np.linalg.norm(x.ravel())
+        est = refsol.score(x + e, rec, cfg)["l2_sketch"]
+        assert 0.6 * true <= est <= 1.5 * true          # 32 projections: relative std 1/sqrt(32) = 18 %
+
+
+def test_sketch_sees_one_wrong_site_that_the_samples_miss(c3):
+    cfg, rec, x, _ = c3
+    miss = next(i for i in range(cfg.vh) if i not in set(rec["sites"].tolist()))
+    y = x.copy()
+    y[miss, 1] += 1e-3 * float(rec["x_absmax"])
+    s = refsol.score(y, rec, cfg)
+    assert s["l2_sites"] == 0.0 and s["max_site"] == 0.0     # not among the sampled sites
+    true = 1e-3 * float(rec["x_absmax"]) / float(rec["x_norm"])
+    assert 0.5 * true <= s["l2_sketch"] <= 1.6 * true        # but every projection moved
+
+
+@pytest.mark.parametrize("name", ["c4_28^3x96", "c5_48^3x96"])
+def test_full_size_records_are_present_and_consistent(name):
+    rec = refsol.load(name)           # checks seeds, dims, mass, residual <= 1e-12
+    cfg = fieldgen.CONFIGS[name]
+    assert len(rec["sites"]) >= 4096 and len(rec["proj"]) >= 32
+    assert rec["x_sites"].shape == (len(rec["sites"]), 3) and rec["sites"].max() < cfg.vh
+    assert float(rec["x_absmax"]) >= np.abs(rec["x_sites"]).max() > 0

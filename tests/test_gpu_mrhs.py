@@ -17,8 +17,7 @@ TOL = {stag.PREC_F64: 1e-13, stag.PREC_F64_R12: 1e-13, stag.PREC_F32: 2e-6, stag
 ALL_PREC = [stag.PREC_F64, stag.PREC_F32, stag.PREC_F64_R12, stag.PREC_F32_R12]
 
 
-def rel_l2(a, b):
-    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
+from tests.parity import rel_err as rel_l2  # L2 AND worst-site bound (tests/parity.py)
 
 
 # nrhs values cover every chunking: 1..4 in one fp32 launch, 5 = 4+1, 7 = 4+3, 12 = the cap;

@@ -44,8 +44,7 @@ def _worker(rank, port, q):
             torch.cuda.synchronize()
             dist.barrier()
 
-        def rel(a, b):
-            return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
+        from tests.parity import rel_err as rel      # L2 AND worst-site bound (tests/parity.py)
 
         out = {}
         # the hop, all four precisions, twice each (both halo buffers)

@@ -47,8 +47,7 @@ def _worker(rank, world, port, q):
         S.connect_distributed()
         S.set_wait_limit(1 << 22)
 
-        def rel(a, c):
-            return float(np.linalg.norm((a - c).ravel()) / np.linalg.norm(c.ravel()))
+        from tests.parity import rel_err as rel      # L2 AND worst-site bound (tests/parity.py)
 
         ref = slab.scatter_spinor(oracle.dslash(b, W, DIMS, 1), DIMS, rank, world)
         for prec, tol in ((0, 1e-13), (3, 2e-6)):
