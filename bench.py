@@ -188,19 +188,19 @@ def time_dslash(stag, torch, fieldgen, cfg, L, prec, launches=60, nrot=6):
             "paper_convention_gbs": paper_bytes * cfg.vh / sec * 1e-9}
 
 
-def time_dslash_mrhs(stag, torch, fieldgen, cfg, L, prec, nrhs, launches=30, nrot=3):
-    """The same for a batch of nrhs spinors through stag_dslash_mrhs (links read once per chunk of
-    4 fp32 / 2 fp64 right-hand sides)."""
+def time_dslash_mrhs(stag, torch, fieldgen, cfg, L, prec, nrhs, launches=30, nrot=3, layout=0):
+    """The same for a batch of nrhs spinors through stag_dslash_batch (links read once per chunk of
+    4 fp32 / 2 fp64 right-hand sides); layout 0 = blocked (stag_dslash_mrhs), 1 = paired."""
     srcs = [fieldgen.spinor_gaussian(cfg.dims, 0, seed=300 + k) for k in range(nrhs)]
-    ins = [stag.spinor_pack_mrhs(srcs, cfg.dims, prec) for _ in range(nrot)]
+    ins = [stag.batch_convert(stag.spinor_pack_mrhs(srcs, cfg.dims, prec), cfg.dims, prec, layout) for _ in range(nrot)]
     outs = [torch.empty_like(ins[0]) for _ in range(nrot)]
     for i in range(3):
-        stag.dslash_mrhs(ins[i % nrot], L, 1, prec, out=outs[i % nrot])
+        stag.dslash_mrhs(ins[i % nrot], L, 1, prec, out=outs[i % nrot], layout=layout)
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for i in range(launches):
-        stag.dslash_mrhs(ins[i % nrot], L, 1, prec, out=outs[i % nrot])
+        stag.dslash_mrhs(ins[i % nrot], L, 1, prec, out=outs[i % nrot], layout=layout)
     e1.record()
     torch.cuda.synchronize()
     sec = e0.elapsed_time(e1) * 1e-3 / launches
@@ -306,8 +306,11 @@ def run_ours(args):
             "time_to_solution_s": st3[0]["seconds"],
             "gflops": sum(t["iters"] for t in st3) * FLOP_PER_SITE_ITER * cfg.vh / st3[0]["seconds"] * 1e-9,
             "us_per_iteration_per_rhs": st3[0]["seconds"] / max(1, max(t["iters"] for t in st3)) / 3 * 1e6,
-            "dslash": {"%s x%d" % (stag.PREC_NAMES[p], n): time_dslash_mrhs(stag, torch, fieldgen, cfg, L, p, n)
-                       for p, n in ((stag.PREC_F32_R12, 3), (stag.PREC_F32_R12, 4), (stag.PREC_F32, 4), (stag.PREC_F64, 2))}}
+            "dslash": {"%s x%d" % (stag.PREC_NAMES[p], n): time_dslash_mrhs(stag, torch, fieldgen, cfg, L, p, n, layout=stag.BATCH_PAIRED if p in (stag.PREC_F32, stag.PREC_F32_R12) else 0)
+                       for p, n in ((stag.PREC_F32_R12, 2), (stag.PREC_F32_R12, 3), (stag.PREC_F32_R12, 4), (stag.PREC_F32, 4), (stag.PREC_F64, 2))},
+            "dslash_blocked_layout": {"%s x%d" % (stag.PREC_NAMES[p], n): time_dslash_mrhs(stag, torch, fieldgen, cfg, L, p, n)
+                                      for p, n in ((stag.PREC_F32_R12, 3), (stag.PREC_F32_R12, 4), (stag.PREC_F32, 4))},
+            "layout": "fp32 batches paired (include/stag.h batch layouts), fp64 blocked"}
     del b3, x3
 
     cpu = None

@@ -218,6 +218,25 @@ int stag_dslash_mrhs(void *out, const void *in, const stag_links_t *links, int p
 int stag_apply_A_mrhs(void *out_even, const void *in_even, const stag_links_t *links, double mass,
                       int prec, int nrhs);
 
+/* Batch layouts.  BLOCKED is the layout above (nrhs spinors back to back) and the only one of fp64
+ * batches.  PAIRED (fp32 only) interleaves right-hand sides 2j and 2j+1 per complex number:
+ *     pair j:  p[j][c][cb] = (re_2j, im_2j, re_2j+1, im_2j+1)    one 16-byte element per (colour, site)
+ * stored where spinors 2j and 2j+1 of the blocked batch would be (2 * stag_spinor_bytes per pair);
+ * an odd last right-hand side stays an ordinary spinor after the pairs, so both layouts take
+ * nrhs * stag_spinor_bytes and nrhs = 1 is the same in both.  In the paired layout a neighbour's
+ * colour for two right-hand sides is ONE 16-byte gather: the batch hop, which is bound by issue
+ * slots and loads in flight rather than by DRAM, needs half the gather
+ * instructions.  The arithmetic per right-hand side, and so every result bit, is the same in both.
+ * The fp32 iteration of stag_cg_solve_mrhs / stag_solve_M keeps its vectors paired internally;
+ * their x and b (fp64) are blocked.  stag_batch_convert changes the layout of a batch (dst != src;
+ * fp64: a copy); stag_dslash_batch / stag_apply_A_batch are the *_mrhs calls on a given layout. */
+enum { STAG_BATCH_BLOCKED = 0, STAG_BATCH_PAIRED = 1 };
+int stag_batch_convert(void *dst, const void *src, const int dims[4], int prec, int nrhs, int to_layout);
+int stag_dslash_batch(void *out, const void *in, const stag_links_t *links, int parity,
+                      const int dims[4], int prec, int nrhs, int layout);
+int stag_apply_A_batch(void *out_even, const void *in_even, const stag_links_t *links, double mass,
+                       int prec, int nrhs, int layout);
+
 /* ---- T-slabs: the hop on a lattice split along time over several GPUs --------------------
  *
  * The paper's subject is the multi-GPU Dirac operation: kernel, boundary collect, memcpy to the

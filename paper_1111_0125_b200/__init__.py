@@ -39,6 +39,7 @@ CG_F64, CG_F32, CG_DEFECT, CG_RELIABLE = 0, 1, 2, 3
 OK, EINVAL, ECUDA, ENOMEM, ETIMEOUT, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, 1, 2
 
 MAX_RHS = 12
+BATCH_BLOCKED, BATCH_PAIRED = 0, 1
 
 PREC_NAMES = {PREC_F64: "fp64/18", PREC_F32: "fp32/18", PREC_F64_R12: "fp64/12", PREC_F32_R12: "fp32/12",
               PREC_F64_R8: "fp64/8", PREC_F32_R8: "fp32/8"}
@@ -112,6 +113,9 @@ SIGNATURES = {
                                         ctypes.c_int, ctypes.POINTER(_Params), ctypes.POINTER(_Stats)]),
     "stag_dslash_mrhs": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, _ip, ctypes.c_int, ctypes.c_int]),
     "stag_apply_A_mrhs": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_int, ctypes.c_int]),
+    "stag_batch_convert": (ctypes.c_int, [_vp, _vp, _ip, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
+    "stag_dslash_batch": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, _ip, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
+    "stag_apply_A_batch": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
     "stag_cg_solve_mrhs": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                           ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Params),
                                           ctypes.POINTER(_Stats)]),
@@ -423,26 +427,39 @@ def _batch(vs):
     return int(vs.shape[0])
 
 
-def dslash_mrhs(vs, links: Links, parity: int, prec, out=None):
-    """One hop of eq. 2.5 applied to every spinor of the batch, links read once per chunk."""
+def batch_convert(vs, dims, prec, to_layout: int, out=None):
+    """stag_batch_convert: the batch in the other layout (BATCH_BLOCKED <-> BATCH_PAIRED)."""
     torch = _require_cuda()
     use_current_stream()
     n = _batch(vs)
     if out is None:
         out = torch.empty_like(vs)
-    _check(lib().stag_dslash_mrhs(ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(vs.data_ptr()),
-                                  links.handle, int(parity), _cdims(links.dims), int(prec), n))
+    _check(lib().stag_batch_convert(ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(vs.data_ptr()),
+                                    _cdims(dims), int(prec), n, int(to_layout)))
     return out
 
 
-def apply_A_mrhs(vs_even, links: Links, mass: float, prec, out=None):
+def dslash_mrhs(vs, links: Links, parity: int, prec, out=None, layout: int = BATCH_BLOCKED):
+    """One hop of eq. 2.5 applied to every spinor of the batch, links read once per chunk
+    (stag_dslash_batch; layout BATCH_BLOCKED is stag_dslash_mrhs)."""
+    torch = _require_cuda()
+    use_current_stream()
+    n = _batch(vs)
+    if out is None:
+        out = torch.empty_like(vs)
+    _check(lib().stag_dslash_batch(ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(vs.data_ptr()),
+                                   links.handle, int(parity), _cdims(links.dims), int(prec), n, int(layout)))
+    return out
+
+
+def apply_A_mrhs(vs_even, links: Links, mass: float, prec, out=None, layout: int = BATCH_BLOCKED):
     torch = _require_cuda()
     use_current_stream()
     n = _batch(vs_even)
     if out is None:
         out = torch.empty_like(vs_even)
-    _check(lib().stag_apply_A_mrhs(ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(vs_even.data_ptr()),
-                                   links.handle, float(mass), int(prec), n))
+    _check(lib().stag_apply_A_batch(ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(vs_even.data_ptr()),
+                                    links.handle, float(mass), int(prec), n, int(layout)))
     return out
 
 

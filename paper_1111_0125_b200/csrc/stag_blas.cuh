@@ -27,22 +27,23 @@ template <typename T> __device__ __forceinline__ void unpack(const double2 &v, T
 __device__ __forceinline__ float4 pack(const float *a) { return make_float4(a[0], a[1], a[2], a[3]); }
 __device__ __forceinline__ double2 pack(const double *a) { return make_double2(a[0], a[1]); }
 
-// Second stage shared by all reducing kernels.  Every block calls it with its partial of
-// right-hand side blockIdx.y; in the LAST block of the grid to arrive it returns true (to all
-// threads) with totals[k] = sum of partials[k*gridDim.x .. +gridDim.x) in index order for every
-// k < gridDim.y (totals is shared memory, MAX_RHS doubles).
-__device__ __forceinline__ bool finish_reduction(double block_value, double *partials,
-                                                 unsigned *ticket, double *red, double *totals)
+// Second stage shared by all reducing kernels.  Every block calls it with its nv (1 or 2)
+// partial sums, of right-hand sides k0 .. k0+nv-1; in the LAST block of the grid to arrive it
+// returns true (to all threads) with totals[k] = sum of partials[k*gridDim.x .. +gridDim.x) in
+// index order for every k < nrhs (totals is shared memory, MAX_RHS doubles).  A right-hand side
+// no block reports keeps the partials of an earlier launch: only frozen ones, which no epilogue reads.
+__device__ __forceinline__ bool finish_reduction_n(const double *block_values, int nv, int k0, int nrhs,
+                                                   double *partials, unsigned *ticket, double *red, double *totals)
 {
     __shared__ bool last;
     if (threadIdx.x == 0) {
-        partials[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = block_value;
+        for (int v = 0; v < nv; ++v) partials[(size_t)(k0 + v) * gridDim.x + blockIdx.x] = block_values[v];
         __threadfence();
         last = (atomicAdd(ticket, 1u) == gridDim.x * gridDim.y - 1);
     }
     __syncthreads();
     if (!last) return false;
-    for (unsigned k = 0; k < gridDim.y; ++k) {
+    for (int k = 0; k < nrhs; ++k) {
         double t = 0.0;
         for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x)
             t += __ldcg(partials + (size_t)k * gridDim.x + i);
@@ -53,15 +54,62 @@ __device__ __forceinline__ bool finish_reduction(double block_value, double *par
     __syncthreads();
     return true;
 }
+// one value per block, right-hand side blockIdx.y of gridDim.y
+__device__ __forceinline__ bool finish_reduction(double block_value, double *partials,
+                                                 unsigned *ticket, double *red, double *totals)
+{
+    return finish_reduction_n(&block_value, 1, (int)blockIdx.y, (int)gridDim.y, partials, ticket, red, totals);
+}
+
+// ---- paired fp32 batches (stag_dslash.cuh; include/stag.h "batch layouts") -----------------------
+// The fp32 vectors of a solve with nrhs >= 2 are kept paired: unit u = blockIdx.y of the vector
+// kernels is, for u < nrhs/2, right-hand sides 2u and 2u+1 interleaved per complex number (16-byte
+// packets (re_a, im_a, re_b, im_b), 2n reals starting 2u*n reals in), and, for odd nrhs, one last
+// unit that is the ordinary spinor nrhs-1.  Each half of a packet is updated with the scalars of
+// its own right-hand side; a frozen half is written back unchanged.
+// Position of real i of right-hand side k inside a batch of nrhs spinors of n reals each:
+__host__ __device__ inline size_t batch_index(int k, long i, long n, int nrhs, bool paired)
+{
+    if (!paired || k >= (nrhs / 2) * 2) return (size_t)k * n + i;
+    return (size_t)(k / 2) * 2 * n + (size_t)(i >> 1) * 4 + (size_t)(k & 1) * 2 + (size_t)(i & 1);
+}
 
 // d = r + beta d   (Fig. 1; eq. 3.1 P:L91 when it follows an update).  beta = 0
 // makes it d = r, which is how the iteration starts and restarts.
-template <typename T>
+template <typename T, bool PAIRED = false>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 xpay_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const CgCtrl *__restrict__ ctrl)
 {
-    const int k = blockIdx.y;
-    if (ctrl->state != CG_RUN || !ctrl->active[k]) return;
+    if (ctrl->state != CG_RUN) return;
+    int k = blockIdx.y;
+    if constexpr (PAIRED) {
+        const int npairs = ctrl->nrhs / 2;
+        if ((int)blockIdx.y < npairs) {
+            const int ka = 2 * blockIdx.y, kb = ka + 1;
+            const bool act_a = ctrl->active[ka], act_b = ctrl->active[kb];
+            if (!act_a && !act_b) return;
+            const float beta_a = (float)ctrl->beta[ka], beta_b = (float)ctrl->beta[kb];
+            float4 *dk = reinterpret_cast<float4 *>(d + (size_t)ka * n);
+            const float4 *rk = reinterpret_cast<const float4 *>(r + (size_t)ka * n);
+            const long nv = n / 2;                       // packets of the pair: one complex number of each
+            for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)gridDim.x * BLAS_BLOCK) {
+                const float4 a = ld_keep(rk + i);
+                float4 b = ld_keep(dk + i);
+                if (act_a) {
+                    b.x = (beta_a == 0.f) ? a.x : fma(beta_a, b.x, a.x);
+                    b.y = (beta_a == 0.f) ? a.y : fma(beta_a, b.y, a.y);
+                }
+                if (act_b) {
+                    b.z = (beta_b == 0.f) ? a.z : fma(beta_b, b.z, a.z);
+                    b.w = (beta_b == 0.f) ? a.w : fma(beta_b, b.w, a.w);
+                }
+                st_keep(dk + i, b);
+            }
+            return;
+        }
+        k = 2 * npairs;                                  // the odd last right-hand side, an ordinary spinor
+    }
+    if (!ctrl->active[k]) return;
     using V = typename Vec4<T>::type;
     constexpr int N = Vec4<T>::N;
     const T beta = (T)ctrl->beta[k];
@@ -160,7 +208,7 @@ __device__ __forceinline__ void cg_iteration_epilogue(CgCtrl *__restrict__ ctrl,
 // block of right-hand side k adds the n_hop partials of k in the same order, so all of them use
 // the same alpha and no extra launch or device-wide fence is needed between the hop and this
 // kernel.  A frozen right-hand side (active == 0) is not touched.
-template <typename T>
+template <typename T, bool PAIRED = false>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
               const T *__restrict__ q, long n, const double *__restrict__ hop_partials,
@@ -171,7 +219,58 @@ update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
     constexpr int N = Vec4<T>::N;
     __shared__ double red[32];
     __shared__ double totals[MAX_RHS];
-    const int k = blockIdx.y;
+    const int nrhs = ctrl->nrhs;
+    int k = blockIdx.y;
+    if constexpr (PAIRED) {
+        const int npairs = nrhs / 2;
+        if ((int)blockIdx.y < npairs) {
+            const int ka = 2 * blockIdx.y, kb = ka + 1;
+            const bool act_a = ctrl->active[ka], act_b = ctrl->active[kb];
+            double s2[2] = {0.0, 0.0};
+            if (act_a || act_b) {
+                double ad[2] = {0.0, 0.0};
+                if (act_a) {
+                    const double dAd = block_total_fixed(hop_partials + (size_t)ka * n_hop, n_hop, red);
+                    ad[0] = (dAd > 0.0) ? ctrl->delta[ka] / dAd : 0.0;
+                    if (blockIdx.x == 0 && threadIdx.x == 0) { ctrl->dAd[ka] = dAd; ctrl->alpha[ka] = ad[0]; }
+                }
+                if (act_b) {
+                    const double dAd = block_total_fixed(hop_partials + (size_t)kb * n_hop, n_hop, red);
+                    ad[1] = (dAd > 0.0) ? ctrl->delta[kb] / dAd : 0.0;
+                    if (blockIdx.x == 0 && threadIdx.x == 0) { ctrl->dAd[kb] = dAd; ctrl->alpha[kb] = ad[1]; }
+                }
+                const float al_a = (float)ad[0], al_b = (float)ad[1];        // 0 for a frozen half: y, r unchanged
+                float4 *yk = reinterpret_cast<float4 *>(y + (size_t)ka * n);
+                float4 *rk = reinterpret_cast<float4 *>(r + (size_t)ka * n);
+                const float4 *dk = reinterpret_cast<const float4 *>(d + (size_t)ka * n);
+                const float4 *qk = reinterpret_cast<const float4 *>(q + (size_t)ka * n);
+                const long nv = n / 2;
+                for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)gridDim.x * BLAS_BLOCK) {
+                    float4 yy = ld_pass(yk + i), rr = ld_keep(rk + i);
+                    const float4 dd = ld_keep(dk + i), qq = ld_keep(qk + i);
+                    if (act_a) {
+                        yy.x = fma(al_a, dd.x, yy.x); yy.y = fma(al_a, dd.y, yy.y);
+                        rr.x = fma(-al_a, qq.x, rr.x); rr.y = fma(-al_a, qq.y, rr.y);
+                        s2[0] += (double)rr.x * (double)rr.x + (double)rr.y * (double)rr.y;
+                    }
+                    if (act_b) {
+                        yy.z = fma(al_b, dd.z, yy.z); yy.w = fma(al_b, dd.w, yy.w);
+                        rr.z = fma(-al_b, qq.z, rr.z); rr.w = fma(-al_b, qq.w, rr.w);
+                        s2[1] += (double)rr.z * (double)rr.z + (double)rr.w * (double)rr.w;
+                    }
+                    st_pass(yk + i, yy);
+                    st_keep(rk + i, rr);
+                }
+            }
+            double bs[2];
+            bs[0] = block_sum(s2[0], red);
+            bs[1] = block_sum(s2[1], red);
+            if (!finish_reduction_n(bs, 2, ka, nrhs, partials, &ctrl->ticket[1], red, totals)) return;
+            if (threadIdx.x == 0) cg_iteration_epilogue(ctrl, totals);
+            return;
+        }
+        k = 2 * npairs;
+    }
     double s = 0.0;
     if (ctrl->active[k]) {
         const double dAd = block_total_fixed(hop_partials + (size_t)k * n_hop, n_hop, red);
@@ -201,7 +300,7 @@ update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
         }
     }
     const double bs = block_sum(s, red);
-    if (!finish_reduction(bs, partials, &ctrl->ticket[1], red, totals)) return;
+    if (!finish_reduction_n(&bs, 1, k, nrhs, partials, &ctrl->ticket[1], red, totals)) return;
     if (threadIdx.x != 0) return;
 
     cg_iteration_epilogue(ctrl, totals);
@@ -215,6 +314,25 @@ accumulate_kernel(double *__restrict__ x, T *__restrict__ y, long n)
     for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < n; i += (long)gridDim.x * BLAS_BLOCK) {
         x[i] += (double)y[i];
         y[i] = (T)0;
+    }
+}
+// The same for the pairs of a paired fp32 batch (y) against the blocked fp64 batch (x): one thread
+// per (pair, complex number); npairs*n/2 packets.
+__global__ void __launch_bounds__(BLAS_BLOCK)
+accumulate_paired_kernel(double *__restrict__ x, float *__restrict__ y, long n, int npairs)
+{
+    const long nv = n / 2;
+    float4 *yp = reinterpret_cast<float4 *>(y);
+    for (long t = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; t < nv * npairs; t += (long)gridDim.x * BLAS_BLOCK) {
+        const long j = t / nv, i = t % nv;
+        const float4 v = yp[t];
+        double2 *xa = reinterpret_cast<double2 *>(x + (size_t)(2 * j) * n) + i;
+        double2 *xb = reinterpret_cast<double2 *>(x + (size_t)(2 * j + 1) * n) + i;
+        double2 a = *xa, b = *xb;
+        a.x += (double)v.x; a.y += (double)v.y;
+        b.x += (double)v.z; b.y += (double)v.w;
+        *xa = a; *xb = b;
+        yp[t] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
 }
 
@@ -283,7 +401,7 @@ template <typename T, int WHAT>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 residual_kernel(double *__restrict__ r, const double *__restrict__ b,
                 const double *__restrict__ q, T *__restrict__ r_lo, long n, long n_plane, long n_valid,
-                double *__restrict__ partials, CgCtrl *__restrict__ ctrl)
+                double *__restrict__ partials, CgCtrl *__restrict__ ctrl, const bool lo_paired = false)
 {
     const size_t off = (size_t)blockIdx.y * n;
     double s = 0.0;
@@ -295,7 +413,7 @@ residual_kernel(double *__restrict__ r, const double *__restrict__ b,
         } else {
             const double v = bi - q[off + i];
             r[off + i] = v;
-            if (r_lo != nullptr) r_lo[off + i] = (T)v;
+            if (r_lo != nullptr) r_lo[batch_index((int)blockIdx.y, i, n, (int)gridDim.y, lo_paired)] = (T)v;   // the fp32 copy in its batch layout
             s += v * v;
         }
     }

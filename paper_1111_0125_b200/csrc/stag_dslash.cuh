@@ -162,8 +162,16 @@ __device__ __forceinline__ void wait_flag(const unsigned long long *f, unsigned 
 }
 
 // T: float or double.  NR: storage of each link (3 = 18-real, 2 = 12-real rows 0,1, 1 = 8-parameter).
-// N: right-hand sides handled by one thread; spinor k of a batch starts rs complex numbers after
-// spinor k-1 (rs = 3*Vh_pad: the batch is N device spinors back to back).
+// N: right-hand sides handled by one thread.  Two batch layouts (include/stag.h "batch layouts"):
+//   blocked (PAIRED = false): spinor k of a batch starts rs complex numbers after spinor k-1
+//           (rs = 3*Vh_pad: the batch is N device spinors back to back);
+//   paired  (PAIRED = true, fp32 only): right-hand sides 2j and 2j+1 are interleaved per complex
+//           number, v[j][c][cb] = (re_2j, im_2j, re_2j+1, im_2j+1), one float4 plane triple per pair
+//           (it occupies the 2*rs float2 slots the two spinors would), an odd last right-hand side
+//           is an ordinary spinor after the pairs.  A neighbour colour of a pair is then ONE
+//           16-byte gather instead of two 8-byte ones: half the gather instructions and address
+//           arithmetic of the batch hop, which is bound by issue slots and loads in flight, not
+//           by DRAM.  The arithmetic per right-hand side is unchanged.
 // links: the gathered field of the OUTPUT parity as packets, L[tile][j][lane], packet j holding
 // complex numbers CPP*j .. CPP*j+CPP-1 of the site's run c = d*K + k (d = direction 0..7,
 // k = 3*row+col).  in: the other parity's spinor planes; out / own: this parity's.
@@ -175,7 +183,7 @@ __device__ __forceinline__ void wait_flag(const unsigned long long *f, unsigned 
 // slice come from the halo buffers once their flag shows this exchange's epoch.  Sites are
 // visited rotated by one time slice (slices 1 .. X3-1, then slice 0), so the blocks that may
 // have to wait for a neighbouring GPU run last and the interior overlaps the exchange.
-template <typename T, int NR, int MODE, int N, bool HALO = false>
+template <typename T, int NR, int MODE, int N, bool HALO = false, bool PAIRED = false>
 __global__ void __launch_bounds__(DSLASH_BLOCK, HopTune<T, NR, N>::MINB)
 dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
               const pkt_t<T> *__restrict__ links, const Geom g, const int p, const T a, const T cD,
@@ -183,6 +191,7 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
               const CgCtrl *__restrict__ ctrl, const HaloArgs<T> halo)
 {
     static_assert(!HALO || N == 1, "slab hops carry one right-hand side");
+    static_assert(!PAIRED || (N > 1 && sizeof(T) == 4), "paired batches are fp32 with at least two right-hand sides");
     using C = cplx_t<T>;
     using P = pkt_t<T>;
     constexpr int K = link_slots(NR);
@@ -261,7 +270,7 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
 #pragma unroll
             for (int i = 0; i < KG; ++i) pk[i] = ld_stream(L + (grp * KG + i) * TILE);
             C vg[VGN][VGD][3];
-            if constexpr (N > 1) {
+            if constexpr (N > 1 && !PAIRED) {
 #pragma unroll
                 for (int k = 0; k < N; ++k)
 #pragma unroll
@@ -269,6 +278,25 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
 #pragma unroll
                         for (int c = 0; c < 3; ++c)
                             vg[k][dd][c] = ld_keep_nc(in + k * rs + (size_t)c * g.Vh_pad + s.nbr[grp * DPG + dd]);
+            }
+            if constexpr (PAIRED) {
+#pragma unroll
+                for (int j = 0; j < N / 2; ++j)
+#pragma unroll
+                    for (int dd = 0; dd < DPG; ++dd)
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            const float4 v = ld_keep_nc((const float4 *)(in + 2 * j * rs) + (size_t)c * g.Vh_pad + s.nbr[grp * DPG + dd]);
+                            vg[2 * j][dd][c] = mk<T>(v.x, v.y);
+                            vg[2 * j + 1][dd][c] = mk<T>(v.z, v.w);
+                        }
+                if constexpr (N & 1) {
+#pragma unroll
+                    for (int dd = 0; dd < DPG; ++dd)
+#pragma unroll
+                        for (int c = 0; c < 3; ++c)
+                            vg[N - 1][dd][c] = ld_keep_nc(in + (N - 1) * rs + (size_t)c * g.Vh_pad + s.nbr[grp * DPG + dd]);
+                }
             }
 #pragma unroll
             for (int dd = 0; dd < DPG; ++dd) {
@@ -298,8 +326,35 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
 #pragma unroll
                 for (int i = 0; i < 3; ++i) acc[k][i] = mk<T>(0, 0);
         }
+        if constexpr (PAIRED) {
+            // a pair's three colours leave as three 16-byte stores; its own-site vector arrives the same way
 #pragma unroll
-        for (int k = 0; k < N; ++k) {
+            for (int j = 0; j < N / 2; ++j)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    float4 *po = (float4 *)(out + 2 * j * rs) + (size_t)c * g.Vh_pad + cb;
+                    if (MODE == HOP_PLAIN) {
+                        st_keep(po, make_float4(acc[2 * j][c].x, acc[2 * j][c].y, acc[2 * j + 1][c].x, acc[2 * j + 1][c].y));
+                    } else {
+                        const float4 o = ld_keep_nc((const float4 *)(own + 2 * j * rs) + (size_t)c * g.Vh_pad + cb);
+                        float4 r;
+                        if (MODE == HOP_AXPBY) {
+                            r.x = fma(a, o.x, -cD * acc[2 * j][c].x);     r.y = fma(a, o.y, -cD * acc[2 * j][c].y);
+                            r.z = fma(a, o.z, -cD * acc[2 * j + 1][c].x); r.w = fma(a, o.w, -cD * acc[2 * j + 1][c].y);
+                        } else {
+                            r.x = fma(a, o.x, -acc[2 * j][c].x);     r.y = fma(a, o.y, -acc[2 * j][c].y);
+                            r.z = fma(a, o.z, -acc[2 * j + 1][c].x); r.w = fma(a, o.w, -acc[2 * j + 1][c].y);
+                        }
+                        st_keep(po, r);
+                        if (MODE == HOP_XPAY_DOT) {
+                            dot[2 * j] += (double)o.x * (double)r.x + (double)o.y * (double)r.y;
+                            dot[2 * j + 1] += (double)o.z * (double)r.z + (double)o.w * (double)r.w;
+                        }
+                    }
+                }
+        }
+#pragma unroll
+        for (int k = PAIRED ? (N / 2) * 2 : 0; k < N; ++k) {
             if (MODE == HOP_PLAIN) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) st_keep(out + k * rs + (size_t)c * g.Vh_pad + cb, acc[k][c]);

@@ -22,8 +22,11 @@ struct Solver {
     long n;          // reals per spinor
     int gb;          // blas grid.x (blocks per right-hand side)
     int applies_f64;
+    bool paired;     // the fp32 vectors are a paired batch (nrhs >= 2, fp32 modes)
+    int gb_lo;       // grid.x of the iteration's vector kernels: blocks per unit (pair or single)
 
     dim3 grid2() const { return dim3((unsigned)gb, (unsigned)nrhs); }
+    dim3 grid_lo() const { return dim3((unsigned)gb_lo, (unsigned)(paired ? (nrhs + 1) / 2 : nrhs)); }
 
     // q64 = A x  in fp64 (two hops), outside the iteration
     int apply_A64(const double *x)
@@ -37,7 +40,7 @@ struct Solver {
     template <int WHAT>
     int residual(const double *b, bool lo_copy)
     {
-        residual_kernel<float, WHAT><<<grid2(), BLAS_BLOCK, 0, s>>>(w.r64, b, w.q64, lo_copy ? w.r32 : nullptr, n, 2L * L->g.Vh_pad, 2L * L->g.Vh, w.partials, w.ctrl);
+        residual_kernel<float, WHAT><<<grid2(), BLAS_BLOCK, 0, s>>>(w.r64, b, w.q64, lo_copy ? w.r32 : nullptr, n, 2L * L->g.Vh_pad, 2L * L->g.Vh, w.partials, w.ctrl, paired);
         count_launch();
         KCHECK();
         return STAG_OK;
@@ -45,9 +48,22 @@ struct Solver {
 
     int accumulate(double *x)
     {
-        accumulate_kernel<float><<<blas_grid(n * nrhs, 1), BLAS_BLOCK, 0, s>>>(x, w.y32, n * nrhs);
+        if (!paired) {
+            accumulate_kernel<float><<<blas_grid(n * nrhs, 1), BLAS_BLOCK, 0, s>>>(x, w.y32, n * nrhs);
+            count_launch();
+            KCHECK();
+            return STAG_OK;
+        }
+        const int npairs = nrhs / 2;
+        accumulate_paired_kernel<<<blas_grid(n * npairs, 1), BLAS_BLOCK, 0, s>>>(x, w.y32, n, npairs);
         count_launch();
         KCHECK();
+        if (nrhs & 1) {
+            const size_t off = (size_t)(nrhs - 1) * n;
+            accumulate_kernel<float><<<blas_grid(n, 1), BLAS_BLOCK, 0, s>>>(x + off, w.y32 + off, n);
+            count_launch();
+            KCHECK();
+        }
         return STAG_OK;
     }
 
@@ -56,14 +72,18 @@ struct Solver {
     template <typename T>
     int iteration(T *y, T *r, T *d, T *q, T *tmp, cudaStream_t st)
     {
-        xpay_kernel<T><<<grid2(), BLAS_BLOCK, 0, st>>>(d, r, n, w.ctrl);                     // d = r + beta d
+        constexpr bool F32 = std::is_same<T, float>::value;
+        const int layout = (F32 && paired) ? STAG_BATCH_PAIRED : STAG_BATCH_BLOCKED;
+        if (F32 && paired) xpay_kernel<float, true><<<grid_lo(), BLAS_BLOCK, 0, st>>>((float *)d, (const float *)r, n, w.ctrl);
+        else xpay_kernel<T><<<grid_lo(), BLAS_BLOCK, 0, st>>>(d, r, n, w.ctrl);             // d = r + beta d
         count_launch();
         KCHECK();
-        int rc = launch_hop(L, prec_lo, HOP_PLAIN, tmp, d, 1, 0.0, 1.0, nullptr, nullptr, w.ctrl, nrhs, st);   // D_oe d
+        int rc = launch_hop(L, prec_lo, HOP_PLAIN, tmp, d, 1, 0.0, 1.0, nullptr, nullptr, w.ctrl, nrhs, st, layout);   // D_oe d
         if (rc) return rc;
-        rc = launch_hop(L, prec_lo, HOP_XPAY_DOT, q, tmp, 0, m2, 1.0, d, w.hop_partials, w.ctrl, nrhs, st);  // q = A d, <d,q>
+        rc = launch_hop(L, prec_lo, HOP_XPAY_DOT, q, tmp, 0, m2, 1.0, d, w.hop_partials, w.ctrl, nrhs, st, layout);  // q = A d, <d,q>
         if (rc) return rc;
-        update_kernel<T><<<grid2(), BLAS_BLOCK, 0, st>>>(y, r, d, q, n, w.hop_partials, w.n_hop, w.partials, w.ctrl);  // alpha, y, r, delta, beta
+        if (F32 && paired) update_kernel<float, true><<<grid_lo(), BLAS_BLOCK, 0, st>>>((float *)y, (float *)r, (const float *)d, (const float *)q, n, w.hop_partials, w.n_hop, w.partials, w.ctrl);
+        else update_kernel<T><<<grid_lo(), BLAS_BLOCK, 0, st>>>(y, r, d, q, n, w.hop_partials, w.n_hop, w.partials, w.ctrl);  // alpha, y, r, delta, beta
         count_launch();
         KCHECK();
         return STAG_OK;
@@ -108,6 +128,8 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
     S.n = (long)6 * L->g.Vh_pad;
     S.gb = blas_grid(S.n, nrhs);
     S.applies_f64 = 0;
+    S.paired = (mode != STAG_CG_F64) && nrhs >= 2;
+    S.gb_lo = S.paired ? blas_grid(2 * S.n, (nrhs + 1) / 2) : S.gb;
     int rc;
     if ((rc = ensure_links(L, S.prec_lo))) return rc;
     if ((rc = ensure_links(L, S.prec_hi))) return rc;

@@ -267,7 +267,7 @@ int ensure_links_locked(const stag_links *L, int prec)
 }
 
 // ---- Dslash launcher ---------------------------------------------------------------------
-template <typename T, int NR, int N>
+template <typename T, int NR, int N, bool PAIRED>
 int launch_hop_n(const stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx_t<T> *in,
                  int parity, double a, double cD, const cplx_t<T> *own, double *partials,
                  const CgCtrl *ctrl, cudaStream_t s)
@@ -278,19 +278,19 @@ int launch_hop_n(const stag_links *L, int prec, int hop, cplx_t<T> *out, const c
     const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
     switch (hop) {
     case HOP_PLAIN:
-        dslash_kernel<T, NR, HOP_PLAIN, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl, HaloArgs<T>{});
+        dslash_kernel<T, NR, HOP_PLAIN, N, false, PAIRED><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl, HaloArgs<T>{});
         break;
     case HOP_XPAY:
-        dslash_kernel<T, NR, HOP_XPAY, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl, HaloArgs<T>{});
+        dslash_kernel<T, NR, HOP_XPAY, N, false, PAIRED><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl, HaloArgs<T>{});
         break;
     case HOP_AXPBY:   // only the fp64 wrapper steps use it
         if constexpr (std::is_same<T, double>::value)
-            dslash_kernel<T, NR, HOP_AXPBY, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl, HaloArgs<T>{});
+            dslash_kernel<T, NR, HOP_AXPBY, N, false, PAIRED><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl, HaloArgs<T>{});
         else
             return STAG_EINVAL;
         break;
     default:
-        dslash_kernel<T, NR, HOP_XPAY_DOT, N><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl, HaloArgs<T>{});
+        dslash_kernel<T, NR, HOP_XPAY_DOT, N, false, PAIRED><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (T)a, (T)cD, own, partials, ctrl, HaloArgs<T>{});
         break;
     }
     count_launch();
@@ -299,12 +299,16 @@ int launch_hop_n(const stag_links *L, int prec, int hop, cplx_t<T> *out, const c
 }
 
 // nrhs right-hand sides in chunks of at most HopMaxRhs<T>: each chunk is one pass over the links.
+// layout: STAG_BATCH_BLOCKED or STAG_BATCH_PAIRED (fp32 only; a chunk starts at an even right-hand
+// side, so chunk k0 of a paired batch begins k0*rs complex numbers in, like a blocked one).
 template <typename T, int NR>
 int launch_hop_t(const stag_links *L, int prec, int hop, cplx_t<T> *out, const cplx_t<T> *in,
                  int parity, double a, double cD, const cplx_t<T> *own, double *partials,
-                 const CgCtrl *ctrl, int nrhs, cudaStream_t s)
+                 const CgCtrl *ctrl, int nrhs, int layout, cudaStream_t s)
 {
     constexpr int NB = HopMaxRhs<T>::value;
+    constexpr bool F32 = std::is_same<T, float>::value;
+    if (layout != STAG_BATCH_BLOCKED && !(F32 && layout == STAG_BATCH_PAIRED)) return STAG_EINVAL;
     const size_t rs = (size_t)3 * L->g.Vh_pad;
     const size_t n_hop = ((size_t)L->g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK;
     for (int k0 = 0; k0 < nrhs; k0 += NB) {
@@ -314,11 +318,20 @@ int launch_hop_t(const stag_links *L, int prec, int hop, cplx_t<T> *out, const c
         const cplx_t<T> *w = own ? own + k0 * rs : nullptr;
         double *pp = partials ? partials + k0 * n_hop : nullptr;
         int rc = STAG_EINVAL;
-        if (nb == 1) rc = launch_hop_n<T, NR, 1>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
-        if (nb == 2) rc = launch_hop_n<T, NR, 2>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+        if (nb == 1) rc = launch_hop_n<T, NR, 1, false>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+        if constexpr (F32) {
+            if (layout == STAG_BATCH_PAIRED) {
+                if (nb == 2) rc = launch_hop_n<T, NR, 2, true>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+                if (nb == 3) rc = launch_hop_n<T, NR, 3, true>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+                if (nb == 4) rc = launch_hop_n<T, NR, 4, true>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+                if (rc) return rc;
+                continue;
+            }
+        }
+        if (nb == 2) rc = launch_hop_n<T, NR, 2, false>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
         if constexpr (NB >= 4) {
-            if (nb == 3) rc = launch_hop_n<T, NR, 3>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
-            if (nb == 4) rc = launch_hop_n<T, NR, 4>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+            if (nb == 3) rc = launch_hop_n<T, NR, 3, false>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+            if (nb == 4) rc = launch_hop_n<T, NR, 4, false>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
         }
         if (rc) return rc;
     }
@@ -327,21 +340,21 @@ int launch_hop_t(const stag_links *L, int prec, int hop, cplx_t<T> *out, const c
 
 int launch_hop(const stag_links *L, int prec, int hop, void *out, const void *in, int parity,
                double a, double cD, const void *own, double *partials, const CgCtrl *ctrl,
-               int nrhs, cudaStream_t s)
+               int nrhs, cudaStream_t s, int layout = STAG_BATCH_BLOCKED)
 {
     switch (prec) {
     case STAG_PREC_F64:
-        return launch_hop_t<double, 3>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, cD, (const double2 *)own, partials, ctrl, nrhs, s);
+        return launch_hop_t<double, 3>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, cD, (const double2 *)own, partials, ctrl, nrhs, layout, s);
     case STAG_PREC_F32:
-        return launch_hop_t<float, 3>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, cD, (const float2 *)own, partials, ctrl, nrhs, s);
+        return launch_hop_t<float, 3>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, cD, (const float2 *)own, partials, ctrl, nrhs, layout, s);
     case STAG_PREC_F64_R12:
-        return launch_hop_t<double, 2>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, cD, (const double2 *)own, partials, ctrl, nrhs, s);
+        return launch_hop_t<double, 2>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, cD, (const double2 *)own, partials, ctrl, nrhs, layout, s);
     case STAG_PREC_F32_R12:
-        return launch_hop_t<float, 2>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, cD, (const float2 *)own, partials, ctrl, nrhs, s);
+        return launch_hop_t<float, 2>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, cD, (const float2 *)own, partials, ctrl, nrhs, layout, s);
     case STAG_PREC_F64_R8:
-        return launch_hop_t<double, 1>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, cD, (const double2 *)own, partials, ctrl, nrhs, s);
+        return launch_hop_t<double, 1>(L, prec, hop, (double2 *)out, (const double2 *)in, parity, a, cD, (const double2 *)own, partials, ctrl, nrhs, layout, s);
     case STAG_PREC_F32_R8:
-        return launch_hop_t<float, 1>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, cD, (const float2 *)own, partials, ctrl, nrhs, s);
+        return launch_hop_t<float, 1>(L, prec, hop, (float2 *)out, (const float2 *)in, parity, a, cD, (const float2 *)own, partials, ctrl, nrhs, layout, s);
     }
     return STAG_EINVAL;
 }
@@ -516,16 +529,72 @@ extern "C" int stag_spinor_unpack(double *dst, const void *src, const int dims[4
 // ------------------------------------------------------------------------------------
 // C ABI: the operator
 // ------------------------------------------------------------------------------------
-extern "C" int stag_dslash_mrhs(void *out, const void *in, const stag_links_t *links, int parity,
-                                const int dims[4], int prec, int nrhs)
+extern "C" int stag_dslash_batch(void *out, const void *in, const stag_links_t *links, int parity,
+                                 const int dims[4], int prec, int nrhs, int layout)
 {
     const stag_links *L = links;
     if (!out || !in || !L || out == in || (parity & ~1) || !prec_ok(prec) || !same_dims(L, dims) ||
         nrhs < 1 || L->is_slab)      // a slab's hop needs its halo: stag_slab_hop
         return STAG_EINVAL;
+    if (layout != STAG_BATCH_BLOCKED && !(layout == STAG_BATCH_PAIRED && prec_is_f32(prec))) return STAG_EINVAL;
     int rc = ensure_links(L, prec);
     if (rc) return rc;
-    return launch_hop(L, prec, HOP_PLAIN, out, in, parity, 0.0, 1.0, nullptr, nullptr, nullptr, nrhs, t_stream);
+    return launch_hop(L, prec, HOP_PLAIN, out, in, parity, 0.0, 1.0, nullptr, nullptr, nullptr, nrhs, t_stream, layout);
+}
+
+extern "C" int stag_dslash_mrhs(void *out, const void *in, const stag_links_t *links, int parity,
+                                const int dims[4], int prec, int nrhs)
+{
+    return stag_dslash_batch(out, in, links, parity, dims, prec, nrhs, STAG_BATCH_BLOCKED);
+}
+
+// blocked <-> paired: rhs 2j, 2j+1 of an fp32 batch interleaved per complex number
+__global__ void __launch_bounds__(256)
+batch_convert_kernel(float4 *__restrict__ dst, const float4 *__restrict__ src, long rs, int npairs, int to_paired)
+{
+    // one thread per (pair, complex index i): blocked holds a[i] at 2j*rs + i and b[i] at (2j+1)*rs + i
+    // (float2 units); paired holds (a[i], b[i]) as the float4 number i of the pair.  Two complex
+    // numbers per thread so that both sides move 16-byte packets (rs is even).
+    const long half = rs / 2;
+    const long t = blockIdx.x * 256L + threadIdx.x;
+    if (t >= (long)npairs * half) return;
+    const long j = t / half, i2 = t % half;                 // complex numbers 2*i2, 2*i2+1
+    const float4 *sj = src + j * rs;                        // the pair's 2*rs float2 = rs float4
+    float4 *dj = dst + j * rs;
+    if (to_paired) {
+        const float4 a = sj[i2], b = sj[half + i2];         // a[2i2], a[2i2+1] ; b[2i2], b[2i2+1]
+        dj[2 * i2] = make_float4(a.x, a.y, b.x, b.y);
+        dj[2 * i2 + 1] = make_float4(a.z, a.w, b.z, b.w);
+    } else {
+        const float4 p = sj[2 * i2], q = sj[2 * i2 + 1];
+        dj[i2] = make_float4(p.x, p.y, q.x, q.y);
+        dj[half + i2] = make_float4(p.z, p.w, q.z, q.w);
+    }
+}
+
+extern "C" int stag_batch_convert(void *dst, const void *src, const int dims[4], int prec, int nrhs,
+                                  int to_layout)
+{
+    Geom g;
+    if (!dst || !src || dst == src || !prec_ok(prec) || !make_geom(g, dims, 0) || nrhs < 1 ||
+        (to_layout != STAG_BATCH_BLOCKED && to_layout != STAG_BATCH_PAIRED))
+        return STAG_EINVAL;
+    const size_t sb = stag_spinor_bytes(dims, prec);
+    if (!prec_is_f32(prec)) {     // fp64 batches have one layout
+        CU(cudaMemcpyAsync(dst, src, sb * nrhs, cudaMemcpyDeviceToDevice, t_stream));
+        return STAG_OK;
+    }
+    const long rs = 3L * g.Vh_pad;
+    const int npairs = nrhs / 2;
+    if (npairs) {
+        const long n = (long)npairs * (rs / 2);
+        batch_convert_kernel<<<(unsigned)((n + 255) / 256), 256, 0, t_stream>>>((float4 *)dst, (const float4 *)src, rs, npairs, to_layout == STAG_BATCH_PAIRED);
+        count_launch();
+        KCHECK();
+    }
+    if (nrhs & 1)                 // the odd last right-hand side is an ordinary spinor in both layouts
+        CU(cudaMemcpyAsync((char *)dst + sb * (nrhs - 1), (const char *)src + sb * (nrhs - 1), sb, cudaMemcpyDeviceToDevice, t_stream));
+    return STAG_OK;
 }
 
 extern "C" int stag_dslash(void *out, const void *in, const stag_links_t *links, int parity,
@@ -534,12 +603,13 @@ extern "C" int stag_dslash(void *out, const void *in, const stag_links_t *links,
     return stag_dslash_mrhs(out, in, links, parity, dims, prec, 1);
 }
 
-extern "C" int stag_apply_A_mrhs(void *out_even, const void *in_even, const stag_links_t *links,
-                                 double mass, int prec, int nrhs)
+extern "C" int stag_apply_A_batch(void *out_even, const void *in_even, const stag_links_t *links,
+                                  double mass, int prec, int nrhs, int layout)
 {
     const stag_links *L = links;
     if (!out_even || !in_even || !L || out_even == in_even || !prec_ok(prec) || nrhs < 1 || nrhs > MAX_RHS || L->is_slab)
         return STAG_EINVAL;
+    if (layout != STAG_BATCH_BLOCKED && !(layout == STAG_BATCH_PAIRED && prec_is_f32(prec))) return STAG_EINVAL;
     int rc = ensure_links(L, prec);
     if (rc) return rc;
     // the odd-site intermediate lives in the workspace (the caller's, or the handle's own)
@@ -548,8 +618,14 @@ extern "C" int stag_apply_A_mrhs(void *out_even, const void *in_even, const stag
     if ((rc = lease_workspace(L, lay.total, lease))) return rc;
     void *tmp_odd = lease.ws->base + lay.scratch;
     // tmp_o = D_oe in_e ;  out_e = m^2 in_e - D_eo tmp_o      (eq. 2.3)
-    if ((rc = launch_hop(L, prec, HOP_PLAIN, tmp_odd, in_even, 1, 0.0, 1.0, nullptr, nullptr, nullptr, nrhs, t_stream))) return rc;
-    return launch_hop(L, prec, HOP_XPAY, out_even, tmp_odd, 0, mass * mass, 1.0, in_even, nullptr, nullptr, nrhs, t_stream);
+    if ((rc = launch_hop(L, prec, HOP_PLAIN, tmp_odd, in_even, 1, 0.0, 1.0, nullptr, nullptr, nullptr, nrhs, t_stream, layout))) return rc;
+    return launch_hop(L, prec, HOP_XPAY, out_even, tmp_odd, 0, mass * mass, 1.0, in_even, nullptr, nullptr, nrhs, t_stream, layout);
+}
+
+extern "C" int stag_apply_A_mrhs(void *out_even, const void *in_even, const stag_links_t *links,
+                                 double mass, int prec, int nrhs)
+{
+    return stag_apply_A_batch(out_even, in_even, links, mass, prec, nrhs, STAG_BATCH_BLOCKED);
 }
 
 extern "C" int stag_apply_A(void *out_even, const void *in_even, const stag_links_t *links,

@@ -91,6 +91,19 @@ __device__ __forceinline__ double2 ld_keep_nc(const double2 *p)
 #endif
 }
 
+// a pair of right-hand sides interleaved per complex number (stag_dslash.cuh, "paired" batches)
+__device__ __forceinline__ float4 ld_keep_nc(const float4 *p)
+{
+#if STAG_SPINOR_POLICY == 0
+    return __ldg(p);
+#else
+    float4 v;
+    asm("ld.global.nc.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+        : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(policy_evict_last()));
+    return v;
+#endif
+}
+
 // coherent loads (the buffer may be written by this kernel)
 __device__ __forceinline__ float2 ld_keep(const float2 *p)
 {
