@@ -2,6 +2,7 @@
 """bench.py -- the headline measurement of the staggered mixed-precision CG hot path.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config NAME]
+                    [--only all|hops] [--cpu-full] [--no-cpu-baseline] [--decomp replicas|slabs]
 
 One STEP = one full mixed-precision CG solve (mode 3: fp32 iteration on 12-real compressed
 links -- the paper's single-precision kernel also reads compressed links, P:L113 -- with the
@@ -17,6 +18,9 @@ solve through stag_cg_solve_host with b and x in pinned HOST memory (copies insi
 region; the gauge field stays resident, as it does across the many solves of one
 configuration).  The dominant kernel (fp32 Dslash) is timed alone for the roofline.
 
+--only hops skips the solves and times the stand-alone hops alone (what the ncu captures under
+profiles/ run); --cpu-full also runs the oracle's complete fp64 solve on the bench config (minutes).
+
 --impl reference times the CPU oracle (oracle/) as it stands on the host cores on a bounded
 sample (a fixed number of CG iterations of the same workload).
 With N > 1 (torchrun) the path does not shard on this single-GPU design: N independent
@@ -25,8 +29,10 @@ replicas, weak scaling, no data-path collective.
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
+import re
 import statistics
 import subprocess
 import sys
@@ -101,6 +107,50 @@ class ClockSampler:
         return out
 
 
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.lower().startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def kernel_source_sha():
+    """Identifies the build of the hop: sha256 over the device headers the hop is made of."""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1111_0125_b200", "csrc")
+    for name in ("stag_common.cuh", "stag_mem.cuh", "stag_dslash.cuh"):
+        h.update(open(os.path.join(d, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def traffic_from_profiles(kernel_tag: str, config: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+    newest profiles/*_ncu_full.md whose header lines
+        traffic_kernel = <tag> / traffic_config = <config> / traffic_source_sha = <kernel_source_sha()>
+        traffic_bytes_per_launch = <bytes>
+    match this build; None (and why) otherwise -- never a number typed in from an older kernel."""
+    pdir = os.path.join(ROOT, "profiles")
+    sha = kernel_source_sha()
+    best = None
+    try:
+        names = sorted(n for n in os.listdir(pdir) if n.endswith("_ncu_full.md"))
+    except OSError:
+        names = []
+    for n in names:
+        kv = dict(re.findall(r"^(traffic_\w+)\s*=\s*(.+?)\s*$", open(os.path.join(pdir, n)).read(), flags=re.M))
+        if kv.get("traffic_kernel") == kernel_tag and kv.get("traffic_config") == config and kv.get("traffic_source_sha") == sha:
+            try:
+                best = (float(kv["traffic_bytes_per_launch"]), "profiles/" + n)
+            except (KeyError, ValueError):
+                pass
+    if best:
+        return best[0], best[1] + " (dram__bytes_read.sum + dram__bytes_write.sum, one launch, same kernel sources)"
+    return None, "no ncu --set full capture under profiles/ matches this build of the hop (source sha %s)" % sha
+
+
 def host_threads():
     try:
         return len(os.sched_getaffinity(0))
@@ -121,6 +171,59 @@ def oracle_sample(cfg, W, b, target_seconds: float):
     return {"iters": it, "seconds": dt, "gflops": it * FLOP_PER_SITE_ITER * cfg.vh / dt * 1e-9}
 
 
+def oracle_hop(cfg, W, b):
+    """One oracle Dslash hop, best of 5 after one warm-up."""
+    import oracle
+    oracle.dslash(b, W, cfg.dims, 1)
+    best = float("inf")
+    for _ in range(5):
+        t0 = time.perf_counter()
+        oracle.dslash(b, W, cfg.dims, 1)
+        best = min(best, time.perf_counter() - t0)
+    return {"seconds": best, "gflops": FLOP_PER_SITE_HOP * cfg.vh / best * 1e-9,
+            "paper_convention_gbs": 1584 * cfg.vh / best * 1e-9}
+
+
+def oracle_solve(cfg, W, b):
+    """The oracle's complete fp64 solve (Fig. 1) to the config's tolerance."""
+    import oracle
+    t0 = time.perf_counter()
+    _, it, rho, restarts, rc = oracle.cg(b, W, cfg.dims, cfg.mass, cfg.tol, cfg.maxiter)
+    dt = time.perf_counter() - t0
+    return {"seconds": dt, "iters": it, "true_resid": rho, "restarts": restarts, "status": rc, "kind": "measured",
+            "gflops": it * FLOP_PER_SITE_ITER * cfg.vh / dt * 1e-9}
+
+
+def cpu_baseline_block(cfg, W, b, full: bool, iters_fp64=None):
+    """cpu_baseline of the JSON line: the oracle as it stands (same source; built -O3 -march=native
+    on this host for the timing) on a bounded CG sample of the bench
+    workload, plus one hop (best of 5) and the complete fp64 solve -- measured on the configs the
+    oracle finishes in seconds and with --cpu-full, otherwise extrapolated from the sample and
+    labelled so."""
+    import fieldgen
+    import oracle
+    flags = oracle.use_native_build()
+    threads = oracle.max_threads()
+    r = oracle_sample(cfg, W, b, 15.0)
+    cpu = {"value": r["gflops"], "unit": UNIT, "cores": threads, "kind": "oracle",
+           "sample": "%d oracle CG iterations (Fig. 1, fp64) on %s, %.1f s" % (r["iters"], cfg.name, r["seconds"]),
+           "threads": threads, "nproc": os.cpu_count(), "affinity": host_threads(), "cpu_model": cpu_model(),
+           "compile_flags": " ".join(flags), "hop": oracle_hop(cfg, W, b)}
+    if full:
+        cpu["solve"] = oracle_solve(cfg, W, b)
+    elif iters_fp64:
+        per_it = r["seconds"] / max(1, r["iters"])
+        cpu["solve"] = {"seconds": per_it * iters_fp64, "iters": iters_fp64, "kind": "extrapolated: sample seconds per iteration x the %d iterations the GPU's fp64 CG needed (run with --cpu-full to measure)" % iters_fp64}
+    others = {}
+    for name in ("c1_4^4", "c2_8^4", "c3_16^3x32"):
+        if name == cfg.name:
+            continue
+        c = fieldgen.CONFIGS[name]
+        Wc, bc = c.links(), c.source()
+        others[name] = {"hop": oracle_hop(c, Wc, bc), "solve": oracle_solve(c, Wc, bc)}
+    return cpu, others
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle on the host cores, same metric / config."""
     import fieldgen
@@ -128,8 +231,10 @@ def run_reference(args):
     rank, _, world = replicas.env_world()
     if rank != 0:
         return 0
+    import oracle
     cfg = fieldgen.CONFIGS[args.config]
     W, b = cfg.links(), cfg.source()
+    flags = oracle.use_native_build()
     per_step = 6.0
     for _ in range(args.warmup):
         oracle_sample(cfg, W, b, 1.0)
@@ -138,14 +243,16 @@ def run_reference(args):
         r = oracle_sample(cfg, W, b, per_step)
         t_tot += r["seconds"]; it_tot += r["iters"]
     value = it_tot * FLOP_PER_SITE_ITER * cfg.vh / t_tot * 1e-9
-    cores = host_threads()
+    cores = oracle.max_threads()
     sample = "%d oracle CG iterations (Fig. 1, fp64) per step on %s, plus the initial and final residual" % (it_tot // max(1, args.steps), cfg.name)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_tot / max(1, args.steps) * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": workload_config(cfg, args.gpus, sample=sample),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                         "threads": cores, "nproc": os.cpu_count(), "affinity": host_threads(),
+                         "cpu_model": cpu_model(), "compile_flags": " ".join(flags)},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -163,27 +270,39 @@ def workload_config(cfg, n_gpus, **extra):
     return c
 
 
-def time_dslash(stag, torch, fieldgen, cfg, L, prec, launches=60, nrot=6):
-    """Average device time of one Dslash hop launched alone, CUDA events on the launch stream.
-    nrot input/output spinors rotate so neither they nor the links can live in L2."""
+def _time_batches(torch, launch, warmups=10, batches=12, per_batch=10):
+    """10 warm-up launches, then >= 100 timed ones; CUDA events on the
+    launch stream around batches of 10 back-to-back launches (an event pair per launch would add
+    its own ~2 us to a 70 us kernel); returns (median, mean) seconds per launch over the batches."""
+    for i in range(warmups):
+        launch(i)
+    torch.cuda.synchronize()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(batches + 1)]
+    k = warmups
+    evs[0].record()
+    for bi in range(batches):
+        for _ in range(per_batch):
+            launch(k)
+            k += 1
+        evs[bi + 1].record()
+    torch.cuda.synchronize()
+    per = [evs[i].elapsed_time(evs[i + 1]) * 1e-3 / per_batch for i in range(batches)]
+    return statistics.median(per), sum(per) / len(per)
+
+
+def time_dslash(stag, torch, fieldgen, cfg, L, prec, nrot=6):
+    """Device time of one Dslash hop launched alone.  nrot input/output spinors rotate so neither
+    they nor the links can live in L2."""
     ins = [stag.spinor_pack(fieldgen.spinor_gaussian(cfg.dims, 0, seed=100 + i), cfg.dims, prec) for i in range(nrot)]
     outs = [stag.empty_spinor(cfg.dims, prec) for _ in range(nrot)]
-    for i in range(5):
-        stag.dslash(ins[i % nrot], L, 1, prec, out=outs[i % nrot])
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for i in range(launches):
-        stag.dslash(ins[i % nrot], L, 1, prec, out=outs[i % nrot])
-    e1.record()
-    torch.cuda.synchronize()
-    sec = e0.elapsed_time(e1) * 1e-3 / launches
+    sec, mean = _time_batches(torch, lambda i: stag.dslash(ins[i % nrot], L, 1, prec, out=outs[i % nrot]))
     f32 = prec in (stag.PREC_F32, stag.PREC_F32_R12, stag.PREC_F32_R8)
     reals = {stag.PREC_F64: 18, stag.PREC_F32: 18, stag.PREC_F64_R12: 12, stag.PREC_F32_R12: 12,
              stag.PREC_F64_R8: 8, stag.PREC_F32_R8: 8}[prec]
     bytes_site = (8 * reals + 6 + 6) * (4 if f32 else 8)        # 8 links + 1 vector in + 1 out
     paper_bytes = (8 * 18 + 8 * 6 + 6) * (4 if f32 else 8)      # P:L62 convention, no reuse
-    return {"us": sec * 1e6, "algorithmic_bytes_per_site": bytes_site,
+    return {"us": sec * 1e6, "us_mean": mean * 1e6, "timing": "median of 12 batches of 10 launches after 10 warm-ups",
+            "algorithmic_bytes_per_site": bytes_site,
             "gbs": bytes_site * cfg.vh / sec * 1e-9, "gflops": FLOP_PER_SITE_HOP * cfg.vh / sec * 1e-9,
             "paper_convention_gbs": paper_bytes * cfg.vh / sec * 1e-9}
 
@@ -194,24 +313,49 @@ def time_dslash_mrhs(stag, torch, fieldgen, cfg, L, prec, nrhs, launches=30, nro
     srcs = [fieldgen.spinor_gaussian(cfg.dims, 0, seed=300 + k) for k in range(nrhs)]
     ins = [stag.batch_convert(stag.spinor_pack_mrhs(srcs, cfg.dims, prec), cfg.dims, prec, layout) for _ in range(nrot)]
     outs = [torch.empty_like(ins[0]) for _ in range(nrot)]
-    for i in range(3):
-        stag.dslash_mrhs(ins[i % nrot], L, 1, prec, out=outs[i % nrot], layout=layout)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for i in range(launches):
-        stag.dslash_mrhs(ins[i % nrot], L, 1, prec, out=outs[i % nrot], layout=layout)
-    e1.record()
-    torch.cuda.synchronize()
-    sec = e0.elapsed_time(e1) * 1e-3 / launches
+    sec, mean = _time_batches(torch, lambda i: stag.dslash_mrhs(ins[i % nrot], L, 1, prec, out=outs[i % nrot], layout=layout))
     f32 = prec in (stag.PREC_F32, stag.PREC_F32_R12)
     rows = 2 if prec in (stag.PREC_F64_R12, stag.PREC_F32_R12) else 3
     sz = 4 if f32 else 8
     chunks = -(-nrhs // (4 if f32 else 2))
     bytes_site = (chunks * 8 * 6 * rows + nrhs * 12) * sz       # links once per chunk + in/out per rhs
-    return {"nrhs": nrhs, "us": sec * 1e6, "us_per_rhs": sec * 1e6 / nrhs,
+    return {"nrhs": nrhs, "us": sec * 1e6, "us_mean": mean * 1e6, "us_per_rhs": sec * 1e6 / nrhs,
             "algorithmic_bytes_per_site": bytes_site, "gbs": bytes_site * cfg.vh / sec * 1e-9,
             "gflops": FLOP_PER_SITE_HOP * nrhs * cfg.vh / sec * 1e-9}
+
+
+def hop_timings(stag, torch, fieldgen, cfg, L, select=None):
+    """Stand-alone hops: the six single forms and the batch hops.  select: names to run (--hops),
+    e.g. {"fp32/12", "fp32/12 x4"}; None = all."""
+    want = (lambda name: True) if not select else (lambda name: name in select)
+    dsl = {stag.PREC_NAMES[p]: time_dslash(stag, torch, fieldgen, cfg, L, p) for p in range(4) if want(stag.PREC_NAMES[p])}
+    for p in (stag.PREC_F64_R8, stag.PREC_F32_R8):      # refused on fields with nearly-unit links (DESIGN.md section 15)
+        if not want(stag.PREC_NAMES[p]):
+            continue
+        try:
+            dsl[stag.PREC_NAMES[p]] = time_dslash(stag, torch, fieldgen, cfg, L, p)
+            dsl[stag.PREC_NAMES[p]]["rebuilt_entry_error"] = L.recon8_error(p)
+        except stag.StagError as e:
+            dsl[stag.PREC_NAMES[p]] = {"refused": str(e)}
+    f32 = (stag.PREC_F32, stag.PREC_F32_R12)
+    batch = {"%s x%d" % (stag.PREC_NAMES[p], n): time_dslash_mrhs(stag, torch, fieldgen, cfg, L, p, n, layout=stag.BATCH_PAIRED if p in f32 else 0)
+             for p, n in ((stag.PREC_F32_R12, 2), (stag.PREC_F32_R12, 3), (stag.PREC_F32_R12, 4), (stag.PREC_F32, 4), (stag.PREC_F64, 2))
+             if want("%s x%d" % (stag.PREC_NAMES[p], n))}
+    blocked = {"%s x%d" % (stag.PREC_NAMES[p], n): time_dslash_mrhs(stag, torch, fieldgen, cfg, L, p, n)
+               for p, n in ((stag.PREC_F32_R12, 3), (stag.PREC_F32_R12, 4), (stag.PREC_F32, 4))
+               if want("%s x%d blocked" % (stag.PREC_NAMES[p], n))}
+    return dsl, batch, blocked
+
+
+def roofline_block(dsl, cfg, peak, peak_src):
+    dom = dsl["fp32/12"]
+    traffic, traffic_src = traffic_from_profiles("dslash_kernel<float,2,HOP_PLAIN,1>", cfg.name)
+    return {"bound": "hbm", "kernel": "dslash_kernel<float,2,*> (fp32, 12-real links: the hop of the timed solve)",
+            "achieved": dom["gbs"], "peak": peak, "unit": "GB/s", "frac": dom["gbs"] / peak,
+            "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
+            "algorithmic_bytes_per_launch": dom["algorithmic_bytes_per_site"] * cfg.vh,
+            "us_per_launch": dom["us"], "us_per_launch_mean": dom["us_mean"], "timing": dom["timing"],
+            "frac_of_nominal_8TBs": dom["gbs"] / 8000.0}
 
 
 def run_ours(args):
@@ -240,9 +384,37 @@ def run_ours(args):
     L = stag.Links(cfg.dims, W)
     torch.cuda.synchronize()
     setup_s = time.perf_counter() - t0
+
+    if args.only == "hops":                      # what the ncu captures under profiles/ run
+        if rank == 0:
+            select = set(v.strip() for v in args.hops.split(",")) if args.hops else None
+            dsl, batch, blocked = hop_timings(stag, torch, fieldgen, cfg, L, select)
+            out = {"only": "hops", "config": {"workload": cfg.name}, "dslash": dsl,
+                   "mrhs_dslash": batch, "mrhs_dslash_blocked_layout": blocked}
+            if "fp32/12" in dsl:
+                out["roofline"] = roofline_block(dsl, cfg, peak, peak_src)
+            print(json.dumps(out), flush=True)
+        replicas.finalize()
+        return 0
+
+    if args.only == "mrhs":
+        if rank == 0:
+            b3 = stag.spinor_pack_mrhs([fieldgen.spinor_gaussian(cfg.dims, 0, seed + 1000 + k) for k in range(3)],
+                                       cfg.dims, stag.PREC_F64)
+            x3, st3 = stag.cg_solve_mrhs(b3, L, cfg.mass, cfg.tol, args.maxiter or cfg.maxiter, stag.CG_RELIABLE, recon12=True)
+            print(json.dumps({"only": "mrhs", "config": {"workload": cfg.name}, "nrhs": 3,
+                              "iters": [t["iters"] for t in st3], "time_to_solution_s": st3[0]["seconds"],
+                              "us_per_iteration_per_rhs": st3[0]["seconds"] / max(1, max(t["iters"] for t in st3)) / 3 * 1e6}), flush=True)
+        replicas.finalize()
+        return 0
+
     b_dev = stag.spinor_pack(b_np, cfg.dims, stag.PREC_F64)
     b_host = torch.from_numpy(b_np.view(np.float64).reshape(-1).copy()).pin_memory()
     x_host = torch.zeros_like(b_host).pin_memory()
+    # the caller owns the workspace (include/stag.h): one allocation for all the solves below
+    ws = torch.empty(max(stag.cg_workspace_bytes(cfg.dims, m, 3) for m in (stag.CG_F64, stag.CG_RELIABLE)),
+                     dtype=torch.uint8, device="cuda")
+    stag.set_workspace(ws)
 
     def solve_device():
         return stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True)
@@ -279,45 +451,53 @@ def run_ours(args):
         return 0
 
     # ---- rank 0, N = any: the per-kernel numbers and the CPU baseline ---------------------------
-    dsl = {stag.PREC_NAMES[p]: time_dslash(stag, torch, fieldgen, cfg, L, p) for p in range(4)}
-    for p in (stag.PREC_F64_R8, stag.PREC_F32_R8):      # refused on fields with nearly-unit links
-        try:
-            dsl[stag.PREC_NAMES[p]] = time_dslash(stag, torch, fieldgen, cfg, L, p)
-            dsl[stag.PREC_NAMES[p]]["rebuilt_entry_error"] = L.recon8_error(p)
-        except stag.StagError as e:
-            dsl[stag.PREC_NAMES[p]] = {"refused": str(e)}
-    dom = dsl["fp32/12"]
-    roofline = {"bound": "hbm", "kernel": "dslash_kernel<float,2,*> (fp32, 12-real links: the hop of the timed solve)",
-                "achieved": dom["gbs"], "peak": peak, "unit": "GB/s", "frac": dom["gbs"] / peak,
-                "peak_source": peak_src, "traffic": args.traffic if cfg.name == "c4_28^3x96" else None,
-                "traffic_source": "profiles/r1e_dslash_fp32r12_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum, one launch)",
-                "algorithmic_bytes_per_launch": dom["algorithmic_bytes_per_site"] * cfg.vh,
-                "us_per_launch": dom["us"], "frac_of_nominal_8TBs": dom["gbs"] / 8000.0}
-    x64, st64 = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_F64)
-    x18, st18 = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE)
-    x64c, st64c = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_F64, recon12=True)
+    dsl, batch, blocked = hop_timings(stag, torch, fieldgen, cfg, L)
+    roofline = roofline_block(dsl, cfg, peak, peak_src)
+
+    def brief(t, **extra):
+        d = {"iters": t["iters"], "n_updates": t["n_updates"], "applies_f64": t["applies_f64"],
+             "time_to_solution_s": t["seconds"], "true_resid": t["true_resid"],
+             "ms_per_iteration": t["seconds"] / max(1, t["iters"]) * 1e3}
+        d.update(extra)
+        return d
+
+    def solve(mode, **kw):
+        stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, mode, **kw)      # warm: graph instantiated, links derived
+        return stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, mode, **kw)[1]
+
+    st64 = solve(stag.CG_F64)
+    st18 = solve(stag.CG_RELIABLE)
+    st64c = solve(stag.CG_F64, recon12=True)
+    # Fig. 2 (defect correction: a fresh inner CG per outer step) against section 3.2
+    # (direction kept across restarts + reliable / group-wise updates): same links, same
+    # source, same tolerance.  P:L84 "preserving the total number of CG iterations"
+    # "significantly faster convergence" of the corrected scheme.
+    st_dc = solve(stag.CG_DEFECT, recon12=True)
+    eps_sweep = {}
+    for eps in (0.1, 0.2, 0.3, 0.5):             # eps_in is never given a value
+        eps_sweep["%.1f" % eps] = brief(solve(stag.CG_RELIABLE, recon12=True, eps_in=eps))
+    dc_sweep = {}
+    for eps in (1e-1, 1e-2, 1e-3):
+        dc_sweep["%g" % eps] = brief(solve(stag.CG_DEFECT, recon12=True, eps_in=eps))
 
     # several right-hand sides sharing each pass over the links: three
-    # Gaussian sources in lockstep, and the batch hop alone
+    # Gaussian sources in lockstep
     b3 = stag.spinor_pack_mrhs([fieldgen.spinor_gaussian(cfg.dims, 0, seed + 1000 + k) for k in range(3)],
                                cfg.dims, stag.PREC_F64)
+    stag.cg_solve_mrhs(b3, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True)
     x3, st3 = stag.cg_solve_mrhs(b3, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True)
     mrhs = {"nrhs": 3, "iters": [t["iters"] for t in st3], "true_resid": [t["true_resid"] for t in st3],
             "time_to_solution_s": st3[0]["seconds"],
             "gflops": sum(t["iters"] for t in st3) * FLOP_PER_SITE_ITER * cfg.vh / st3[0]["seconds"] * 1e-9,
             "us_per_iteration_per_rhs": st3[0]["seconds"] / max(1, max(t["iters"] for t in st3)) / 3 * 1e6,
-            "dslash": {"%s x%d" % (stag.PREC_NAMES[p], n): time_dslash_mrhs(stag, torch, fieldgen, cfg, L, p, n, layout=stag.BATCH_PAIRED if p in (stag.PREC_F32, stag.PREC_F32_R12) else 0)
-                       for p, n in ((stag.PREC_F32_R12, 2), (stag.PREC_F32_R12, 3), (stag.PREC_F32_R12, 4), (stag.PREC_F32, 4), (stag.PREC_F64, 2))},
-            "dslash_blocked_layout": {"%s x%d" % (stag.PREC_NAMES[p], n): time_dslash_mrhs(stag, torch, fieldgen, cfg, L, p, n)
-                                      for p, n in ((stag.PREC_F32_R12, 3), (stag.PREC_F32_R12, 4), (stag.PREC_F32, 4))},
+            "dslash": batch, "dslash_blocked_layout": blocked,
             "layout": "fp32 batches paired (include/stag.h batch layouts), fp64 blocked"}
     del b3, x3
+    stag.set_workspace(None)
 
-    cpu = None
+    cpu, cpu_others = None, None
     if world == 1 and not args.no_cpu_baseline:
-        r = oracle_sample(cfg, W, b_np, 15.0)
-        cpu = {"value": r["gflops"], "unit": UNIT, "cores": host_threads(), "kind": "oracle",
-               "sample": "%d oracle CG iterations (Fig. 1, fp64) on %s, %.1f s" % (r["iters"], cfg.name, r["seconds"])}
+        cpu, cpu_others = cpu_baseline_block(cfg, W, b_np, args.cpu_full, iters_fp64=st64["iters"])
 
     line = {
         "metric": METRIC, "value": agg["throughput"] * 1e-9, "unit": UNIT, "n_gpus": world,
@@ -333,18 +513,24 @@ def run_ours(args):
         "clocks": clocks,
         "roofline": roofline,
         "cpu_baseline": cpu,
+        "cpu_baseline_other_configs": cpu_others,
         "cg": {"iters": st["iters"], "n_updates": st["n_updates"], "applies_f64": st["applies_f64"],
                "fp32_share_of_A_applications": st["iters"] / (st["iters"] + st["applies_f64"]),
                "true_resid": st["true_resid"], "time_to_solution_s": st["seconds"],
                "ms_per_iteration": st["seconds"] / max(1, st["iters"]) * 1e3,
-               "fp64_cg": {"iters": st64["iters"], "time_to_solution_s": st64["seconds"], "true_resid": st64["true_resid"]},
-               "fp64_cg_12real_links": {"iters": st64c["iters"], "time_to_solution_s": st64c["seconds"], "true_resid": st64c["true_resid"]},
-               "mixed_18real_links": {"iters": st18["iters"], "time_to_solution_s": st18["seconds"], "true_resid": st18["true_resid"],
-                                      "ms_per_iteration": st18["seconds"] / max(1, st18["iters"]) * 1e3},
+               "fp64_cg": brief(st64),
+               "fp64_cg_12real_links": brief(st64c),
+               "mixed_18real_links": brief(st18),
+               "defect_correction": brief(st_dc, outer_steps=st_dc["n_updates"], eps_in=1e-2,
+                                          iters_vs_reliable=st_dc["iters"] / max(1, st["iters"]),
+                                          time_vs_reliable=st_dc["seconds"] / st["seconds"]),
+               "defect_correction_eps_in_sweep": dc_sweep,
+               "reliable_eps_in_sweep": eps_sweep,
                "speedup_mixed_vs_fp64": st64["seconds"] / st["seconds"]},
         "dslash": dsl,
         "mrhs": mrhs,
         "setup_s0_seconds": setup_s,
+        "workspace": "caller-owned (stag_set_workspace), %d bytes" % ws.numel(),
         "paper_context": "GTX480: 145 GFLOPS SP / 55 DP per GPU pure-GPU CG (P:L131), 1.04 / 2.77 ms per Dirac op on a quarter lattice (Table 1)",
     }
     print(json.dumps(line), flush=True)
@@ -466,9 +652,14 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--decomp", choices=["replicas", "slabs"], default="replicas",
                     help="N > 1: independent replicas (weak scaling, default) or one lattice in T-slabs (strong)")
-    ap.add_argument("--traffic", type=float, default=436.2e6,
-                    help="dram bytes (read + write) per launch of the dominant kernel from the ncu --set full "
-                         "capture profiles/r1e_dslash_fp32r12_ncu_full.md (28^3x96, fp32/12 plain hop)")
+    ap.add_argument("--only", choices=["all", "hops", "mrhs"], default="all",
+                    help="hops: time the stand-alone hops only; mrhs: only the three-source lockstep solve "
+                         "(the commands the ncu captures under profiles/ run)")
+    ap.add_argument("--maxiter", type=int, default=0, help="with --only mrhs: cap the iterations (0 = the config's)")
+    ap.add_argument("--hops", default="",
+                    help='with --only hops: comma-separated names to run, e.g. "fp32/12,fp32/12 x4,fp32/12 x4 blocked"')
+    ap.add_argument("--cpu-full", action="store_true",
+                    help="also run the oracle's complete fp64 solve on the bench config (minutes of CPU)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

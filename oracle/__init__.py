@@ -23,21 +23,56 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 _lib = None
 
 
+CFLAGS = ["-O2", "-fopenmp"]                       # the checker: portable code, it travels between machines
+CFLAGS_NATIVE = ["-O3", "-march=native", "-fopenmp"]   # the timed CPU baseline, built where it runs
+_flags_in_use = list(CFLAGS)
+
+
 def build(force: bool = False) -> str:
     """Compile the oracle as it stands (plain -O2 + OpenMP; never tuned)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".tmp.%d" % os.getpid()
         subprocess.check_call(
-            ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-o", tmp, _SRC, "-lm"]
+            ["gcc"] + CFLAGS + ["-fPIC", "-shared", "-std=c11", "-o", tmp, _SRC, "-lm"]
         )
         os.replace(tmp, _LIB)
     return _LIB
 
 
-def _load():
+def use_native_build() -> list:
+    """For the timed CPU baseline only (bench.py): rebuild the SAME source with -O3 -march=native
+    on the machine it will run on (a .so built for another CPU could not be carried there) into a
+    private temporary file, and use it from now on in this process.  Falls back to the portable
+    build if the compiler refuses.  Returns the flags in use."""
+    global _lib, _flags_in_use
+    import tempfile
+    out = os.path.join(tempfile.mkdtemp(prefix="oracle_native_"), "liboracle_native.so")
+    try:
+        subprocess.check_call(["gcc"] + CFLAGS_NATIVE + ["-fPIC", "-shared", "-std=c11", "-o", out, _SRC, "-lm"],
+                              stderr=subprocess.DEVNULL)
+    except (OSError, subprocess.CalledProcessError):
+        return list(_flags_in_use)
+    _lib = None
+    _load(out)
+    _flags_in_use = list(CFLAGS_NATIVE)
+    return list(_flags_in_use)
+
+
+def compile_flags() -> list:
+    return list(_flags_in_use)
+
+
+def max_threads() -> int:
+    """omp_get_max_threads() of the loaded oracle."""
+    return int(_load().so_max_threads())
+
+
+def _load(path=None):
     global _lib
     if _lib is None:
-        lib = ctypes.CDLL(build())
+        lib = ctypes.CDLL(path or build())
+        lib.so_max_threads.argtypes = []
+        lib.so_max_threads.restype = ctypes.c_int
         dp = ctypes.POINTER(ctypes.c_double)
         ip = ctypes.POINTER(ctypes.c_int)
         u64p = ctypes.POINTER(ctypes.c_uint64)

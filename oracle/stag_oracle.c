@@ -23,6 +23,19 @@
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* threads the loops below run on (reported beside the timed CPU baseline; no arithmetic) */
+int so_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
 
 typedef struct { int X[4]; long V, Vh; } geom_t;
 

@@ -27,23 +27,22 @@ template <typename T> __device__ __forceinline__ void unpack(const double2 &v, T
 __device__ __forceinline__ float4 pack(const float *a) { return make_float4(a[0], a[1], a[2], a[3]); }
 __device__ __forceinline__ double2 pack(const double *a) { return make_double2(a[0], a[1]); }
 
-// Second stage shared by all reducing kernels.  Every block calls it with its nv (1 or 2)
-// partial sums, of right-hand sides k0 .. k0+nv-1; in the LAST block of the grid to arrive it
-// returns true (to all threads) with totals[k] = sum of partials[k*gridDim.x .. +gridDim.x) in
-// index order for every k < nrhs (totals is shared memory, MAX_RHS doubles).  A right-hand side
-// no block reports keeps the partials of an earlier launch: only frozen ones, which no epilogue reads.
-__device__ __forceinline__ bool finish_reduction_n(const double *block_values, int nv, int k0, int nrhs,
-                                                   double *partials, unsigned *ticket, double *red, double *totals)
+// Second stage shared by all reducing kernels.  Every block calls it with its partial of
+// right-hand side blockIdx.y; in the LAST block of the grid to arrive it returns true (to all
+// threads) with totals[k] = sum of partials[k*gridDim.x .. +gridDim.x) in index order for every
+// k < gridDim.y (totals is shared memory, MAX_RHS doubles).
+__device__ __forceinline__ bool finish_reduction(double block_value, double *partials,
+                                                 unsigned *ticket, double *red, double *totals)
 {
     __shared__ bool last;
     if (threadIdx.x == 0) {
-        for (int v = 0; v < nv; ++v) partials[(size_t)(k0 + v) * gridDim.x + blockIdx.x] = block_values[v];
+        partials[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = block_value;
         __threadfence();
         last = (atomicAdd(ticket, 1u) == gridDim.x * gridDim.y - 1);
     }
     __syncthreads();
     if (!last) return false;
-    for (int k = 0; k < nrhs; ++k) {
+    for (unsigned k = 0; k < gridDim.y; ++k) {
         double t = 0.0;
         for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x)
             t += __ldcg(partials + (size_t)k * gridDim.x + i);
@@ -53,12 +52,6 @@ __device__ __forceinline__ bool finish_reduction_n(const double *block_values, i
     if (threadIdx.x == 0) *ticket = 0;
     __syncthreads();
     return true;
-}
-// one value per block, right-hand side blockIdx.y of gridDim.y
-__device__ __forceinline__ bool finish_reduction(double block_value, double *partials,
-                                                 unsigned *ticket, double *red, double *totals)
-{
-    return finish_reduction_n(&block_value, 1, (int)blockIdx.y, (int)gridDim.y, partials, ticket, red, totals);
 }
 
 // ---- paired fp32 batches (stag_dslash.cuh; include/stag.h "batch layouts") -----------------------
@@ -76,40 +69,12 @@ __host__ __device__ inline size_t batch_index(int k, long i, long n, int nrhs, b
 
 // d = r + beta d   (Fig. 1; eq. 3.1 P:L91 when it follows an update).  beta = 0
 // makes it d = r, which is how the iteration starts and restarts.
-template <typename T, bool PAIRED = false>
+template <typename T>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 xpay_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const CgCtrl *__restrict__ ctrl)
 {
-    if (ctrl->state != CG_RUN) return;
-    int k = blockIdx.y;
-    if constexpr (PAIRED) {
-        const int npairs = ctrl->nrhs / 2;
-        if ((int)blockIdx.y < npairs) {
-            const int ka = 2 * blockIdx.y, kb = ka + 1;
-            const bool act_a = ctrl->active[ka], act_b = ctrl->active[kb];
-            if (!act_a && !act_b) return;
-            const float beta_a = (float)ctrl->beta[ka], beta_b = (float)ctrl->beta[kb];
-            float4 *dk = reinterpret_cast<float4 *>(d + (size_t)ka * n);
-            const float4 *rk = reinterpret_cast<const float4 *>(r + (size_t)ka * n);
-            const long nv = n / 2;                       // packets of the pair: one complex number of each
-            for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)gridDim.x * BLAS_BLOCK) {
-                const float4 a = ld_keep(rk + i);
-                float4 b = ld_keep(dk + i);
-                if (act_a) {
-                    b.x = (beta_a == 0.f) ? a.x : fma(beta_a, b.x, a.x);
-                    b.y = (beta_a == 0.f) ? a.y : fma(beta_a, b.y, a.y);
-                }
-                if (act_b) {
-                    b.z = (beta_b == 0.f) ? a.z : fma(beta_b, b.z, a.z);
-                    b.w = (beta_b == 0.f) ? a.w : fma(beta_b, b.w, a.w);
-                }
-                st_keep(dk + i, b);
-            }
-            return;
-        }
-        k = 2 * npairs;                                  // the odd last right-hand side, an ordinary spinor
-    }
-    if (!ctrl->active[k]) return;
+    const int k = blockIdx.y;
+    if (ctrl->state != CG_RUN || !ctrl->active[k]) return;
     using V = typename Vec4<T>::type;
     constexpr int N = Vec4<T>::N;
     const T beta = (T)ctrl->beta[k];
@@ -128,6 +93,64 @@ xpay_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const CgCtrl *__
             for (int j = 0; j < N; ++j) b[j] = fma(beta, b[j], a[j]);
         }
         st_keep(dk + i, pack(b));
+    }
+}
+
+// ---- the vector kernels on a paired fp32 batch ------------------------------------------------
+// One-dimensional grid of nrhs*B blocks, every block the same number of packets: pair u (twice the
+// data of a single right-hand side) owns blocks [u*2B, (u+1)*2B), an odd last right-hand side the
+// last B blocks.  (A 2-D grid with as many blocks per pair as per single leaves half the SMs idle
+// while the pairs finish.)
+struct PairedUnit {
+    int k0;        // first right-hand side of the unit
+    bool pair;     // two right-hand sides interleaved per complex number, or one ordinary spinor
+    int lb, nb;    // this block's index inside the unit, blocks in the unit
+};
+__device__ __forceinline__ PairedUnit paired_unit(int nrhs)
+{
+    const int B = gridDim.x / nrhs, npairs = nrhs / 2, b = blockIdx.x;
+    PairedUnit u;
+    if (b < npairs * 2 * B) { u.k0 = 2 * (b / (2 * B)); u.pair = true; u.lb = b % (2 * B); u.nb = 2 * B; }
+    else { u.k0 = 2 * npairs; u.pair = false; u.lb = b - npairs * 2 * B; u.nb = B; }
+    return u;
+}
+
+__global__ void __launch_bounds__(BLAS_BLOCK)
+xpay_paired_kernel(float *__restrict__ d, const float *__restrict__ r, long n, const CgCtrl *__restrict__ ctrl)
+{
+    if (ctrl->state != CG_RUN) return;
+    const PairedUnit u = paired_unit(ctrl->nrhs);
+    float4 *dk = reinterpret_cast<float4 *>(d + (size_t)u.k0 * n);
+    const float4 *rk = reinterpret_cast<const float4 *>(r + (size_t)u.k0 * n);
+    if (u.pair) {
+        const bool act_a = ctrl->active[u.k0], act_b = ctrl->active[u.k0 + 1];
+        if (!act_a && !act_b) return;
+        const float beta_a = (float)ctrl->beta[u.k0], beta_b = (float)ctrl->beta[u.k0 + 1];
+        const long nv = n / 2;                       // packets of the pair: one complex number of each
+        for (long i = u.lb * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)u.nb * BLAS_BLOCK) {
+            const float4 a = ld_keep(rk + i);
+            float4 b = ld_keep(dk + i);
+            if (act_a) {
+                b.x = (beta_a == 0.f) ? a.x : fma(beta_a, b.x, a.x);
+                b.y = (beta_a == 0.f) ? a.y : fma(beta_a, b.y, a.y);
+            }
+            if (act_b) {
+                b.z = (beta_b == 0.f) ? a.z : fma(beta_b, b.z, a.z);
+                b.w = (beta_b == 0.f) ? a.w : fma(beta_b, b.w, a.w);
+            }
+            st_keep(dk + i, b);
+        }
+        return;
+    }
+    if (!ctrl->active[u.k0]) return;
+    const float beta = (float)ctrl->beta[u.k0];
+    const long nv = n / 4;
+    for (long i = u.lb * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)u.nb * BLAS_BLOCK) {
+        const float4 a = ld_keep(rk + i);
+        float4 b = ld_keep(dk + i);
+        if (beta == 0.f) b = a;
+        else { b.x = fma(beta, b.x, a.x); b.y = fma(beta, b.y, a.y); b.z = fma(beta, b.z, a.z); b.w = fma(beta, b.w, a.w); }
+        st_keep(dk + i, b);
     }
 }
 
@@ -208,7 +231,7 @@ __device__ __forceinline__ void cg_iteration_epilogue(CgCtrl *__restrict__ ctrl,
 // block of right-hand side k adds the n_hop partials of k in the same order, so all of them use
 // the same alpha and no extra launch or device-wide fence is needed between the hop and this
 // kernel.  A frozen right-hand side (active == 0) is not touched.
-template <typename T, bool PAIRED = false>
+template <typename T>
 __global__ void __launch_bounds__(BLAS_BLOCK)
 update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
               const T *__restrict__ q, long n, const double *__restrict__ hop_partials,
@@ -219,58 +242,7 @@ update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
     constexpr int N = Vec4<T>::N;
     __shared__ double red[32];
     __shared__ double totals[MAX_RHS];
-    const int nrhs = ctrl->nrhs;
-    int k = blockIdx.y;
-    if constexpr (PAIRED) {
-        const int npairs = nrhs / 2;
-        if ((int)blockIdx.y < npairs) {
-            const int ka = 2 * blockIdx.y, kb = ka + 1;
-            const bool act_a = ctrl->active[ka], act_b = ctrl->active[kb];
-            double s2[2] = {0.0, 0.0};
-            if (act_a || act_b) {
-                double ad[2] = {0.0, 0.0};
-                if (act_a) {
-                    const double dAd = block_total_fixed(hop_partials + (size_t)ka * n_hop, n_hop, red);
-                    ad[0] = (dAd > 0.0) ? ctrl->delta[ka] / dAd : 0.0;
-                    if (blockIdx.x == 0 && threadIdx.x == 0) { ctrl->dAd[ka] = dAd; ctrl->alpha[ka] = ad[0]; }
-                }
-                if (act_b) {
-                    const double dAd = block_total_fixed(hop_partials + (size_t)kb * n_hop, n_hop, red);
-                    ad[1] = (dAd > 0.0) ? ctrl->delta[kb] / dAd : 0.0;
-                    if (blockIdx.x == 0 && threadIdx.x == 0) { ctrl->dAd[kb] = dAd; ctrl->alpha[kb] = ad[1]; }
-                }
-                const float al_a = (float)ad[0], al_b = (float)ad[1];        // 0 for a frozen half: y, r unchanged
-                float4 *yk = reinterpret_cast<float4 *>(y + (size_t)ka * n);
-                float4 *rk = reinterpret_cast<float4 *>(r + (size_t)ka * n);
-                const float4 *dk = reinterpret_cast<const float4 *>(d + (size_t)ka * n);
-                const float4 *qk = reinterpret_cast<const float4 *>(q + (size_t)ka * n);
-                const long nv = n / 2;
-                for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)gridDim.x * BLAS_BLOCK) {
-                    float4 yy = ld_pass(yk + i), rr = ld_keep(rk + i);
-                    const float4 dd = ld_keep(dk + i), qq = ld_keep(qk + i);
-                    if (act_a) {
-                        yy.x = fma(al_a, dd.x, yy.x); yy.y = fma(al_a, dd.y, yy.y);
-                        rr.x = fma(-al_a, qq.x, rr.x); rr.y = fma(-al_a, qq.y, rr.y);
-                        s2[0] += (double)rr.x * (double)rr.x + (double)rr.y * (double)rr.y;
-                    }
-                    if (act_b) {
-                        yy.z = fma(al_b, dd.z, yy.z); yy.w = fma(al_b, dd.w, yy.w);
-                        rr.z = fma(-al_b, qq.z, rr.z); rr.w = fma(-al_b, qq.w, rr.w);
-                        s2[1] += (double)rr.z * (double)rr.z + (double)rr.w * (double)rr.w;
-                    }
-                    st_pass(yk + i, yy);
-                    st_keep(rk + i, rr);
-                }
-            }
-            double bs[2];
-            bs[0] = block_sum(s2[0], red);
-            bs[1] = block_sum(s2[1], red);
-            if (!finish_reduction_n(bs, 2, ka, nrhs, partials, &ctrl->ticket[1], red, totals)) return;
-            if (threadIdx.x == 0) cg_iteration_epilogue(ctrl, totals);
-            return;
-        }
-        k = 2 * npairs;
-    }
+    const int k = blockIdx.y;
     double s = 0.0;
     if (ctrl->active[k]) {
         const double dAd = block_total_fixed(hop_partials + (size_t)k * n_hop, n_hop, red);
@@ -300,9 +272,90 @@ update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d,
         }
     }
     const double bs = block_sum(s, red);
-    if (!finish_reduction_n(&bs, 1, k, nrhs, partials, &ctrl->ticket[1], red, totals)) return;
+    if (!finish_reduction(bs, partials, &ctrl->ticket[1], red, totals)) return;
     if (threadIdx.x != 0) return;
 
+    cg_iteration_epilogue(ctrl, totals);
+}
+
+// The same on a paired fp32 batch (grid and units: paired_unit above).  Partial sums of right-hand
+// side k sit in partials[k*S + block-in-unit], S = 2B slots per right-hand side.
+__global__ void __launch_bounds__(BLAS_BLOCK)
+update_paired_kernel(float *__restrict__ y, float *__restrict__ r, const float *__restrict__ d,
+                     const float *__restrict__ q, long n, const double *__restrict__ hop_partials,
+                     int n_hop, double *__restrict__ partials, CgCtrl *__restrict__ ctrl)
+{
+    if (ctrl->state != CG_RUN) return;
+    __shared__ double red[32];
+    __shared__ double totals[MAX_RHS];
+    __shared__ bool last;
+    const int nrhs = ctrl->nrhs;
+    const PairedUnit u = paired_unit(nrhs);
+    const int S = 2 * (gridDim.x / nrhs);
+    const int ka = u.k0, kb = u.k0 + 1;
+    const bool act_a = ctrl->active[ka], act_b = u.pair && ctrl->active[kb];
+    double s2[2] = {0.0, 0.0};
+    if (act_a || act_b) {
+        double ad[2] = {0.0, 0.0};
+        if (act_a) {
+            const double dAd = block_total_fixed(hop_partials + (size_t)ka * n_hop, n_hop, red);
+            ad[0] = (dAd > 0.0) ? ctrl->delta[ka] / dAd : 0.0;                       // P:L51; 0 also for NaN
+            if (u.lb == 0 && threadIdx.x == 0) { ctrl->dAd[ka] = dAd; ctrl->alpha[ka] = ad[0]; }
+        }
+        if (act_b) {
+            const double dAd = block_total_fixed(hop_partials + (size_t)kb * n_hop, n_hop, red);
+            ad[1] = (dAd > 0.0) ? ctrl->delta[kb] / dAd : 0.0;
+            if (u.lb == 0 && threadIdx.x == 0) { ctrl->dAd[kb] = dAd; ctrl->alpha[kb] = ad[1]; }
+        }
+        float4 *yk = reinterpret_cast<float4 *>(y + (size_t)ka * n);
+        float4 *rk = reinterpret_cast<float4 *>(r + (size_t)ka * n);
+        const float4 *dk = reinterpret_cast<const float4 *>(d + (size_t)ka * n);
+        const float4 *qk = reinterpret_cast<const float4 *>(q + (size_t)ka * n);
+        // pair: halves .xy / .zw belong to ka / kb; single: the whole packet belongs to ka
+        const float al_a = (float)ad[0], al_b = u.pair ? (float)ad[1] : al_a;
+        const bool upd_xy = act_a, upd_zw = u.pair ? act_b : act_a;
+        const long nv = u.pair ? n / 2 : n / 4;
+        for (long i = u.lb * (long)BLAS_BLOCK + threadIdx.x; i < nv; i += (long)u.nb * BLAS_BLOCK) {
+            float4 yy = ld_pass(yk + i), rr = ld_keep(rk + i);
+            const float4 dd = ld_keep(dk + i), qq = ld_keep(qk + i);
+            double sxy = 0.0, szw = 0.0;
+            if (upd_xy) {
+                yy.x = fma(al_a, dd.x, yy.x); yy.y = fma(al_a, dd.y, yy.y);
+                rr.x = fma(-al_a, qq.x, rr.x); rr.y = fma(-al_a, qq.y, rr.y);
+                sxy = (double)rr.x * (double)rr.x + (double)rr.y * (double)rr.y;
+            }
+            if (upd_zw) {
+                yy.z = fma(al_b, dd.z, yy.z); yy.w = fma(al_b, dd.w, yy.w);
+                rr.z = fma(-al_b, qq.z, rr.z); rr.w = fma(-al_b, qq.w, rr.w);
+                szw = (double)rr.z * (double)rr.z + (double)rr.w * (double)rr.w;
+            }
+            s2[0] += sxy;
+            if (u.pair) s2[1] += szw; else s2[0] += szw;
+            st_pass(yk + i, yy);
+            st_keep(rk + i, rr);
+        }
+    }
+    double bs[2];
+    bs[0] = block_sum(s2[0], red);
+    bs[1] = block_sum(s2[1], red);
+    if (threadIdx.x == 0) {
+        partials[(size_t)ka * S + u.lb] = bs[0];
+        if (u.pair) partials[(size_t)kb * S + u.lb] = bs[1];
+        __threadfence();
+        last = (atomicAdd(&ctrl->ticket[1], 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!last) return;
+    for (int k = 0; k < nrhs; ++k) {       // fixed order; a frozen right-hand side's slots hold old values nobody reads
+        const int nbk = (k < (nrhs / 2) * 2) ? S : S / 2;
+        double t = 0.0;
+        for (int i = threadIdx.x; i < nbk; i += blockDim.x) t += __ldcg(partials + (size_t)k * S + i);
+        t = block_sum(t, red);
+        if (threadIdx.x == 0) totals[k] = t;
+    }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    ctrl->ticket[1] = 0;
     cg_iteration_epilogue(ctrl, totals);
 }
 

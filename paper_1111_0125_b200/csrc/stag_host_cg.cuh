@@ -26,7 +26,8 @@ struct Solver {
     int gb_lo;       // grid.x of the iteration's vector kernels: blocks per unit (pair or single)
 
     dim3 grid2() const { return dim3((unsigned)gb, (unsigned)nrhs); }
-    dim3 grid_lo() const { return dim3((unsigned)gb_lo, (unsigned)(paired ? (nrhs + 1) / 2 : nrhs)); }
+    // paired: 1-D grid of nrhs*gb_lo equal blocks (stag_blas.cuh, paired_unit); else (blocks, right-hand sides)
+    dim3 grid_lo() const { return paired ? dim3((unsigned)(gb_lo * nrhs), 1u) : dim3((unsigned)gb_lo, (unsigned)nrhs); }
 
     // q64 = A x  in fp64 (two hops), outside the iteration
     int apply_A64(const double *x)
@@ -74,7 +75,7 @@ struct Solver {
     {
         constexpr bool F32 = std::is_same<T, float>::value;
         const int layout = (F32 && paired) ? STAG_BATCH_PAIRED : STAG_BATCH_BLOCKED;
-        if (F32 && paired) xpay_kernel<float, true><<<grid_lo(), BLAS_BLOCK, 0, st>>>((float *)d, (const float *)r, n, w.ctrl);
+        if (F32 && paired) xpay_paired_kernel<<<grid_lo(), BLAS_BLOCK, 0, st>>>((float *)d, (const float *)r, n, w.ctrl);
         else xpay_kernel<T><<<grid_lo(), BLAS_BLOCK, 0, st>>>(d, r, n, w.ctrl);             // d = r + beta d
         count_launch();
         KCHECK();
@@ -82,7 +83,7 @@ struct Solver {
         if (rc) return rc;
         rc = launch_hop(L, prec_lo, HOP_XPAY_DOT, q, tmp, 0, m2, 1.0, d, w.hop_partials, w.ctrl, nrhs, st, layout);  // q = A d, <d,q>
         if (rc) return rc;
-        if (F32 && paired) update_kernel<float, true><<<grid_lo(), BLAS_BLOCK, 0, st>>>((float *)y, (float *)r, (const float *)d, (const float *)q, n, w.hop_partials, w.n_hop, w.partials, w.ctrl);
+        if (F32 && paired) update_paired_kernel<<<grid_lo(), BLAS_BLOCK, 0, st>>>((float *)y, (float *)r, (const float *)d, (const float *)q, n, w.hop_partials, w.n_hop, w.partials, w.ctrl);
         else update_kernel<T><<<grid_lo(), BLAS_BLOCK, 0, st>>>(y, r, d, q, n, w.hop_partials, w.n_hop, w.partials, w.ctrl);  // alpha, y, r, delta, beta
         count_launch();
         KCHECK();
@@ -129,7 +130,7 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
     S.gb = blas_grid(S.n, nrhs);
     S.applies_f64 = 0;
     S.paired = (mode != STAG_CG_F64) && nrhs >= 2;
-    S.gb_lo = S.paired ? blas_grid(2 * S.n, (nrhs + 1) / 2) : S.gb;
+    S.gb_lo = S.gb;      // blocks per right-hand side: a pair gets twice as many
     int rc;
     if ((rc = ensure_links(L, S.prec_lo))) return rc;
     if ((rc = ensure_links(L, S.prec_hi))) return rc;

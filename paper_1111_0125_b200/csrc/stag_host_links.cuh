@@ -298,6 +298,34 @@ int launch_hop_n(const stag_links *L, int prec, int hop, cplx_t<T> *out, const c
     return STAG_OK;
 }
 
+// fp32, 2..4 right-hand sides: the batch kernel with its explicit load pipeline (stag_dslash_batch.cuh).
+template <int NR, int MODE, int N, bool PAIRED>
+int launch_batch_mode(const float4 *field, unsigned grid, float2 *out, const float2 *in, const Geom &g, int parity,
+                      double a, double cD, const float2 *own, double *partials, const CgCtrl *ctrl, cudaStream_t s)
+{
+    // tiles (warps) of one wave of resident blocks: how far ahead a warp prefetches link tiles into L2
+    const int pf_ahead = (blas_full_grid() / 4) * BatchTune<NR, N>::MINB * (DSLASH_BLOCK / TILE);
+    dslash_batch_kernel<NR, MODE, N, PAIRED><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (float)a, (float)cD, own, partials, ctrl, pf_ahead);
+    count_launch();
+    KCHECK();
+    return STAG_OK;
+}
+
+template <int NR, int N, bool PAIRED>
+int launch_batch_n(const stag_links *L, int prec, int hop, float2 *out, const float2 *in, int parity,
+                   double a, double cD, const float2 *own, double *partials, const CgCtrl *ctrl, cudaStream_t s)
+{
+    const Geom &g = L->g;
+    const float4 *field = (const float4 *)L->L[prec] + (size_t)parity * L->ntiles * (8 * link_slots(NR) / 2) * TILE;
+    const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
+    switch (hop) {
+    case HOP_PLAIN:    return launch_batch_mode<NR, HOP_PLAIN, N, PAIRED>(field, grid, out, in, g, parity, a, cD, own, partials, ctrl, s);
+    case HOP_XPAY:     return launch_batch_mode<NR, HOP_XPAY, N, PAIRED>(field, grid, out, in, g, parity, a, cD, own, partials, ctrl, s);
+    case HOP_XPAY_DOT: return launch_batch_mode<NR, HOP_XPAY_DOT, N, PAIRED>(field, grid, out, in, g, parity, a, cD, own, partials, ctrl, s);
+    }
+    return STAG_EINVAL;      // HOP_AXPBY: only the fp64 wrapper steps use it
+}
+
 // nrhs right-hand sides in chunks of at most HopMaxRhs<T>: each chunk is one pass over the links.
 // layout: STAG_BATCH_BLOCKED or STAG_BATCH_PAIRED (fp32 only; a chunk starts at an even right-hand
 // side, so chunk k0 of a paired batch begins k0*rs complex numbers in, like a blocked one).
@@ -320,18 +348,17 @@ int launch_hop_t(const stag_links *L, int prec, int hop, cplx_t<T> *out, const c
         int rc = STAG_EINVAL;
         if (nb == 1) rc = launch_hop_n<T, NR, 1, false>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
         if constexpr (F32) {
-            if (layout == STAG_BATCH_PAIRED) {
-                if (nb == 2) rc = launch_hop_n<T, NR, 2, true>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
-                if (nb == 3) rc = launch_hop_n<T, NR, 3, true>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
-                if (nb == 4) rc = launch_hop_n<T, NR, 4, true>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
-                if (rc) return rc;
-                continue;
+            if (nb >= 2) {
+                const bool pr = layout == STAG_BATCH_PAIRED;
+                if (nb == 2) rc = pr ? launch_batch_n<NR, 2, true>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s)
+                                     : launch_batch_n<NR, 2, false>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+                if (nb == 3) rc = pr ? launch_batch_n<NR, 3, true>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s)
+                                     : launch_batch_n<NR, 3, false>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+                if (nb == 4) rc = pr ? launch_batch_n<NR, 4, true>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s)
+                                     : launch_batch_n<NR, 4, false>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
             }
-        }
-        if (nb == 2) rc = launch_hop_n<T, NR, 2, false>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
-        if constexpr (NB >= 4) {
-            if (nb == 3) rc = launch_hop_n<T, NR, 3, false>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
-            if (nb == 4) rc = launch_hop_n<T, NR, 4, false>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
+        } else {
+            if (nb == 2) rc = launch_hop_n<T, NR, 2, false>(L, prec, hop, o, i, parity, a, cD, w, pp, ctrl, s);
         }
         if (rc) return rc;
     }

@@ -11,6 +11,7 @@
 #include "stag_blas.cuh"
 #include "stag_common.cuh"
 #include "stag_dslash.cuh"
+#include "stag_dslash_batch.cuh"
 #include "stag_slab.cuh"
 
 using namespace stag;
