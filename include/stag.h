@@ -258,9 +258,24 @@ int stag_apply_A_batch(void *out_even, const void *in_even, const stag_links_t *
 #define STAG_IPC_HANDLE_BYTES 64
 #define STAG_MAX_RANKS 16       /* most slabs a lattice is split into */
 
-/* W_global: canonical fp64 links of the WHOLE lattice global_dims (eta*bc folded). */
+/* W_global: canonical fp64 links of the WHOLE lattice global_dims (eta*bc folded).  From host
+ * memory only the rank's own part is copied to the device (the sub-ranges stag_slab_create_local
+ * takes); from device memory the field is read in place. */
 int stag_slab_create(stag_links_t **slab_out, const int global_dims[4], int antiperiodic_t,
                      const double *W_global, int on_device, int rank, int nranks);
+/* The same slab from the rank's OWN part of the field, so that no rank ever holds or moves the
+ * whole lattice (per-rank setup memory and time shrink with nranks).  Time slices are contiguous
+ * in the checkerboard index, so with s3 = X0*X1*X2/2, Tl = X3/nranks, t0 = rank*Tl:
+ *   W_local[mu][p][cb'][3][3]  = W_global[mu][p][t0*s3 + cb'],  cb' = 0 .. Tl*s3-1
+ *                                (the canonical layout of a lattice of the LOCAL dims);
+ *   W_back[p][j][3][3]         = W_global[3][p][((t0-1) mod X3)*s3 + j],  j = 0 .. s3-1
+ *                                (the t-links leaving the time slice before the slab: the
+ *                                backward t-links of the slab's first slice, owned by rank-1).
+ * eta*bc folded by the caller as in stag_links_create; both in host (on_device = 0) or both in
+ * device memory.  The result is bit-identical to stag_slab_create on the whole field. */
+int stag_slab_create_local(stag_links_t **slab_out, const int global_dims[4], int antiperiodic_t,
+                           const double *W_local, const double *W_back, int on_device,
+                           int rank, int nranks);
 /* Any output pointer may be NULL. */
 int stag_slab_info(const stag_links_t *slab, int local_dims_out[4], int *rank_out, int *nranks_out,
                    void **exchange_ptr_out, size_t *exchange_bytes_out);
@@ -280,12 +295,25 @@ int stag_slab_hop(void *out, const void *in, stag_links_t *slab, int parity, int
 int stag_slab_dslash(void *out, const void *in, stag_links_t *slab, int parity, int prec);
 
 /* Watchdog.  A kernel that waits for a neighbour's flag polls it at most `polls` times (about a
- * microsecond each; 0 restores the default of 2^23, roughly ten seconds), then gives up, marks the
- * slab and finishes on stale data instead of spinning for ever.  stag_slab_status synchronises
- * the stream and returns STAG_ETIMEOUT if that has happened since the slab was made (also reported
- * by stag_slab_cg_control / _finish), STAG_OK otherwise. */
+ * microsecond each; 0 restores the default of 2^23, roughly ten seconds), then gives up and marks
+ * the slab DEAD.  A dead slab publishes nothing any more: the kernel whose wait gave up finishes
+ * its own stores but sets no neighbour's flag and bumps no count, and every later kernel of the
+ * slab path returns at once, so the neighbours' waits run into their own limit in turn and EVERY
+ * rank ends with STAG_ETIMEOUT instead of consuming stale data.  The limit counts rank skew too
+ * (a peer that starts late is indistinguishable from a dead one): put a barrier before the first
+ * exchange.  stag_slab_status synchronises the stream and returns STAG_ETIMEOUT for a dead slab
+ * (also reported by stag_slab_cg_control / _finish), STAG_OK otherwise.
+ * stag_slab_reset revives a slab: flags, counts, reduction slots and the mark are cleared (the wait
+ * limit is kept).  Collective: ALL ranks must call it, with nothing of the slab path in flight
+ * anywhere, and synchronise with each other (a barrier) both before and after the call; the
+ * alternative is to destroy the handles. */
 int stag_slab_set_wait_limit(stag_links_t *slab, unsigned long long polls);
 int stag_slab_status(stag_links_t *slab);
+int stag_slab_reset(stag_links_t *slab);
+/* Diagnostics since creation / the last reset: how many acquire-waits of this slab's kernels did
+ * not find their flag already set, and how many polls they spent (either pointer may be NULL).
+ * Zero when every kernel found its peers' data waiting, as in a lockstep run. */
+int stag_slab_wait_stats(stag_links_t *slab, unsigned long long *waits_spun_out, unsigned long long *polls_out);
 
 /* ---- the solver -------------------------------------------------------- */
 
@@ -393,7 +421,10 @@ int stag_slab_cg_step(stag_links_t *slab, int action, int phase, int *more_out);
 /* Returns STAG_OK / STAG_ENOCONV / STAG_EBREAKDOWN like stag_cg_solve; stats as there. */
 int stag_slab_cg_finish(stag_links_t *slab, stag_cg_stats_t *stats_out);
 /* begin + the loop above + finish: the call of a one-process-per-GPU run (all ranks together).
- * NOT for slabs sharing a device: there a waiting kernel would block the kernel it waits for. */
+ * Slabs sharing a device may call it too -- one host thread and one stream per slab -- as long as
+ * all their kernels can be resident at the same time (small lattices; tests/test_gpu_slab_concurrent.py):
+ * a waiting kernel that fills the device would block the kernel it waits for, and the watchdog
+ * turns that into STAG_ETIMEOUT. */
 int stag_slab_cg_run(stag_links_t *slab, void *x_even, const void *b_even, double mass, double tol,
                      int maxiter, int mode, const stag_cg_params_t *params, stag_cg_stats_t *stats_out);
 

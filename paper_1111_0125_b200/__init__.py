@@ -124,6 +124,8 @@ SIGNATURES = {
                                     ctypes.POINTER(_Stats)]),
     "stag_slab_create": (ctypes.c_int, [ctypes.POINTER(_vp), _ip, ctypes.c_int, _vp, ctypes.c_int,
                                         ctypes.c_int, ctypes.c_int]),
+    "stag_slab_create_local": (ctypes.c_int, [ctypes.POINTER(_vp), _ip, ctypes.c_int, _vp, _vp, ctypes.c_int,
+                                              ctypes.c_int, ctypes.c_int]),
     "stag_slab_info": (ctypes.c_int, [_vp, _ip, _ip, _ip, ctypes.POINTER(_vp), ctypes.POINTER(ctypes.c_size_t)]),
     "stag_slab_ipc_handle": (ctypes.c_int, [_vp, ctypes.c_char_p]),
     "stag_slab_ipc_open": (ctypes.c_int, [ctypes.c_char_p, ctypes.POINTER(_vp)]),
@@ -134,6 +136,8 @@ SIGNATURES = {
     "stag_slab_dslash": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, ctypes.c_int]),
     "stag_slab_set_wait_limit": (ctypes.c_int, [_vp, ctypes.c_ulonglong]),
     "stag_slab_status": (ctypes.c_int, [_vp]),
+    "stag_slab_reset": (ctypes.c_int, [_vp]),
+    "stag_slab_wait_stats": (ctypes.c_int, [_vp, ctypes.POINTER(ctypes.c_ulonglong), ctypes.POINTER(ctypes.c_ulonglong)]),
     "stag_slab_connect_all": (ctypes.c_int, [_vp, ctypes.POINTER(_vp)]),
     "stag_slab_cg_begin": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                           ctypes.c_int, ctypes.POINTER(_Params)]),

@@ -186,6 +186,9 @@ struct XchHeader {
     // shows up as an error from the next host call instead of a GPU that spins for ever
     unsigned timed_out;
     unsigned long long wait_limit;  // polls (~1 us each); 0 = the default below
+    // diagnostics (stag_slab_wait_stats): acquire-waits that did not find their flag set at once, and
+    // the polls they spent; proof that a test really ran ranks concurrently
+    unsigned long long waits_spun, polls_spent;
 };
 constexpr unsigned long long XCH_DEFAULT_WAIT_POLLS = 1ull << 23;     // roughly ten seconds
 static_assert(sizeof(XchHeader) <= XCH_RED, "exchange header must fit its slot");

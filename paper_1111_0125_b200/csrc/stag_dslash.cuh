@@ -147,18 +147,34 @@ template <typename T> struct HaloArgs {
     unsigned n_push_blocks;   // blocks of this launch that own boundary-slice sites (they alone take the ticket)
 };
 
-// hdr: the header of the slab whose flag f belongs to (for the watchdog, stag_common.cuh)
-__device__ __forceinline__ void wait_flag(const unsigned long long *f, unsigned long long epoch, XchHeader *hdr)
+// hdr: the header of the slab whose flag f belongs to (for the watchdog, stag_common.cuh).
+// Returns false when the wait gave up: the slab is then marked (hdr->timed_out, sticky until
+// stag_slab_reset) and the caller must not publish anything derived from the data it waited for.
+__device__ __forceinline__ bool wait_flag(const unsigned long long *f, unsigned long long epoch, XchHeader *hdr)
 {
     unsigned long long v, polls = 0;
     unsigned long long limit = __ldcg(&hdr->wait_limit);
     if (limit == 0) limit = XCH_DEFAULT_WAIT_POLLS;
     for (;;) {
         asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(f) : "memory");
-        if (v >= epoch) return;
-        if (++polls >= limit) { hdr->timed_out = 1u; return; }
+        if (v >= epoch) {
+            if (polls) { atomicAdd(&hdr->waits_spun, 1ull); atomicAdd(&hdr->polls_spent, polls); }
+            return true;
+        }
+        if (++polls >= limit || __ldcg(&hdr->timed_out) != 0u) {
+            *(volatile unsigned *)&hdr->timed_out = 1u;
+            return false;
+        }
         __nanosleep(200);
     }
+}
+// A slab whose watchdog fired is dead until stag_slab_reset: every kernel of the slab path begins with
+// this test (uniform over the grid when the mark predates the launch) and leaves without storing to a
+// peer, bumping a count or setting a flag, so the neighbours' waits run into their own limit and every
+// rank reports STAG_ETIMEOUT instead of consuming stale data.
+__device__ __forceinline__ bool slab_dead(const char *xch)
+{
+    return __ldcg(&((const XchHeader *)xch)->timed_out) != 0u;
 }
 
 // T: float or double.  NR: storage of each link (3 = 18-real, 2 = 12-real rows 0,1, 1 = 8-parameter).
@@ -201,6 +217,9 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
     constexpr int KG = K * GM;                // packets per group
     static_assert(8 % DPG == 0, "group must divide the eight directions");
     if (ctrl != nullptr && ctrl->state != CG_RUN) return;
+    if constexpr (HALO) {
+        if (slab_dead(halo.xch)) return;
+    }
 
     int cb = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
     if constexpr (HALO) {
@@ -407,7 +426,9 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
                 e_in = s_e;
                 __threadfence();      // release at gpu scope; the ticket's last holder fences at system scope
             }
-            if (any && threadIdx.x == 0 && atomicAdd(&hdr->ticket, 1u) == halo.n_push_blocks - 1) {
+            // every boundary block waited for its own halo before it got here, so the ticket's last
+            // holder sees a timeout of any of them (their marks precede their gpu-scope fences)
+            if (any && threadIdx.x == 0 && atomicAdd(&hdr->ticket, 1u) == halo.n_push_blocks - 1 && !slab_dead(halo.xch)) {
                 hdr->ticket = 0;
                 hdr->epoch = e_in + 1;
                 __threadfence_system();   // cumulativity: every block's peer stores precede the flags

@@ -19,14 +19,24 @@ size_t links_elems(const stag_links *L, int rows)   // complex numbers in one ga
 // here by eta_mu(x') bc_mu(x') of ITS OWN site x' (x for the forward link, x - mu^ for the
 // backward one), the device-side form of the paper's "gauge link preconditioning".
 // The sign comes from det_sign_mask: det M_d = eta bc for d < 4 and -(eta bc) for d >= 4.
-// g is the geometry of the lattice the handle covers, gg that of the lattice W covers: the same
-// for a whole-lattice handle; for a T-slab (stag_slab_create) g is the slab (time slices
-// [g.t0, g.t0 + g.X3) of gg) and every link, including the backward t-links of the slab's first
-// slice that belong to the neighbouring slab, is read from the whole field.
+// g is the geometry of the lattice the handle covers, gg that of the whole lattice: the same
+// for a whole-lattice handle; for a T-slab g is the slab (time slices [g.t0, g.t0 + g.X3) of gg).
+// src says where the canonical links are: the whole field (stag_links_create, stag_slab_create from
+// device memory), or only the slab's own time slices plus the t-links of the slice before it, which
+// are the backward t-links of the slab's first slice and belong to the neighbouring slab
+// (stag_slab_create_local): no rank then ever holds the whole lattice.
+struct LinkSrc {
+    const double *W;       // [mu][p][vh][3][3], cb index = global cb - off
+    const double *Wback;   // [p][s3][3][3]: W_3 on time slice t0-1 (mod X3g); null when W holds it
+    long vh;               // sites per (mu, p) plane of W
+    long off;              // t0*s3 for a slab's own part, 0 for the whole field
+};
+
 __global__ void __launch_bounds__(128)
-gather_links_kernel(double2 *__restrict__ L, const double *__restrict__ W, const Geom g,
+gather_links_kernel(double2 *__restrict__ L, const LinkSrc src_, const Geom g,
                     const Geom gg, unsigned long long *__restrict__ err_bits, const int fold)
 {
+    const double *__restrict__ W = src_.W;
     const long idx = blockIdx.x * 128L + threadIdx.x;
     if (idx >= 2L * g.Vh_pad) return;
     const int p = (int)(idx / g.Vh_pad);
@@ -45,10 +55,13 @@ gather_links_kernel(double2 *__restrict__ L, const double *__restrict__ W, const
     for (int d = 0; d < 8; ++d) {
         double2 m[9];
         if (d < 4) {
-            const double *src = W + (((size_t)d * 2 + p) * gg.Vh + cbg) * 18;
+            const double *src = W + (((size_t)d * 2 + p) * src_.vh + (cbg - src_.off)) * 18;
             for (int k = 0; k < 9; ++k) m[k] = make_double2(src[2 * k], src[2 * k + 1]);
         } else {
-            const double *src = W + (((size_t)(d - 4) * 2 + (1 - p)) * gg.Vh + s.nbr[d]) * 18;
+            const long at = (long)s.nbr[d] - src_.off;
+            const double *src = W + (((size_t)(d - 4) * 2 + (1 - p)) * src_.vh + at) * 18;
+            if (at < 0 || at >= src_.vh)      // only d = 7 on the slab's first slice: the neighbour slab's t-link
+                src = src_.Wback + ((size_t)(1 - p) * gg.s3 + (s.nbr[d] % gg.s3)) * 18;
             for (int i = 0; i < 3; ++i)
                 for (int j = 0; j < 3; ++j)   // M = -W^dag : M_ij = -conj(W_ji)
                     m[3 * i + j] = make_double2(-src[2 * (3 * j + i)], src[2 * (3 * j + i) + 1]);
@@ -424,7 +437,8 @@ extern "C" void stag_reset_launch_count(void) { g_launches.store(0); }
 // C ABI: links
 // ------------------------------------------------------------------------------------
 static int links_create(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
-                        const double *W, int on_device, int fold, int rank, int nranks);
+                        const double *W, int on_device, int fold, int rank, int nranks,
+                        const double *W_back = nullptr, bool local = false);
 
 extern "C" int stag_links_create(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
                                  const double *W, int on_device)
@@ -438,10 +452,13 @@ extern "C" int stag_links_create_unfolded(stag_links_t **links_out, const int di
     return links_create(links_out, dims, antiperiodic_t, U, on_device, 1, 0, 1);
 }
 
-// dims: the lattice W covers.  nranks > 1 (or slab != 0): the handle covers time slices
-// [rank*X3/nranks, (rank+1)*X3/nranks) only and is a T-slab (exchange region allocated).
+// dims: the whole lattice.  nranks > 1: the handle covers time slices [rank*X3/nranks, (rank+1)*X3/nranks)
+// only.  local: W is the slab's own part and W_back the t-links of the slice before it (LinkSrc);
+// otherwise W is the whole field, and from HOST memory only those same sub-ranges are copied to the
+// device (8 + 2 contiguous ranges: time slices are contiguous in cb), never the whole lattice.
 static int links_create(stag_links_t **links_out, const int dims[4], int antiperiodic_t,
-                        const double *W, int on_device, int fold, int rank, int nranks)
+                        const double *W, int on_device, int fold, int rank, int nranks,
+                        const double *W_back, bool local)
 {
     if (!links_out || !W) return STAG_EINVAL;
     *links_out = nullptr;
@@ -450,6 +467,7 @@ static int links_create(stag_links_t **links_out, const int dims[4], int antiper
     if (nranks < 1 || rank < 0 || rank >= nranks || dims[3] % nranks) return STAG_EINVAL;
     const int ldims[4] = { dims[0], dims[1], dims[2], dims[3] / nranks };
     if (!make_geom(g, ldims, antiperiodic_t)) return STAG_EINVAL;     // local extent even, >= 2
+    if (local && nranks > 1 && !W_back) return STAG_EINVAL;
     g.t0 = rank * ldims[3];
     g.X3g = dims[3];
     stag_links *L = new (std::nothrow) stag_links();
@@ -461,21 +479,46 @@ static int links_create(stag_links_t **links_out, const int dims[4], int antiper
     L->nranks = nranks;
     L->ntiles = g.Vh_pad / TILE;
 
-    const size_t canon_bytes = (size_t)4 * 2 * gg.Vh * 18 * sizeof(double);
-    double *Wd = nullptr;
+    const size_t plane_l = (size_t)g.Vh * 18, plane_g = (size_t)gg.Vh * 18;      // doubles per (mu, p)
+    const size_t slice = (size_t)gg.s3 * 18;
+    const bool part = local || (nranks > 1 && !on_device);    // the device sees only the slab's part
+    double *Wd = nullptr, *Wbd = nullptr;
     unsigned long long *err = nullptr;
     int rc = STAG_OK;
-    cudaError_t e;
+    cudaError_t e = cudaSuccess;
+    LinkSrc src;
+    src.W = W; src.Wback = W_back;
+    src.vh = part ? g.Vh : gg.Vh;
+    src.off = part ? (long)g.t0 * gg.s3 : 0;
     do {
         if (!on_device) {
-            if ((e = cudaMalloc(&Wd, canon_bytes)) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(staging)", __LINE__); break; }
-            if ((e = cudaMemcpyAsync(Wd, W, canon_bytes, cudaMemcpyHostToDevice, t_stream)) != cudaSuccess) { rc = cuda_fail(e, "cudaMemcpyAsync(W)", __LINE__); break; }
+            if ((e = cudaMalloc(&Wd, 8 * (part ? plane_l : plane_g) * sizeof(double))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(staging)", __LINE__); break; }
+            if (local || !part) {
+                e = cudaMemcpyAsync(Wd, W, 8 * (part ? plane_l : plane_g) * sizeof(double), cudaMemcpyHostToDevice, t_stream);
+            } else {
+                for (int mp = 0; mp < 8 && e == cudaSuccess; ++mp)
+                    e = cudaMemcpyAsync(Wd + mp * plane_l, W + mp * plane_g + (size_t)src.off * 18, plane_l * sizeof(double), cudaMemcpyHostToDevice, t_stream);
+            }
+            if (e != cudaSuccess) { rc = cuda_fail(e, "cudaMemcpyAsync(W)", __LINE__); break; }
+            src.W = Wd;
+            if (part && nranks > 1) {
+                if ((e = cudaMalloc(&Wbd, 2 * slice * sizeof(double))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(staging)", __LINE__); break; }
+                if (local) {
+                    e = cudaMemcpyAsync(Wbd, W_back, 2 * slice * sizeof(double), cudaMemcpyHostToDevice, t_stream);
+                } else {
+                    const size_t tb = (size_t)((g.t0 + dims[3] - 1) % dims[3]) * slice;
+                    for (int pp = 0; pp < 2 && e == cudaSuccess; ++pp)
+                        e = cudaMemcpyAsync(Wbd + pp * slice, W + (size_t)(6 + pp) * plane_g + tb, slice * sizeof(double), cudaMemcpyHostToDevice, t_stream);
+                }
+                if (e != cudaSuccess) { rc = cuda_fail(e, "cudaMemcpyAsync(W_back)", __LINE__); break; }
+                src.Wback = Wbd;
+            }
         }
         if ((e = cudaMalloc(&L->L[STAG_PREC_F64], links_elems(L, 3) * sizeof(double2))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(links)", __LINE__); break; }
         if ((e = cudaMalloc(&err, sizeof(*err))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(err)", __LINE__); break; }
         if ((e = cudaMemsetAsync(err, 0, sizeof(*err), t_stream)) != cudaSuccess) { rc = cuda_fail(e, "cudaMemsetAsync", __LINE__); break; }
         const unsigned grid = (unsigned)((2L * g.Vh_pad + 127) / 128);
-        gather_links_kernel<<<grid, 128, 0, t_stream>>>((double2 *)L->L[STAG_PREC_F64], on_device ? W : Wd, g, gg, err, fold);
+        gather_links_kernel<<<grid, 128, 0, t_stream>>>((double2 *)L->L[STAG_PREC_F64], src, g, gg, err, fold);
         count_launch();
         if ((e = cudaGetLastError()) != cudaSuccess) { rc = cuda_fail(e, "gather_links_kernel", __LINE__); break; }
         unsigned long long bits = 0;
@@ -485,6 +528,7 @@ static int links_create(stag_links_t **links_out, const int dims[4], int antiper
         L->L_ready[STAG_PREC_F64].store(1, std::memory_order_release);
     } while (0);
     if (Wd) cudaFree(Wd);
+    if (Wbd) cudaFree(Wbd);
     if (err) cudaFree(err);
     if (rc != STAG_OK) { stag_links_destroy(L); return rc; }
     *links_out = L;

@@ -9,10 +9,23 @@
 // ------------------------------------------------------------------------------------
 extern "C" int stag_slab_connect_all(stag_links_t *L, void *const *regions);
 
+static int slab_finish_create(stag_links_t **slab_out, int rc, int nranks);
+
 extern "C" int stag_slab_create(stag_links_t **slab_out, const int global_dims[4], int antiperiodic_t,
                                 const double *W_global, int on_device, int rank, int nranks)
 {
-    int rc = links_create(slab_out, global_dims, antiperiodic_t, W_global, on_device, 0, rank, nranks);
+    return slab_finish_create(slab_out, links_create(slab_out, global_dims, antiperiodic_t, W_global, on_device, 0, rank, nranks), nranks);
+}
+
+extern "C" int stag_slab_create_local(stag_links_t **slab_out, const int global_dims[4], int antiperiodic_t,
+                                      const double *W_local, const double *W_back, int on_device,
+                                      int rank, int nranks)
+{
+    return slab_finish_create(slab_out, links_create(slab_out, global_dims, antiperiodic_t, W_local, on_device, 0, rank, nranks, W_back, true), nranks);
+}
+
+static int slab_finish_create(stag_links_t **slab_out, int rc, int nranks)
+{
     if (rc) return rc;
     stag_links *L = *slab_out;
     L->is_slab = 1;
@@ -193,6 +206,32 @@ extern "C" int stag_slab_set_wait_limit(stag_links_t *L, unsigned long long poll
     if (!L || !L->is_slab) return STAG_EINVAL;
     CU(cudaMemcpyAsync(&((XchHeader *)L->xch)->wait_limit, &polls, sizeof(polls), cudaMemcpyHostToDevice, t_stream));
     CU(cudaStreamSynchronize(t_stream));
+    return STAG_OK;
+}
+
+extern "C" int stag_slab_wait_stats(stag_links_t *L, unsigned long long *waits_spun_out, unsigned long long *polls_out)
+{
+    if (!L || !L->is_slab) return STAG_EINVAL;
+    unsigned long long v[2] = {0, 0};
+    CU(cudaMemcpyAsync(v, &((XchHeader *)L->xch)->waits_spun, sizeof(v), cudaMemcpyDeviceToHost, t_stream));
+    CU(cudaStreamSynchronize(t_stream));
+    if (waits_spun_out) *waits_spun_out = v[0];
+    if (polls_out) *polls_out = v[1];
+    return STAG_OK;
+}
+
+extern "C" int stag_slab_reset(stag_links_t *L)
+{
+    if (!L || !L->is_slab) return STAG_EINVAL;
+    CU(cudaStreamSynchronize(t_stream));
+    unsigned long long limit = 0;
+    XchHeader *hdr = (XchHeader *)L->xch;
+    CU(cudaMemcpyAsync(&limit, &hdr->wait_limit, sizeof(limit), cudaMemcpyDeviceToHost, t_stream));
+    CU(cudaStreamSynchronize(t_stream));
+    CU(cudaMemsetAsync(L->xch, 0, XCH_HDR, t_stream));        // flags, counts, tickets, the mark, reduction slots and flags
+    CU(cudaMemcpyAsync(&hdr->wait_limit, &limit, sizeof(limit), cudaMemcpyHostToDevice, t_stream));
+    CU(cudaStreamSynchronize(t_stream));
+    L->epoch = 0;
     return STAG_OK;
 }
 

@@ -52,6 +52,7 @@ face_push_kernel(const cplx_t<T> *__restrict__ in, const int Vh, const int Vh_pa
                  char *mine, char *peer_fwd, char *peer_bwd)
 {
     XchHeader *hdr = (XchHeader *)mine;
+    if (slab_dead(mine)) return;              // watchdog fired earlier: publish nothing (stag_dslash.cuh)
     // every block reads the count before it takes its ticket; the last block bumps it afterwards
     const unsigned long long epoch = __ldcg(&hdr->epoch) + 1;
     cplx_t<T> *fwd_back = (cplx_t<T> *)(peer_fwd + xch_halo_offset(s3, epoch, 0));
@@ -85,6 +86,7 @@ slab_xpay_push_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const 
                       const int Vh, const int Vh_pad, const int s3, char *mine, char *peer_fwd, char *peer_bwd)
 {
     if (ctrl->state != CG_RUN || !ctrl->active[0]) return;     // the same in every block: no ticket taken
+    if (slab_dead(mine)) return;
     using V = typename Vec4<T>::type;
     constexpr int N = Vec4<T>::N;
     constexpr int CPK = N / 2;                                 // complex numbers per packet
@@ -146,12 +148,14 @@ __device__ __forceinline__ void publish_total(char *const *peers, int nranks, in
 }
 
 // Any thread: the sum over ranks of reduction seq, added in rank order (same bits on every rank).
-__device__ __forceinline__ double gather_total(char *mine, int nranks, unsigned long long seq)
+// *ok = false when a wait gave up (the slab is then marked dead; the sum is not to be used).
+__device__ __forceinline__ double gather_total(char *mine, int nranks, unsigned long long seq, bool *ok)
 {
     const XchReduce *R = (const XchReduce *)(mine + XCH_RED);
     double t = 0.0;
+    *ok = true;
     for (int r = 0; r < nranks; ++r) {
-        wait_flag(&R->flag[r], seq, (XchHeader *)mine);
+        if (!wait_flag(&R->flag[r], seq, (XchHeader *)mine)) { *ok = false; return 0.0; }
         t += __ldcg(&R->slot[seq & 1ull][r]);
     }
     return t;
@@ -176,9 +180,9 @@ __device__ __forceinline__ void publish_next(const Comm &c, double value)
     hdr->red_seq = seq;
 }
 // any thread of a kernel launched after the publishing one
-__device__ __forceinline__ double gather_current(const Comm &c)
+__device__ __forceinline__ double gather_current(const Comm &c, bool *ok)
 {
-    return gather_total(c.mine, c.nranks, __ldcg(&((const XchHeader *)c.mine)->red_seq));
+    return gather_total(c.mine, c.nranks, __ldcg(&((const XchHeader *)c.mine)->red_seq), ok);
 }
 
 // Local fixed-order sum of the second hop's per-block partials of <d,Ad>, published to all ranks.
@@ -186,7 +190,7 @@ __global__ void __launch_bounds__(1024)
 slab_publish_partials_kernel(const double *__restrict__ partials, int n, const Comm c,
                              const CgCtrl *__restrict__ ctrl)
 {
-    if (ctrl->state != CG_RUN) return;
+    if (ctrl->state != CG_RUN || slab_dead(c.mine)) return;
     __shared__ double red[32];
     const double t = block_total_fixed(partials, n, red);
     if (threadIdx.x == 0) publish_next(c, t);
@@ -200,14 +204,16 @@ slab_update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d
                    const T *__restrict__ q, long n, double *__restrict__ partials,
                    CgCtrl *__restrict__ ctrl, const Comm c)
 {
-    if (ctrl->state != CG_RUN) return;
+    if (ctrl->state != CG_RUN || slab_dead(c.mine)) return;
     using V = typename Vec4<T>::type;
     constexpr int N = Vec4<T>::N;
     __shared__ double red[32];
     __shared__ double totals[MAX_RHS];
     __shared__ double s_dAd;
-    if (threadIdx.x == 0) s_dAd = gather_current(c);     // every block reads red_seq before the last one bumps it
+    __shared__ bool s_ok;
+    if (threadIdx.x == 0) s_dAd = gather_current(c, &s_ok);     // every block reads red_seq before the last one bumps it
     __syncthreads();
+    if (!s_ok) return;            // a peer never published <d,Ad>: leave y, r alone and publish nothing
     const double dAd = s_dAd;
     const bool ok = dAd > 0.0;
     const double alpha_d = ok ? ctrl->delta[0] / dAd : 0.0;
@@ -246,6 +252,7 @@ slab_residual_kernel(double *__restrict__ r, const double *__restrict__ b,
                      const double *__restrict__ q, T *__restrict__ r_lo, long n, long n_plane, long n_valid,
                      double *__restrict__ partials, CgCtrl *__restrict__ ctrl, const Comm c)
 {
+    if (slab_dead(c.mine)) return;
     double s = 0.0;
     for (long i = blockIdx.x * (long)BLAS_BLOCK + threadIdx.x; i < n; i += (long)gridDim.x * BLAS_BLOCK) {
         const double bi = (n_valid == n_plane || i % n_plane < n_valid) ? b[i] : 0.0;   // b's pad lanes count as zero
@@ -274,7 +281,10 @@ __global__ void slab_scalar_kernel(CgCtrl *__restrict__ ctrl, const Comm c)
 {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     if (WHAT == SCALAR_ITER && ctrl->state != CG_RUN) return;
-    double total = gather_current(c);
+    if (slab_dead(c.mine)) return;
+    bool ok;
+    double total = gather_current(c, &ok);
+    if (!ok) return;              // the scalars stay as they were; the host reads STAG_ETIMEOUT from the header
     if (WHAT == SCALAR_ITER) cg_iteration_epilogue(ctrl, &total);
     else residual_epilogue<WHAT>(ctrl, &total);
 }

@@ -52,6 +52,14 @@ def neighbours(rank: int, nranks: int):
     return (rank - 1) % nranks, (rank + 1) % nranks
 
 
+def stag_vh(dims) -> int:
+    """Sites of one parity."""
+    v = 1
+    for d in dims:
+        v *= int(d)
+    return v // 2
+
+
 def slice_sites(global_dims) -> int:
     """s3: sites of one parity in one time slice."""
     return int(global_dims[0]) * int(global_dims[1]) * int(global_dims[2]) // 2
@@ -62,6 +70,15 @@ def scatter_spinor(chi_global, global_dims, rank: int, nranks: int):
     t0, t1 = slab_range(global_dims, rank, nranks)
     s3 = slice_sites(global_dims)
     return chi_global[t0 * s3:t1 * s3]
+
+
+def scatter_links(W_global, global_dims, rank: int, nranks: int):
+    """(W_local, W_back) for stag_slab_create_local: the rank's own time slices of the canonical
+    links W[mu][p][cb][3][3] and the t-links leaving the slice before the slab (slicing only)."""
+    t0, t1 = slab_range(global_dims, rank, nranks)
+    s3 = slice_sites(global_dims)
+    tb = (t0 - 1) % int(global_dims[3])
+    return W_global[:, :, t0 * s3:t1 * s3], W_global[3, :, tb * s3:(tb + 1) * s3]
 
 
 def gather_spinor(parts, global_dims):
@@ -96,9 +113,11 @@ def exchange_handles(my_handle: bytes, rank: int, nranks: int, group=None):
 
 # ---- the handle --------------------------------------------------------------------------
 class SlabLinks:
-    """One rank's slab (stag_slab_create).  W: canonical complex128 links of the WHOLE lattice."""
+    """One rank's slab.  W: canonical complex128 links of the WHOLE lattice (stag_slab_create; only
+    the rank's part goes to the device), or, with W_back given, of the rank's OWN time slices
+    (stag_slab_create_local, see scatter_links): no rank then needs the whole field."""
 
-    def __init__(self, global_dims, W, rank: int, nranks: int, antiperiodic_t: bool = True):
+    def __init__(self, global_dims, W, rank: int, nranks: int, antiperiodic_t: bool = True, W_back=None):
         import numpy as np
         torch = stag._require_cuda()
         stag.use_current_stream()
@@ -108,9 +127,19 @@ class SlabLinks:
         self._h = ctypes.c_void_p()
         self._opened = []
         W = np.ascontiguousarray(W, dtype=np.complex128)
-        stag._check(stag.lib().stag_slab_create(ctypes.byref(self._h), stag._cdims(self.global_dims),
-                                                int(bool(antiperiodic_t)), ctypes.c_void_p(W.ctypes.data), 0,
-                                                self.rank, self.nranks))
+        if W_back is None:
+            if W.shape[2] != stag_vh(self.global_dims):
+                raise ValueError("W must cover the whole lattice when W_back is not given")
+            stag._check(stag.lib().stag_slab_create(ctypes.byref(self._h), stag._cdims(self.global_dims),
+                                                    int(bool(antiperiodic_t)), ctypes.c_void_p(W.ctypes.data), 0,
+                                                    self.rank, self.nranks))
+        else:
+            Wb = np.ascontiguousarray(W_back, dtype=np.complex128)
+            if W.shape[:3] != (4, 2, stag_vh(self.dims)) or Wb.shape[:2] != (2, slice_sites(self.global_dims)):
+                raise ValueError("W_local / W_back have the wrong shape for this slab")
+            stag._check(stag.lib().stag_slab_create_local(ctypes.byref(self._h), stag._cdims(self.global_dims),
+                                                          int(bool(antiperiodic_t)), ctypes.c_void_p(W.ctypes.data),
+                                                          ctypes.c_void_p(Wb.ctypes.data), 0, self.rank, self.nranks))
         torch.cuda.current_stream().synchronize()
 
     @property
@@ -214,6 +243,18 @@ class SlabLinks:
         """Watchdog of the acquire-waits (stag_slab_set_wait_limit); 0 = the default (~10 s)."""
         stag.use_current_stream()
         stag._check(stag.lib().stag_slab_set_wait_limit(self._h, int(polls)))
+
+    def reset(self):
+        """Revive a slab whose watchdog fired (stag_slab_reset): collective, see include/stag.h."""
+        stag.use_current_stream()
+        stag._check(stag.lib().stag_slab_reset(self._h))
+
+    def wait_stats(self):
+        """(waits that had to spin, polls they spent) since creation / reset (stag_slab_wait_stats)."""
+        stag.use_current_stream()
+        a, b = ctypes.c_ulonglong(), ctypes.c_ulonglong()
+        stag._check(stag.lib().stag_slab_wait_stats(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return a.value, b.value
 
     def status(self) -> int:
         """stag.OK, or stag.ETIMEOUT once a kernel of this slab gave up waiting for a peer."""

@@ -64,6 +64,33 @@ def test_slab_hop_matches_oracle_and_whole_lattice_kernel(dims, nranks, prec):
             assert float(planes[:, vh:, :].abs().max()) == 0.0 if planes.shape[1] > vh else True
 
 
+@pytest.mark.parametrize("dims,nranks", [((4, 4, 4, 8), 2), ((6, 2, 2, 12), 3), ((4, 4, 4, 4), 1), ((2, 2, 2, 8), 4)])
+def test_slab_from_its_own_time_slices_equals_slab_from_the_whole_field(dims, nranks):
+    """stag_slab_create_local: a rank hands over only its own time slices of the links plus the
+    t-links of the slice before them (slab.scatter_links), never the whole lattice.  Both hops, all
+    four link forms: bitwise equal to the slabs made from the whole field, and within tolerance of
+    the oracle (which only ever sees the whole field)."""
+    W = fieldgen.links(dims, "random", seed=63)
+    whole = make_slabs(dims, W, nranks)
+    local = []
+    for r in range(nranks):
+        Wl, Wb = slab.scatter_links(W, dims, r, nranks)
+        local.append(slab.SlabLinks(dims, Wl, r, nranks, W_back=Wb))
+    slab.connect_in_process(local)
+    for parity in (0, 1):
+        chi = fieldgen.spinor_gaussian(dims, 1 - parity, seed=64 + parity)
+        ref = oracle.dslash(chi, W, dims, parity)
+        for prec in ALL_PREC:
+            _, a = slab_hop_all(whole, chi, dims, parity, prec)
+            _, b = slab_hop_all(local, chi, dims, parity, prec)
+            assert np.array_equal(a, b)
+            assert rel_l2(b, ref) <= TOL[prec]
+    with pytest.raises(ValueError):
+        slab.SlabLinks(dims, W[:, :, :7], 0, nranks)                    # neither whole nor local + back
+    for s in whole + local:
+        s.close()
+
+
 @pytest.mark.parametrize("prec", ALL_PREC)
 def test_slab_hop_periodic_time_boundary(prec):
     dims = (4, 4, 2, 8)

@@ -1,0 +1,186 @@
+"""The T-slab path under REAL concurrency on one GPU: the slabs of a decomposition live in one
+process, each driven by its own host thread on its own CUDA stream, with no fence between phases.
+The lattices are small enough for all slabs' kernels to be resident at the same time, so the
+kernels of different ranks genuinely overlap and the acquire-waits (wait_flag, stag_dslash.cuh:
+halo flags in the hop, reduction flags in the global sums) genuinely spin on a peer that is still
+running or has not been launched yet -- what test_gpu_slab.py (lockstep) and test_gpu_slab_ipc.py
+(a fence after every phase) never do.  The parity checks are those of test_gpu_slab_multi.py (one
+GPU per rank), which needs a box with several GPUs.
+
+Each test first runs the same work in lockstep once: that loads every kernel and makes every
+allocation, neither of which may happen while another slab's kernel is spinning (lazy module
+loading and cudaFree synchronise the device).  A threading.Barrier stands where a real run has
+dist.barrier(): before the first exchange, so that rank skew does not eat the watchdog's budget;
+after it rank r deliberately starts 20 ms x r late, so that the first waits are certain to spin
+(stag_slab_wait_stats counts them, and the tests assert the count).  The watchdog is lowered so
+a protocol error ends as STAG_ETIMEOUT, not as a hang."""
+import threading
+import time
+
+import numpy as np
+import pytest
+
+import fieldgen
+import oracle
+import paper_1111_0125_b200 as stag
+from paper_1111_0125_b200 import slab
+from tests.parity import rel_err
+
+pytestmark = pytest.mark.gpu
+
+WAIT_LIMIT = 1 << 22          # polls of >= 200 ns: a few seconds
+
+
+def make_slabs(dims, W, nranks):
+    slabs = [slab.SlabLinks(dims, W, r, nranks) for r in range(nranks)]
+    slab.connect_in_process(slabs)
+    for s in slabs:
+        s.set_wait_limit(WAIT_LIMIT)
+    return slabs
+
+
+def run_ranks(nranks, body):
+    """body(rank) on one host thread and one CUDA stream per rank; returns the results in rank order.
+    A failing rank's exception is re-raised here (the others then run into the watchdog)."""
+    import torch
+    streams = [torch.cuda.Stream() for _ in range(nranks)]
+    gate = threading.Barrier(nranks)
+    out, err = [None] * nranks, [None] * nranks
+
+    def worker(r):
+        try:
+            torch.cuda.set_device(0)
+            with torch.cuda.stream(streams[r]):
+                gate.wait(timeout=60)
+                out[r] = body(r)
+                streams[r].synchronize()
+        except BaseException as e:          # noqa: BLE001 -- reported to the main thread
+            err[r] = e
+
+    torch.cuda.synchronize()
+    threads = [threading.Thread(target=worker, args=(r,)) for r in range(nranks)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=300)
+        assert not t.is_alive(), "a rank's thread is still running"
+    for e in err:
+        if e is not None:
+            raise e
+    return out
+
+
+@pytest.mark.parametrize("dims,nranks", [((4, 4, 4, 8), 2), ((4, 4, 4, 16), 4), ((8, 8, 8, 16), 2)])
+def test_hops_back_to_back_from_one_thread_per_slab(dims, nranks):
+    """Forty push + hop pairs per rank with no host synchronisation anywhere: a rank may run ahead of
+    its neighbours by as much as the double-buffered halo allows, and its boundary threads wait for
+    real.  Every rank's last result must equal the lockstep result bitwise and the oracle within tolerance."""
+    W = fieldgen.links(dims, "random", seed=71)
+    chi = fieldgen.spinor_gaussian(dims, 0, seed=72)
+    ref = oracle.dslash(chi, W, dims, 1)
+    slabs = make_slabs(dims, W, nranks)
+    spun = []
+    for prec, tol in ((stag.PREC_F64, 1e-13), (stag.PREC_F32_R12, 2e-6)):
+        vs = [stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(chi, dims, r, nranks)), slabs[r].dims, prec)
+              for r in range(nranks)]
+        for r in range(nranks):                      # lockstep: loads the kernels, gives the expected bits
+            slabs[r].push(vs[r], prec)
+        lock = [slabs[r].hop(vs[r], 1, prec).clone() for r in range(nranks)]
+        outs = [stag.empty_spinor(slabs[r].dims, prec) for r in range(nranks)]
+
+        def body(r):
+            time.sleep(0.02 * r)                 # rank skew: rank 0's first hop is certain to wait for its neighbours' pushes
+            for _ in range(40):
+                slabs[r].dslash(vs[r], 1, prec, out=outs[r])
+            return slabs[r].status()
+
+        assert sum(s.wait_stats()[0] for s in slabs) == 0      # lockstep so far: nobody ever had to wait
+        assert run_ranks(nranks, body) == [stag.OK] * nranks
+        spun.append(sum(s.wait_stats()[0] for s in slabs))
+        for s in slabs:
+            s.reset()                                          # clears the counters too (all streams idle here)
+        for r in range(nranks):
+            assert bool((outs[r] == lock[r]).all())
+            got = stag.spinor_unpack(outs[r], slabs[r].dims, prec)
+            assert rel_err(got, slab.scatter_spinor(ref, dims, r, nranks)) <= tol
+    # the point of the test: some boundary thread really did find its flag not yet set and spun
+    assert sum(spun) > 0, "no acquire-wait ever spun: the ranks did not run concurrently"
+    for s in slabs:
+        s.close()
+
+
+@pytest.mark.parametrize("dims,nranks,mass", [((4, 4, 4, 8), 2, 0.1), ((4, 4, 4, 16), 4, 0.1), ((8, 8, 8, 16), 2, 0.05)])
+@pytest.mark.parametrize("mode", [stag.CG_F64, stag.CG_RELIABLE])
+def test_slab_cg_run_from_one_thread_per_slab(dims, nranks, mass, mode):
+    """stag_slab_cg_run -- the call of a one-process-per-GPU run: CUDA-graph replays of whole chunks of
+    iterations, the in-kernel pushes of hop 1 and of the direction update, global sums through the
+    exchange regions -- issued concurrently by every rank's own thread.  Solution against the oracle's
+    solve (1e-8), true residual with the oracle's A, identical scalars on every rank."""
+    tol = 1e-10
+    W = fieldgen.links(dims, "random", seed=73)
+    b = fieldgen.spinor_gaussian(dims, 0, seed=74)
+    x_ref, _, _, _, rc = oracle.cg(b, W, dims, mass, 1e-12, 50000)
+    assert rc == 0
+    slabs = make_slabs(dims, W, nranks)
+    bs = [stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(b, dims, r, nranks)), slabs[r].dims, 0)
+          for r in range(nranks)]
+    slab.cg_solve_in_process(slabs, bs, mass, tol, 20000, mode, recon12=True, chunk=8)     # lockstep warm-up
+    assert sum(s.wait_stats()[0] for s in slabs) == 0          # lockstep: nobody ever had to wait
+
+    def body(r):
+        time.sleep(0.02 * r)                     # rank skew: the first global sum is certain to wait for the last rank
+        return slabs[r].cg_solve(bs[r], mass, tol, 20000, mode, recon12=True, chunk=8)
+
+    res = run_ranks(nranks, body)
+    sts = [st for _, st in res]
+    assert all(st["status"] == stag.OK and st["true_resid"] <= tol for st in sts), sts
+    for st in sts[1:]:
+        assert (st["iters"], st["true_resid"], st["n_updates"]) == (sts[0]["iters"], sts[0]["true_resid"], sts[0]["n_updates"])
+    x = slab.gather_spinor([stag.spinor_unpack(res[r][0], slabs[r].dims, 0) for r in range(nranks)], dims)
+    assert rel_err(x, x_ref) <= 1e-8
+    resid = np.linalg.norm((b - oracle.apply_A(x, W, dims, mass)).ravel()) / np.linalg.norm(b.ravel())
+    assert resid <= tol * (1 + 1e-3)
+    assert all(s.status() == stag.OK for s in slabs)
+    # the point of the test: halo and reduction waits really spun on peers that were still running
+    assert sum(s.wait_stats()[0] for s in slabs) > 0, "no acquire-wait ever spun: the ranks did not run concurrently"
+    for s in slabs:
+        s.close()
+
+
+def test_a_dead_slab_takes_its_neighbours_down_and_reset_revives_them():
+    """Rank 0 hops after an exchange rank 1 never joined: its watchdog fires.  From then on rank 0
+    publishes nothing, so rank 1 -- whose first exchange still completes, rank 0's push preceded its
+    death -- times out on the next one instead of reading stale faces: every rank ends with
+    STAG_ETIMEOUT.  stag_slab_reset on both brings the pair back, and the hop is right again."""
+    dims = (4, 4, 4, 8)
+    W = fieldgen.links(dims, "random", seed=75)
+    chi = fieldgen.spinor_gaussian(dims, 0, seed=76)
+    ref = oracle.dslash(chi, W, dims, 1)
+    slabs = make_slabs(dims, W, 2)
+    for s in slabs:
+        s.set_wait_limit(2000)
+    prec = stag.PREC_F64
+    vs = [stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(chi, dims, r, 2)), slabs[r].dims, prec) for r in range(2)]
+    slabs[0].push(vs[0], prec)
+    slabs[0].hop(vs[0], 1, prec)                      # waits for rank 1's push of exchange 1: never comes
+    assert slabs[0].status() == stag.ETIMEOUT and slabs[1].status() == stag.OK
+    slabs[1].push(vs[1], prec)
+    o1 = slabs[1].hop(vs[1], 1, prec)                 # exchange 1 was pushed by rank 0 before it died
+    assert slabs[1].status() == stag.OK
+    assert rel_err(stag.spinor_unpack(o1, slabs[1].dims, prec), slab.scatter_spinor(ref, dims, 1, 2)) <= 1e-13
+    slabs[0].push(vs[0], prec)                        # a dead slab's push is a no-op
+    slabs[1].push(vs[1], prec)
+    slabs[1].hop(vs[1], 1, prec)                      # exchange 2 from rank 0 never arrives
+    assert slabs[1].status() == stag.ETIMEOUT
+    for s in slabs:
+        s.reset()
+    assert [s.status() for s in slabs] == [stag.OK, stag.OK]
+    for rep in range(3):
+        for r in range(2):
+            slabs[r].push(vs[r], prec)
+        outs = [slabs[r].hop(vs[r], 1, prec) for r in range(2)]
+    got = slab.gather_spinor([stag.spinor_unpack(outs[r], slabs[r].dims, prec) for r in range(2)], dims)
+    assert rel_err(got, ref) <= 1e-13
+    assert [s.status() for s in slabs] == [stag.OK, stag.OK]
+    for s in slabs:
+        s.close()

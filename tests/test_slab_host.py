@@ -72,6 +72,32 @@ def test_only_the_two_boundary_slices_of_a_slab_need_the_neighbours():
         assert np.array_equal(out2[t0 + 1:t1], refr[t0 + 1:t1])
 
 
+def test_a_slab_needs_only_its_own_links_and_the_t_links_of_the_slice_before_it():
+    """What stag_slab_create_local is given (slab.scatter_links), stated with the oracle alone: take a
+    DIFFERENT gauge field, overwrite the slab's own time slices and the t-links leaving slice t0-1
+    with those of W, and the hop on the slab's sites is the hop with W -- for both parities.
+    Without the t-links of slice t0-1 the slab's first slice (and only it) changes."""
+    dims, nranks = (4, 2, 4, 12), 3
+    W = fieldgen.links(dims, "random", seed=6)
+    s3 = slab.slice_sites(dims)
+    for parity in (0, 1):
+        chi = fieldgen.spinor_gaussian(dims, 1 - parity, seed=7 + parity)
+        ref = oracle.dslash(chi, W, dims, parity).reshape(dims[3], s3, 3)
+        for r in range(nranks):
+            t0, t1 = slab.slab_range(dims, r, nranks)
+            Wl, Wb = slab.scatter_links(W, dims, r, nranks)
+            assert Wl.shape == (4, 2, (t1 - t0) * s3, 3, 3) and Wb.shape == (2, s3, 3, 3)
+            other = fieldgen.links(dims, "random", seed=99)
+            other[:, :, t0 * s3:t1 * s3] = Wl
+            no_back = other.copy()
+            tb = (t0 - 1) % dims[3]
+            other[3, :, tb * s3:(tb + 1) * s3] = Wb
+            out = oracle.dslash(chi, other, dims, parity).reshape(dims[3], s3, 3)
+            assert np.array_equal(out[t0:t1], ref[t0:t1])
+            out2 = oracle.dslash(chi, no_back, dims, parity).reshape(dims[3], s3, 3)
+            assert not np.array_equal(out2[t0], ref[t0]) and np.array_equal(out2[t0 + 1:t1], ref[t0 + 1:t1])
+
+
 def _free_port():
     s = socket.socket()
     s.bind(("127.0.0.1", 0))
