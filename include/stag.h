@@ -327,6 +327,11 @@ typedef struct stag_cg_params {
                              (default 32); < 0 disables graphs (plain launches)               */
     int    recon12_f64;   /* 1: the fp64 correction steps use 12-real links too               */
     int    recon8;        /* 1: the iteration's Dslash uses 8-parameter links (overrides recon12) */
+    int    persistent;    /* the iteration as ONE persistent cooperative kernel per chunk of passes
+                             (grid barriers instead of four kernel boundaries per pass; one
+                             right-hand side, 18- or 12-real links): 1 = yes, -1 = no, 0 = the
+                             library decides by lattice volume         */
+    int    persist_chunk; /* passes per persistent launch between host checks (default 1024) */
 } stag_cg_params_t;
 
 typedef struct stag_cg_stats {
@@ -420,6 +425,16 @@ int stag_slab_cg_control(stag_links_t *slab, int *action_out);
 int stag_slab_cg_step(stag_links_t *slab, int action, int phase, int *more_out);
 /* Returns STAG_OK / STAG_ENOCONV / STAG_EBREAKDOWN like stag_cg_solve; stats as there. */
 int stag_slab_cg_finish(stag_links_t *slab, stag_cg_stats_t *stats_out);
+/* One STAG_SLAB_ACT_ITER (up to persist_chunk passes of the loop) of the n slabs given, in ONE
+ * cooperative launch of the persistent iteration kernel: each slab's blocks form a rank group with
+ * its own barrier, and the groups talk only through the exchange regions.  n = 1: what a process of
+ * a one-process-per-GPU run launches for its own slab (stag_slab_cg_run does, with
+ * params->persistent = 1).  n = nranks with all slabs on the calling thread's device: the
+ * single-GPU emulation of the multi-GPU run -- the ranks' kernels run concurrently and really wait
+ * for each other, which separate launches on one device cannot promise.  Replaces the phases of
+ * that action in the stepped loop; every slab must have been told STAG_SLAB_ACT_ITER by
+ * stag_slab_cg_control.  18- and 12-real links. */
+int stag_slab_cg_iter_all(stag_links_t *const *slabs, int n);
 /* begin + the loop above + finish: the call of a one-process-per-GPU run (all ranks together).
  * Slabs sharing a device may call it too -- one host thread and one stream per slab -- as long as
  * all their kernels can be resident at the same time (small lattices; tests/test_gpu_slab_concurrent.py):

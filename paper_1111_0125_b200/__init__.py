@@ -76,7 +76,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 class _Params(ctypes.Structure):
     _fields_ = [("eps_in", ctypes.c_double), ("recon12", ctypes.c_int),
-                ("graph_chunk", ctypes.c_int), ("recon12_f64", ctypes.c_int), ("recon8", ctypes.c_int)]
+                ("graph_chunk", ctypes.c_int), ("recon12_f64", ctypes.c_int), ("recon8", ctypes.c_int),
+                ("persistent", ctypes.c_int), ("persist_chunk", ctypes.c_int)]
 
 
 class _Stats(ctypes.Structure):
@@ -144,6 +145,7 @@ SIGNATURES = {
     "stag_slab_cg_control": (ctypes.c_int, [_vp, _ip]),
     "stag_slab_cg_step": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _ip]),
     "stag_slab_cg_finish": (ctypes.c_int, [_vp, ctypes.POINTER(_Stats)]),
+    "stag_slab_cg_iter_all": (ctypes.c_int, [ctypes.POINTER(_vp), ctypes.c_int]),
     "stag_slab_cg_run": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                         ctypes.c_int, ctypes.POINTER(_Params), ctypes.POINTER(_Stats)]),
     "stag_cg_solve_host": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double,
@@ -350,9 +352,11 @@ def apply_A(v_even, links: Links, mass: float, prec, out=None):
     return out
 
 
-def _params(eps_in, recon12, graph_chunk, recon12_f64, recon8=False):
+def _params(eps_in, recon12, graph_chunk, recon12_f64, recon8=False, persistent=None, persist_chunk=None):
     p = _Params()
     p.recon8 = int(bool(recon8))
+    p.persistent = 0 if persistent is None else (1 if persistent else -1)
+    p.persist_chunk = int(persist_chunk or 0)
     p.eps_in = float(eps_in or 0.0)
     p.recon12 = int(bool(recon12))
     p.graph_chunk = int(graph_chunk or 0)
@@ -367,14 +371,16 @@ def _stats_dict(st: _Stats, status: int):
 
 
 def cg_solve(b, links: Links, mass: float, tol: float, maxiter: int, mode: int = CG_RELIABLE,
-             x0=None, eps_in=None, recon12=False, graph_chunk=None, recon12_f64=False, recon8=False):
+             x0=None, eps_in=None, recon12=False, graph_chunk=None, recon12_f64=False, recon8=False,
+             persistent=None, persist_chunk=None):
     """Solve A x = b on the even sites.  b, x0: fp64 device spinors.  Returns (x, stats dict);
-    stats["status"] is 0, ENOCONV or EBREAKDOWN.  Errors (< 0) raise StagError."""
+    stats["status"] is 0, ENOCONV or EBREAKDOWN.  Errors (< 0) raise StagError.
+    persistent: True / False forces the persistent-kernel iteration on / off, None = by volume."""
     torch = _require_cuda()
     use_current_stream()
     x = torch.zeros_like(b) if x0 is None else x0.clone()
     st = _Stats()
-    p = _params(eps_in, recon12, graph_chunk, recon12_f64, recon8)
+    p = _params(eps_in, recon12, graph_chunk, recon12_f64, recon8, persistent, persist_chunk)
     rc = lib().stag_cg_solve_ex(ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(b.data_ptr()),
                                 links.handle, float(mass), float(tol), int(maxiter), int(mode),
                                 ctypes.byref(p), ctypes.byref(st))

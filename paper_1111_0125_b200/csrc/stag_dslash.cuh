@@ -177,6 +177,78 @@ __device__ __forceinline__ bool slab_dead(const char *xch)
     return __ldcg(&((const XchHeader *)xch)->timed_out) != 0u;
 }
 
+// One output site, one right-hand side: acc[i] = sum_d (M_d(x) chi(nbr_d(x)))_i -- the arithmetic of
+// eq. 2.5 and its order, shared by dslash_kernel (N = 1) and the persistent iteration kernel
+// (stag_persist.cuh), so that the two produce the same bits per site.  All 24 neighbour loads are
+// issued before the link stream; the links arrive in groups of KG 16-byte packets (HopTune).
+// HALO: the +-t neighbours of the slab's first / last time slice come from the halo buffers of
+// exchange epoch() once the slab's own flag shows it (decode_site wrapped them onto the slab's other
+// end; their in-slice index addresses the buffers).  epoch() is only evaluated by boundary threads.
+// NC: the input spinor is read-only for the whole kernel (non-coherent loads, the plain kernels);
+// false inside the persistent kernel, where another phase of the same launch wrote it.
+template <typename T, int NR, bool HALO, bool NC = true, typename EpochFn>
+__device__ __forceinline__ void hop_site(cplx_t<T> (&acc)[3], const cplx_t<T> *__restrict__ in,
+                                         const pkt_t<T> *__restrict__ links, const Geom &g, const int cb,
+                                         const Site &s, const unsigned neg, char *xch, EpochFn epoch)
+{
+    using C = cplx_t<T>;
+    using P = pkt_t<T>;
+    constexpr int K = link_slots(NR);
+    constexpr int GM = HopTune<T, NR, 1>::GM;
+    constexpr int DPG = Pkt<T>::CPP * GM;     // directions per group
+    constexpr int NG = 8 / DPG;               // groups per site
+    constexpr int KG = K * GM;                // packets per group
+    static_assert(8 % DPG == 0, "group must divide the eight directions");
+    const P *L = links + (size_t)(cb >> 5) * (size_t)(NG * KG * TILE) + (cb & 31);
+    C v1[8][3];
+#pragma unroll
+    for (int d = 0; d < 8; ++d)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            if constexpr (NC) v1[d][c] = ld_keep_nc(in + (size_t)c * g.Vh_pad + s.nbr[d]);
+            else v1[d][c] = ld_keep(in + (size_t)c * g.Vh_pad + s.nbr[d]);
+        }
+    if constexpr (HALO) {
+        XchHeader *hdr = (XchHeader *)xch;
+        if (s.x3 == g.X3 - 1) {
+            const unsigned long long e = epoch();
+            const C *fwd = (const C *)(xch + xch_halo_offset(g.s3, e, 1));
+            wait_flag(&hdr->flag_fwd, e, hdr);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) v1[3][c] = __ldcg(fwd + (size_t)c * g.s3 + s.nbr[3]);
+        }
+        if (s.x3 == 0) {
+            const unsigned long long e = epoch();
+            const C *back = (const C *)(xch + xch_halo_offset(g.s3, e, 0));
+            wait_flag(&hdr->flag_back, e, hdr);
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+                v1[7][c] = __ldcg(back + (size_t)c * g.s3 + (s.nbr[7] - (g.X3 - 1) * g.s3));
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) acc[i] = mk<T>(0, 0);
+#pragma unroll
+    for (int grp = 0; grp < NG; ++grp) {
+        P pk[KG];
+#pragma unroll
+        for (int i = 0; i < KG; ++i) pk[i] = ld_stream(L + (grp * KG + i) * TILE);
+#pragma unroll
+        for (int dd = 0; dd < DPG; ++dd) {
+            const int d = grp * DPG + dd;
+            C m[9];
+#pragma unroll
+            for (int k = 0; k < K; ++k) m[k] = pk_get(pk, dd * K + k);
+            if (NR == 2) rebuild_row2<T>(m, (neg >> d) & 1u);
+            if (NR == 1) rebuild_from8<T>(m, (neg >> d) & 1u);
+#pragma unroll
+            for (int i = 0; i < 3; ++i)
+#pragma unroll
+                for (int j = 0; j < 3; ++j) cfma(acc[i], m[3 * i + j], v1[d][j]);
+        }
+    }
+}
+
 // T: float or double.  NR: storage of each link (3 = 18-real, 2 = 12-real rows 0,1, 1 = 8-parameter).
 // N: right-hand sides handled by one thread.  Two batch layouts (include/stag.h "batch layouts"):
 //   blocked (PAIRED = false): spinor k of a batch starts rs complex numbers after spinor k-1
@@ -246,94 +318,65 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
         unsigned neg = 0;
         if (NR != 3) neg = det_sign_mask(g, s);
 
-        // one right-hand side: all 24 neighbour loads are issued before the link stream;
-        // several: the neighbours of one group of directions at a time (register budget)
-        constexpr int V1D = (N == 1) ? 8 : 1, VGN = (N == 1) ? 1 : N, VGD = (N == 1) ? 1 : DPG;
-        C v1[V1D][3];
-        if constexpr (N == 1) {
-#pragma unroll
-            for (int d = 0; d < 8; ++d)
-#pragma unroll
-                for (int c = 0; c < 3; ++c) v1[d][c] = ld_keep_nc(in + (size_t)c * g.Vh_pad + s.nbr[d]);
-            if constexpr (HALO) {
-                // decode_site wrapped the +-t neighbours of the boundary slices onto the slab's
-                // own other end; their in-slice index is what addresses the halo buffers
-                XchHeader *hdr = (XchHeader *)halo.xch;
-                if (s.x3 == g.X3 - 1) {
-                    const unsigned long long e = __ldcg(&hdr->epoch);
-                    const C *fwd = (const C *)(halo.xch + xch_halo_offset(g.s3, e, 1));
-                    wait_flag(&hdr->flag_fwd, e, hdr);
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) v1[3][c] = __ldcg(fwd + (size_t)c * g.s3 + s.nbr[3]);
-                }
-                if (s.x3 == 0) {
-                    const unsigned long long e = __ldcg(&hdr->epoch);
-                    const C *back = (const C *)(halo.xch + xch_halo_offset(g.s3, e, 0));
-                    wait_flag(&hdr->flag_back, e, hdr);
-#pragma unroll
-                    for (int c = 0; c < 3; ++c)
-                        v1[7][c] = __ldcg(back + (size_t)c * g.s3 + (s.nbr[7] - (g.X3 - 1) * g.s3));
-                }
-            }
-        }
-
         C acc[N][3];
+        if constexpr (N == 1) {
+            hop_site<T, NR, HALO, true>(acc[0], in, links, g, cb, s, neg, halo.xch,
+                                  [&]() { return __ldcg(&((const XchHeader *)halo.xch)->epoch); });
+        } else {
+            // several right-hand sides: the neighbours of one group of directions at a time (register budget)
 #pragma unroll
-        for (int k = 0; k < N; ++k)
+            for (int k = 0; k < N; ++k)
 #pragma unroll
-            for (int i = 0; i < 3; ++i) acc[k][i] = mk<T>(0, 0);
-
+                for (int i = 0; i < 3; ++i) acc[k][i] = mk<T>(0, 0);
 #pragma unroll
-        for (int grp = 0; grp < NG; ++grp) {
-            P pk[KG];
+            for (int grp = 0; grp < NG; ++grp) {
+                P pk[KG];
 #pragma unroll
-            for (int i = 0; i < KG; ++i) pk[i] = ld_stream(L + (grp * KG + i) * TILE);
-            C vg[VGN][VGD][3];
-            if constexpr (N > 1 && !PAIRED) {
+                for (int i = 0; i < KG; ++i) pk[i] = ld_stream(L + (grp * KG + i) * TILE);
+                C vg[N][DPG][3];
+                if constexpr (!PAIRED) {
 #pragma unroll
-                for (int k = 0; k < N; ++k)
+                    for (int k = 0; k < N; ++k)
 #pragma unroll
-                    for (int dd = 0; dd < DPG; ++dd)
+                        for (int dd = 0; dd < DPG; ++dd)
 #pragma unroll
-                        for (int c = 0; c < 3; ++c)
-                            vg[k][dd][c] = ld_keep_nc(in + k * rs + (size_t)c * g.Vh_pad + s.nbr[grp * DPG + dd]);
-            }
-            if constexpr (PAIRED) {
-#pragma unroll
-                for (int j = 0; j < N / 2; ++j)
-#pragma unroll
-                    for (int dd = 0; dd < DPG; ++dd)
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) {
-                            const float4 v = ld_keep_nc((const float4 *)(in + 2 * j * rs) + (size_t)c * g.Vh_pad + s.nbr[grp * DPG + dd]);
-                            vg[2 * j][dd][c] = mk<T>(v.x, v.y);
-                            vg[2 * j + 1][dd][c] = mk<T>(v.z, v.w);
-                        }
-                if constexpr (N & 1) {
-#pragma unroll
-                    for (int dd = 0; dd < DPG; ++dd)
-#pragma unroll
-                        for (int c = 0; c < 3; ++c)
-                            vg[N - 1][dd][c] = ld_keep_nc(in + (N - 1) * rs + (size_t)c * g.Vh_pad + s.nbr[grp * DPG + dd]);
+                            for (int c = 0; c < 3; ++c)
+                                vg[k][dd][c] = ld_keep_nc(in + k * rs + (size_t)c * g.Vh_pad + s.nbr[grp * DPG + dd]);
                 }
-            }
+                if constexpr (PAIRED) {
 #pragma unroll
-            for (int dd = 0; dd < DPG; ++dd) {
-                const int d = grp * DPG + dd;
-                C m[9];
+                    for (int j = 0; j < N / 2; ++j)
 #pragma unroll
-                for (int k = 0; k < K; ++k) m[k] = pk_get(pk, dd * K + k);
-                if (NR == 2) rebuild_row2<T>(m, (neg >> d) & 1u);
-                if (NR == 1) rebuild_from8<T>(m, (neg >> d) & 1u);
+                        for (int dd = 0; dd < DPG; ++dd)
 #pragma unroll
-                for (int k = 0; k < N; ++k)
+                            for (int c = 0; c < 3; ++c) {
+                                const float4 v = ld_keep_nc((const float4 *)(in + 2 * j * rs) + (size_t)c * g.Vh_pad + s.nbr[grp * DPG + dd]);
+                                vg[2 * j][dd][c] = mk<T>(v.x, v.y);
+                                vg[2 * j + 1][dd][c] = mk<T>(v.z, v.w);
+                            }
+                    if constexpr (N & 1) {
 #pragma unroll
-                    for (int i = 0; i < 3; ++i)
+                        for (int dd = 0; dd < DPG; ++dd)
 #pragma unroll
-                        for (int j = 0; j < 3; ++j) {
-                            if constexpr (N == 1) cfma(acc[k][i], m[3 * i + j], v1[d][j]);
-                            else cfma(acc[k][i], m[3 * i + j], vg[k][dd][j]);
-                        }
+                            for (int c = 0; c < 3; ++c)
+                                vg[N - 1][dd][c] = ld_keep_nc(in + (N - 1) * rs + (size_t)c * g.Vh_pad + s.nbr[grp * DPG + dd]);
+                    }
+                }
+#pragma unroll
+                for (int dd = 0; dd < DPG; ++dd) {
+                    const int d = grp * DPG + dd;
+                    C m[9];
+#pragma unroll
+                    for (int k = 0; k < K; ++k) m[k] = pk_get(pk, dd * K + k);
+                    if (NR == 2) rebuild_row2<T>(m, (neg >> d) & 1u);
+                    if (NR == 1) rebuild_from8<T>(m, (neg >> d) & 1u);
+#pragma unroll
+                    for (int k = 0; k < N; ++k)
+#pragma unroll
+                        for (int i = 0; i < 3; ++i)
+#pragma unroll
+                            for (int j = 0; j < 3; ++j) cfma(acc[k][i], m[3 * i + j], vg[k][dd][j]);
+                }
             }
         }
 

@@ -115,6 +115,7 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
     if (prm) P = *prm;
     if (!(P.eps_in > 0.0)) P.eps_in = (mode == STAG_CG_DEFECT) ? 1e-2 : 0.1;
     if (P.graph_chunk == 0) P.graph_chunk = 32;
+    if (P.persist_chunk <= 0) P.persist_chunk = 1024;
 
     Solver S;
     S.L = L;
@@ -199,10 +200,25 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
     // Instantiated once per (handle, mode, link form, nrhs, chunk, mass[, x]) and kept with the
     // workspace: everything else the nodes bake in (vector addresses, control block) is a
     // function of the workspace's base address and those.
+    // Or, for one right-hand side, as one persistent kernel per chunk (stag_persist.cuh).
+    const bool persist = nrhs == 1 && persist_prec_ok(S.prec_lo) &&
+                         (P.persistent > 0 || (P.persistent == 0 && persist_by_volume(L->g, lo)));
+    IterArgs<float> pa32;
+    IterArgs<double> pa64;
+    if (persist) {
+        CU(cudaMemsetAsync((char *)w.ctrl + PERSIST_BAR_OFF, 0, 2 * sizeof(unsigned), s));
+        if (lo) {
+            persist_fill<float>(pa32.rk[0], L, w, S.prec_lo, S.m2, w.y32, w.r32, w.d32, w.q32, w.tmp32);
+            pa32.nlocal = 1; pa32.max_iters = P.persist_chunk;
+        } else {
+            persist_fill<double>(pa64.rk[0], L, w, S.prec_lo, S.m2, x, w.r64, w.d64, w.q64, w.tmp64);
+            pa64.nlocal = 1; pa64.max_iters = P.persist_chunk;
+        }
+    }
     const int chunk = P.graph_chunk;
     cudaGraphExec_t gexec = nullptr;
     unsigned long long graph_nodes = 0;
-    if (chunk > 0) {
+    if (chunk > 0 && !persist) {
         const void *xkey = (mode == STAG_CG_F64) ? (const void *)x : nullptr;
         GraphSlot *slot = nullptr, *victim = &ws->graphs[0];
         for (GraphSlot &gs : ws->graphs) {
@@ -245,7 +261,9 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
         if (state == CG_RUN) {
             if (verifying) ++n_restarts;
             verifying = false;
-            if (gexec) {
+            if (persist) {
+                if ((rc = lo ? persist_launch<float>(pa32, S.prec_lo, false, s) : persist_launch<double>(pa64, S.prec_lo, false, s))) return rc;
+            } else if (gexec) {
                 CU(cudaGraphLaunch(gexec, s));
                 count_launch(graph_nodes);
             } else {

@@ -270,6 +270,7 @@ struct stag_slab_cg {
     int stage;                       // 0: nothing done, 1: |b|^2 on its way, 2: in the loop, 3: done
     bool have_true, verifying;
     int n_restarts, applies_f64, final_state;
+    bool persist;                    // stag_slab_cg_run iterates in the persistent kernel (stag_persist.cuh)
     double bnorm2;
     int rc_final;
 };
@@ -387,6 +388,7 @@ extern "C" int stag_slab_cg_begin(stag_links_t *L, void *x_even, const void *b_e
     if (params) C->P = *params;
     if (!(C->P.eps_in > 0.0)) C->P.eps_in = 0.1;
     if (C->P.graph_chunk <= 0) C->P.graph_chunk = 32;    // iterations between host checks (plain launches)
+    if (C->P.persist_chunk <= 0) C->P.persist_chunk = 1024;
     C->x = (double *)x_even;
     C->b = (const double *)b_even;
     C->mass = mass;
@@ -425,9 +427,50 @@ extern "C" int stag_slab_cg_begin(stag_links_t *L, void *x_even, const void *b_e
     h->eps_in = C->P.eps_in;
     h->nrhs = 1;
     CU(cudaMemcpyAsync(C->w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, t_stream));
+    CU(cudaMemsetAsync((char *)C->w.ctrl + PERSIST_BAR_OFF, 0, 2 * sizeof(unsigned), t_stream));
+    C->persist = persist_prec_ok(C->prec_lo) &&
+                 (C->P.persistent > 0 || (C->P.persistent == 0 && persist_by_volume(L->g, C->lo)));
     CU(cudaEventRecord(L->own.ev0, t_stream));
     C->stage = 0;
     return STAG_OK;
+}
+
+// One ACT_ITER of the slabs given, all of them in ONE cooperative launch of the persistent kernel
+// (stag_persist.cuh): every slab is a rank group of the grid.  n = 1 is what a process of a
+// one-process-per-GPU run launches for itself; n = nranks with every slab on this device is the
+// single-GPU emulation of the multi-GPU run, the ranks concurrent by construction.
+namespace {
+template <typename T>
+int slab_iter_all_t(stag_links_t *const *slabs, int n, cudaStream_t s)
+{
+    IterArgs<T> A;
+    const stag_slab_cg *C0 = slabs[0]->cg;
+    for (int i = 0; i < n; ++i) {
+        stag_links *L = slabs[i];
+        stag_slab_cg *C = L->cg;
+        Workspace &w = C->w;
+        if (std::is_same<T, float>::value)
+            persist_fill<T>(A.rk[i], L, w, C->prec_lo, C->m2, (T *)w.y32, (T *)w.r32, (T *)w.d32, (T *)w.q32, (T *)w.tmp32);
+        else
+            persist_fill<T>(A.rk[i], L, w, C->prec_lo, C->m2, (T *)C->x, (T *)w.r64, (T *)w.d64, (T *)w.q64, (T *)w.tmp64);
+        ++L->epoch;
+    }
+    A.nlocal = n;
+    A.max_iters = C0->P.persist_chunk;
+    return persist_launch<T>(A, C0->prec_lo, true, s);
+}
+}  // namespace
+
+extern "C" int stag_slab_cg_iter_all(stag_links_t *const *slabs, int n)
+{
+    if (!slabs || n < 1 || n > MAX_RANKS) return STAG_EINVAL;
+    for (int i = 0; i < n; ++i) {
+        const stag_links *L = slabs[i];
+        if (!L || !L->is_slab || !L->cg || L->cg->stage != 2 || !persist_prec_ok(L->cg->prec_lo)) return STAG_EINVAL;
+        if (L->cg->prec_lo != slabs[0]->cg->prec_lo || L->cg->P.persist_chunk != slabs[0]->cg->P.persist_chunk) return STAG_EINVAL;
+        for (int j = 0; j < i; ++j) if (slabs[j] == L) return STAG_EINVAL;
+    }
+    return slabs[0]->cg->lo ? slab_iter_all_t<float>(slabs, n, t_stream) : slab_iter_all_t<double>(slabs, n, t_stream);
 }
 
 // Decide what every rank does next.  Synchronises the stream and reads the control block; all
@@ -605,6 +648,11 @@ extern "C" int stag_slab_cg_run(stag_links_t *L, void *x_even, const void *b_eve
             // the chunk of iterations as ONE graph launch: possible because the exchange and
             // reduction numbers live in device memory, not in the kernels' arguments
             stag_slab_cg *C = L->cg;
+            if (C->persist) {
+                stag_links_t *one[1] = { L };
+                if ((rc = stag_slab_cg_iter_all(one, 1))) return rc;
+                continue;
+            }
             if (!C->iter_graph) {
                 cudaGraph_t graph = nullptr;
                 cudaError_t e = cudaStreamBeginCapture(L->own.cap_stream, cudaStreamCaptureModeThreadLocal);

@@ -184,9 +184,10 @@ class SlabLinks:
         self.connect_all_pointers(ptrs)
 
     # -- CG over the slabs: control flow only, every decision is taken in the library --------
-    def cg_begin(self, x, b, mass, tol, maxiter, mode, eps_in=None, recon12=False, chunk=None, recon12_f64=False):
+    def cg_begin(self, x, b, mass, tol, maxiter, mode, eps_in=None, recon12=False, chunk=None, recon12_f64=False,
+                 persistent=None, persist_chunk=None):
         stag.use_current_stream()
-        p = stag._params(eps_in, recon12, chunk, recon12_f64)
+        p = stag._params(eps_in, recon12, chunk, recon12_f64, False, persistent, persist_chunk)
         stag._check(stag.lib().stag_slab_cg_begin(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(b.data_ptr()),
                                                   float(mass), float(tol), int(maxiter), int(mode), ctypes.byref(p)))
 
@@ -218,7 +219,8 @@ class SlabLinks:
         if after_phase is None:                 # the whole loop in the library: stag_slab_cg_run
             stag.use_current_stream()
             st = stag._Stats()
-            p = stag._params(kw.get("eps_in"), kw.get("recon12", False), kw.get("chunk"), kw.get("recon12_f64", False))
+            p = stag._params(kw.get("eps_in"), kw.get("recon12", False), kw.get("chunk"), kw.get("recon12_f64", False),
+                             False, kw.get("persistent"), kw.get("persist_chunk"))
             rc = stag.lib().stag_slab_cg_run(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(b.data_ptr()),
                                              float(mass), float(tol), int(maxiter), int(mode), ctypes.byref(p),
                                              ctypes.byref(st))
@@ -312,10 +314,15 @@ def connect_in_process(slabs):
         s.connect_all_pointers(ptrs)
 
 
-def cg_solve_in_process(slabs, bs, mass, tol, maxiter, mode=stag.CG_RELIABLE, **kw):
-    """The multi-GPU solve with all slabs in THIS process on one device: every phase is enqueued
-    for rank 0, 1, ... before the next phase, so a kernel that waits for its peers always finds
-    their kernels already launched.  bs[r]: rank r's fp64 device spinor.  Returns (xs, [stats])."""
+def cg_solve_in_process(slabs, bs, mass, tol, maxiter, mode=stag.CG_RELIABLE, fused=False, **kw):
+    """The multi-GPU solve with all slabs in THIS process on one device.  bs[r]: rank r's fp64 device
+    spinor.  Returns (xs, [stats]).
+    fused = False: every phase is enqueued for rank 0, 1, ... before the next phase, so a kernel
+    that waits for its peers always finds their kernels already finished (lockstep).
+    fused = True: the iterations of ALL ranks run in one cooperative launch of the persistent kernel
+    (stag_slab_cg_iter_all), each rank a group of blocks: the ranks execute concurrently and their
+    acquire-waits really spin on peers that are still running, as on separate GPUs.  The rare fp64
+    steps (initial residual, reliable updates, verification) stay stepped."""
     torch = stag._require_cuda()
     xs = [torch.zeros_like(b) for b in bs]
     for s, x, b in zip(slabs, xs, bs):
@@ -326,6 +333,11 @@ def cg_solve_in_process(slabs, bs, mass, tol, maxiter, mode=stag.CG_RELIABLE, **
             raise RuntimeError("ranks disagree on the next action: %r" % (acts,))
         if acts[0] == ACT_DONE:
             break
+        if fused and acts[0] == ACT_ITER:
+            stag.use_current_stream()
+            arr = (ctypes.c_void_p * len(slabs))(*[s.handle.value for s in slabs])
+            stag._check(stag.lib().stag_slab_cg_iter_all(arr, len(slabs)))
+            continue
         ph = 0
         while True:
             more = [s.cg_step(acts[0], ph) for s in slabs]

@@ -147,6 +147,44 @@ def test_slab_cg_run_from_one_thread_per_slab(dims, nranks, mass, mode):
         s.close()
 
 
+@pytest.mark.parametrize("dims,nranks,mass", [((4, 4, 4, 8), 2, 0.1), ((4, 4, 4, 16), 4, 0.1), ((8, 8, 8, 16), 2, 0.05),
+                                              ((8, 8, 8, 32), 8, 0.05), ((6, 2, 2, 12), 3, 0.1), ((4, 4, 4, 4), 1, 0.1)])
+@pytest.mark.parametrize("mode", [stag.CG_F64, stag.CG_RELIABLE])
+def test_all_ranks_in_one_cooperative_launch(dims, nranks, mass, mode):
+    """The sanctioned way to run ranks that wait on one another on ONE GPU (B200_PROFILING.md): all
+    ranks' iterations in one cooperative launch of the persistent kernel (stag_slab_cg_iter_all), each
+    rank a group of blocks with its own barrier.  Every block is resident, so the ranks run
+    concurrently by construction; they exchange faces through peer stores into each other's halo
+    buffers and sum their inner products through the exchange regions, waiting on flags, exactly
+    as one process per GPU does.  Same checks as test_gpu_slab_multi.py."""
+    tol = 1e-10
+    W = fieldgen.links(dims, "random", seed=77)
+    b = fieldgen.spinor_gaussian(dims, 0, seed=78)
+    x_ref, _, _, _, rc = oracle.cg(b, W, dims, mass, 1e-12, 50000)
+    assert rc == 0
+    slabs = make_slabs(dims, W, nranks)
+    bs = [stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(b, dims, r, nranks)), slabs[r].dims, 0)
+          for r in range(nranks)]
+    xs, sts = slab.cg_solve_in_process(slabs, bs, mass, tol, 20000, mode, fused=True, recon12=True, persist_chunk=50)
+    assert all(st["status"] == stag.OK and st["true_resid"] <= tol for st in sts), sts
+    for st in sts[1:]:
+        assert (st["iters"], st["true_resid"], st["n_updates"]) == (sts[0]["iters"], sts[0]["true_resid"], sts[0]["n_updates"])
+    x = slab.gather_spinor([stag.spinor_unpack(xs[r], slabs[r].dims, 0) for r in range(nranks)], dims)
+    assert rel_err(x, x_ref) <= 1e-8
+    resid = np.linalg.norm((b - oracle.apply_A(x, W, dims, mass)).ravel()) / np.linalg.norm(b.ravel())
+    assert resid <= tol * (1 + 1e-3)
+    assert all(s.status() == stag.OK for s in slabs)
+    # against the lockstep, kernel-per-step solve of the same slabs: same algorithm, other summation order
+    xs2, sts2 = slab.cg_solve_in_process(slabs, bs, mass, tol, 20000, mode, recon12=True)
+    assert abs(sts[0]["iters"] - sts2[0]["iters"]) <= max(3, 0.05 * sts2[0]["iters"])
+    # (the lockstep solve above adds no spinning wait: its counters are those of the fused run)
+    spun = [s.wait_stats()[0] for s in slabs]
+    print("waits that spun, per rank:", spun)
+    assert sum(spun) > 0, "no acquire-wait ever spun"
+    for s in slabs:
+        s.close()
+
+
 def test_a_dead_slab_takes_its_neighbours_down_and_reset_revives_them():
     """Rank 0 hops after an exchange rank 1 never joined: its watchdog fires.  From then on rank 0
     publishes nothing, so rank 1 -- whose first exchange still completes, rank 0's push preceded its
