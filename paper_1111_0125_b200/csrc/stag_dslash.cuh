@@ -168,6 +168,30 @@ __device__ __forceinline__ bool wait_flag(const unsigned long long *f, unsigned 
         __nanosleep(200);
     }
 }
+// One thread, after it has observed (at gpu scope: ticket or barrier) every block's stores into the
+// neighbours' halo buffers: make them visible at system scope, then set the neighbours' flags to e.
+// STAG_FLAG_FENCE selects how (measured on B200, profiles/README.md round 2): 0 = two release
+// stores, 1 = one fence.acq_rel.sys + two relaxed stores, 2 = __threadfence_system (fence.sc.sys).
+#ifndef STAG_FLAG_FENCE
+#define STAG_FLAG_FENCE 1
+#endif
+__device__ __forceinline__ void raise_halo_flags(char *peer_fwd, char *peer_bwd, unsigned long long e)
+{
+    unsigned long long *ff = &((XchHeader *)peer_fwd)->flag_back, *fb = &((XchHeader *)peer_bwd)->flag_fwd;
+#if STAG_FLAG_FENCE == 0
+    asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(ff), "l"(e) : "memory");
+    asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(fb), "l"(e) : "memory");
+#else
+#if STAG_FLAG_FENCE == 1
+    asm volatile("fence.acq_rel.sys;" ::: "memory");
+#else
+    __threadfence_system();
+#endif
+    asm volatile("st.relaxed.sys.global.u64 [%0], %1;" :: "l"(ff), "l"(e) : "memory");
+    asm volatile("st.relaxed.sys.global.u64 [%0], %1;" :: "l"(fb), "l"(e) : "memory");
+#endif
+}
+
 // A slab whose watchdog fired is dead until stag_slab_reset: every kernel of the slab path begins with
 // this test (uniform over the grid when the mark predates the launch) and leaves without storing to a
 // peer, bumping a count or setting a flag, so the neighbours' waits run into their own limit and every
@@ -186,7 +210,9 @@ __device__ __forceinline__ bool slab_dead(const char *xch)
 // end; their in-slice index addresses the buffers).  epoch() is only evaluated by boundary threads.
 // NC: the input spinor is read-only for the whole kernel (non-coherent loads, the plain kernels);
 // false inside the persistent kernel, where another phase of the same launch wrote it.
-template <typename T, int NR, bool HALO, bool NC = true, typename EpochFn>
+// LRES: the gauge field is small enough to stay in L2 next to the vectors (persistent kernel on
+// small lattices): its packets are then loaded with the keep policy instead of streamed through.
+template <typename T, int NR, bool HALO, bool NC = true, bool LRES = false, typename EpochFn>
 __device__ __forceinline__ void hop_site(cplx_t<T> (&acc)[3], const cplx_t<T> *__restrict__ in,
                                          const pkt_t<T> *__restrict__ links, const Geom &g, const int cb,
                                          const Site &s, const unsigned neg, char *xch, EpochFn epoch)
@@ -232,7 +258,10 @@ __device__ __forceinline__ void hop_site(cplx_t<T> (&acc)[3], const cplx_t<T> *_
     for (int grp = 0; grp < NG; ++grp) {
         P pk[KG];
 #pragma unroll
-        for (int i = 0; i < KG; ++i) pk[i] = ld_stream(L + (grp * KG + i) * TILE);
+        for (int i = 0; i < KG; ++i) {
+            if constexpr (LRES) pk[i] = ld_keep_nc(L + (grp * KG + i) * TILE);
+            else pk[i] = ld_stream(L + (grp * KG + i) * TILE);
+        }
 #pragma unroll
         for (int dd = 0; dd < DPG; ++dd) {
             const int d = grp * DPG + dd;
@@ -474,9 +503,7 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
             if (any && threadIdx.x == 0 && atomicAdd(&hdr->ticket, 1u) == halo.n_push_blocks - 1 && !slab_dead(halo.xch)) {
                 hdr->ticket = 0;
                 hdr->epoch = e_in + 1;
-                __threadfence_system();   // cumulativity: every block's peer stores precede the flags
-                asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)halo.peer_fwd)->flag_back), "l"(e_in + 1) : "memory");
-                asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)halo.peer_bwd)->flag_fwd), "l"(e_in + 1) : "memory");
+                raise_halo_flags(halo.peer_fwd, halo.peer_bwd, e_in + 1);   // cumulative: every block's peer stores precede the flags
             }
         }
     }

@@ -202,11 +202,10 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
     // function of the workspace's base address and those.
     // Or, for one right-hand side, as one persistent kernel per chunk (stag_persist.cuh).
     const bool persist = nrhs == 1 && persist_prec_ok(S.prec_lo) &&
-                         (P.persistent > 0 || (P.persistent == 0 && persist_by_volume(L->g, lo)));
+                         (P.persistent > 0 || (P.persistent == 0 && persist_by_volume(L->g, false)));
     IterArgs<float> pa32;
     IterArgs<double> pa64;
     if (persist) {
-        CU(cudaMemsetAsync((char *)w.ctrl + PERSIST_BAR_OFF, 0, 2 * sizeof(unsigned), s));
         if (lo) {
             persist_fill<float>(pa32.rk[0], L, w, S.prec_lo, S.m2, w.y32, w.r32, w.d32, w.q32, w.tmp32);
             pa32.nlocal = 1; pa32.max_iters = P.persist_chunk;

@@ -8,9 +8,13 @@ namespace {
 
 // offset of the rank group's barrier words inside the workspace's control slot (behind CgCtrl)
 constexpr size_t PERSIST_BAR_OFF = 1792;
-static_assert(sizeof(CgCtrl) <= PERSIST_BAR_OFF && PERSIST_BAR_OFF + 2 * sizeof(unsigned) <= CTRL_SLOT, "barrier words must fit the control slot");
+static_assert(sizeof(CgCtrl) <= PERSIST_BAR_OFF && PERSIST_BAR_OFF + sizeof(unsigned) <= CTRL_SLOT, "barrier words must fit the control slot");
 
-constexpr int PERSIST_AUTO_MAX_VH = 0;     // set from the measurements (profiles/README.md)
+// persistent = 0 picks the persistent kernel for whole lattices of at most this many sites per parity
+// (28^3 x 24 = 263 424: 47.8 us per pass against 50.4 on the kernel-per-step path; at 28^3 x 48 the
+// two are level and beyond it the stand-alone hops win, profiles/README.md round 2), and always for
+// T-slabs, whose kernel-per-step pass has six launches.
+constexpr int PERSIST_AUTO_MAX_VH = 300000;
 
 inline bool persist_prec_ok(int prec)     // the 8-parameter forms stay on the kernel-per-step path
 {
@@ -19,7 +23,7 @@ inline bool persist_prec_ok(int prec)     // the 8-parameter forms stay on the k
 
 // Blocks of the persistent kernel that can be resident at once on this device (the cooperative
 // launch refuses more).  One query per instantiation.
-template <typename T, int NR, bool SLAB>
+template <typename T, int NR, bool SLAB, bool LRES>
 int persist_capacity()
 {
     static std::atomic<int> cap{0};
@@ -28,7 +32,7 @@ int persist_capacity()
         int dev = 0, sms = 0, per = 0;
         if (cudaGetDevice(&dev) != cudaSuccess ||
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, cg_iter_persistent_kernel<T, NR, SLAB>, PERSIST_THREADS, 0) != cudaSuccess)
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, cg_iter_persistent_kernel<T, NR, SLAB, LRES>, PERSIST_THREADS, 0) != cudaSuccess)
             return -1;
         c = sms * per;
         cap.store(c, std::memory_order_relaxed);
@@ -37,12 +41,28 @@ int persist_capacity()
 }
 
 // persistent = 0: which lattices iterate in the persistent kernel.  The kernel boundaries it removes
-// cost a fixed ~12 us per pass; its own hop is a few per cent slower than the stand-alone kernel
-// on lattices that stream from HBM, so it pays for small volumes only.
-inline bool persist_by_volume(const Geom &g, bool lo)
+// cost a fixed ~5 us per pass; its hops end with 4-8 us of stragglers at the barrier on lattices
+// that stream from HBM, so on one GPU it pays for small volumes only.
+inline bool persist_by_volume(const Geom &g, bool is_slab)
 {
-    (void)lo;
-    return g.Vh <= PERSIST_AUTO_MAX_VH;
+    return is_slab || g.Vh <= PERSIST_AUTO_MAX_VH;
+}
+
+// Bytes of links + vectors up to which the persistent kernel keeps the links in L2: 5/8 of the
+// device's L2 (126 MB on B200), which leaves room for the two dies' duplicates and the fp64 vectors.
+inline size_t persist_l2_budget()
+{
+    static std::atomic<size_t> budget{0};
+    size_t b = budget.load(std::memory_order_relaxed);
+    if (b == 0) {
+        int dev = 0, l2 = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev) != cudaSuccess) l2 = 0;
+        if (const char *e = getenv("STAG_PERSIST_L2_BUDGET_MB")) b = (size_t)atol(e) << 20;     // measurement knob
+        else b = (size_t)l2 / 8 * 5;
+        if (b == 0) b = 1;
+        budget.store(b, std::memory_order_relaxed);
+    }
+    return b;
 }
 
 // Blocks a rank group of this volume can use: one site per thread per trip at most.
@@ -69,10 +89,10 @@ void persist_fill(IterRank<T> &R, const stag_links *L, const Workspace &w, int p
     R.nranks = L->nranks; R.myrank = L->rank;
 }
 
-template <typename T, int NR, bool SLAB>
+template <typename T, int NR, bool SLAB, bool LRES>
 int persist_launch_t(IterArgs<T> &A, cudaStream_t s)
 {
-    const int cap = persist_capacity<T, NR, SLAB>();
+    const int cap = persist_capacity<T, NR, SLAB, LRES>();
     if (cap < A.nlocal) return STAG_ECUDA;
     // split the resident blocks evenly among the rank groups, no group larger than its volume needs
     const int share = cap / A.nlocal;
@@ -85,10 +105,23 @@ int persist_launch_t(IterArgs<T> &A, cudaStream_t s)
         A.rk[i].nblocks = nb;
         grid += nb;
     }
+    for (int i = 0; i < A.nlocal; ++i) CU(cudaMemsetAsync(A.rk[i].bar, 0, sizeof(unsigned), s));
     void *args[] = { (void *)&A };
-    CU(cudaLaunchCooperativeKernel((const void *)cg_iter_persistent_kernel<T, NR, SLAB>, dim3((unsigned)grid),
+    CU(cudaLaunchCooperativeKernel((const void *)cg_iter_persistent_kernel<T, NR, SLAB, LRES>, dim3((unsigned)grid),
                                    dim3(PERSIST_THREADS), args, 0, s));
     count_launch();
+#ifdef STAG_PERSIST_TIMING
+    {
+        unsigned long long h[16];
+        cudaStreamSynchronize(s);
+        if (cudaMemcpyFromSymbol(h, g_persist_stamps, sizeof(h)) == cudaSuccess) {
+            static const char *what[10] = { "P0 xpay", "barrier", "P1 hop", "barrier", "P2 hop+dot", "barrier", "sum <d,Ad>", "P3 update", "barrier", "sum |r|^2" };
+            fprintf(stderr, "[persist pass 20, ns]");
+            for (int k = 0; k < 10; ++k) fprintf(stderr, " %s %llu |", what[k], h[k + 1] - h[k]);
+            fprintf(stderr, " total %llu\n", h[10] - h[0]);
+        }
+    }
+#endif
     return STAG_OK;
 }
 
@@ -96,8 +129,19 @@ template <typename T>
 int persist_launch(IterArgs<T> &A, int prec, bool slab, cudaStream_t s)
 {
     const int rows = prec_rows(prec);
-    if (rows == 3) return slab ? persist_launch_t<T, 3, true>(A, s) : persist_launch_t<T, 3, false>(A, s);
-    if (rows == 2) return slab ? persist_launch_t<T, 2, true>(A, s) : persist_launch_t<T, 2, false>(A, s);
+    // do the links of both parities and the five vectors of every rank group fit L2 together?
+    size_t bytes = 0;
+    for (int i = 0; i < A.nlocal; ++i)
+        bytes += (size_t)A.rk[i].g.Vh_pad * (2 * 8 * link_slots(rows) * 2 + 5 * 6) * sizeof(T);
+    const bool lres = bytes <= persist_l2_budget();
+    if (rows == 3) {
+        if (lres) return slab ? persist_launch_t<T, 3, true, true>(A, s) : persist_launch_t<T, 3, false, true>(A, s);
+        return slab ? persist_launch_t<T, 3, true, false>(A, s) : persist_launch_t<T, 3, false, false>(A, s);
+    }
+    if (rows == 2) {
+        if (lres) return slab ? persist_launch_t<T, 2, true, true>(A, s) : persist_launch_t<T, 2, false, true>(A, s);
+        return slab ? persist_launch_t<T, 2, true, false>(A, s) : persist_launch_t<T, 2, false, false>(A, s);
+    }
     return STAG_EINVAL;
 }
 

@@ -427,9 +427,8 @@ extern "C" int stag_slab_cg_begin(stag_links_t *L, void *x_even, const void *b_e
     h->eps_in = C->P.eps_in;
     h->nrhs = 1;
     CU(cudaMemcpyAsync(C->w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, t_stream));
-    CU(cudaMemsetAsync((char *)C->w.ctrl + PERSIST_BAR_OFF, 0, 2 * sizeof(unsigned), t_stream));
     C->persist = persist_prec_ok(C->prec_lo) &&
-                 (C->P.persistent > 0 || (C->P.persistent == 0 && persist_by_volume(L->g, C->lo)));
+                 (C->P.persistent > 0 || (C->P.persistent == 0 && persist_by_volume(L->g, true)));
     CU(cudaEventRecord(L->own.ev0, t_stream));
     C->stage = 0;
     return STAG_OK;

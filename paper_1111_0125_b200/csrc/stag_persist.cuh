@@ -38,10 +38,29 @@
 
 namespace stag {
 
-constexpr int PERSIST_THREADS = 256;
+#ifndef STAG_PERSIST_THREADS
+#define STAG_PERSIST_THREADS 256
+#endif
+constexpr int PERSIST_THREADS = STAG_PERSIST_THREADS;
+
+// -DSTAG_PERSIST_TIMING: block 0 of rank group 0 stamps %globaltimer after every phase and barrier of
+// pass 20; the host prints the differences after the launch (profiles/README.md, round 2).  Off in
+// the product build.
+#ifdef STAG_PERSIST_TIMING
+__device__ unsigned long long g_persist_stamps[16];
+__device__ __forceinline__ unsigned long long persist_now()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define PSTAMP(k) do { if (blockIdx.x == 0 && threadIdx.x == 0 && pass == 20) g_persist_stamps[k] = persist_now(); } while (0)
+#else
+#define PSTAMP(k) do { } while (0)
+#endif
 
 // How many blocks per SM the launch bounds promise ptxas (registers per thread = 65536 / (256 * BPS)).
-template <typename T, int NR> struct PersistTune { static constexpr int BPS = 2; };
+template <typename T, int NR> struct PersistTune { static constexpr int BPS = 512 / PERSIST_THREADS; };
 
 template <typename T> struct IterRank {
     T *y, *r, *d, *q, *tmp;                  // flat spinors, 6*Vh_pad reals; y = x itself in mode 0
@@ -49,7 +68,7 @@ template <typename T> struct IterRank {
     Geom g;
     CgCtrl *ctrl;
     double *partials;                        // 2 * nblocks doubles
-    unsigned *bar;                           // [0] arrivals, [1] generation; [0] must be 0 at launch
+    unsigned *bar;                           // arrival counter of the group's barrier; 0 at launch (the host zeroes it)
     T m2;
     int block0, nblocks;                     // this rank's slice of the grid
     // T-slab only (xch == null: a whole lattice, periodic wrap inside decode_site)
@@ -68,31 +87,28 @@ struct IterScalars {
     int state, iter, maxiter, mode, iters, active;
 };
 
-// Barrier among the nb blocks of one rank group.  hdr != null (slab): the spin is bounded by the
-// slab's watchdog like every other wait, a timeout marks the slab dead and returns false.
-__device__ __forceinline__ bool group_barrier(unsigned *bar, unsigned nb, XchHeader *hdr)
+// Barrier among the nb blocks of one rank group: a monotonic arrival counter, zeroed by the host
+// before the launch.  Barrier number k (k = 1, 2, ...) is passed once the counter shows k*nb: one
+// fire-and-forget release-add per block, then acquire-polls -- no returning atomic, no reset, no
+// generation word, so the critical path is one L2 write plus one L2 read after the last arrival.
+// hdr != null (slab): the spin is bounded by the slab's watchdog like every other wait; a timeout
+// marks the slab dead and returns false.
+__device__ __forceinline__ bool group_barrier(unsigned *bar, unsigned target, XchHeader *hdr)
 {
     __shared__ bool ok;
     __syncthreads();
     if (threadIdx.x == 0) {
         ok = true;
-        unsigned gen;
-        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(gen) : "l"(bar + 1) : "memory");
-        __threadfence();                                  // the block's writes, cumulatively, before its arrival
-        if (atomicAdd(bar, 1u) == nb - 1) {
-            *(volatile unsigned *)bar = 0u;
-            asm volatile("st.release.gpu.global.u32 [%0], %1;" :: "l"(bar + 1), "r"(gen + 1u) : "memory");
-        } else {
-            unsigned v;
-            unsigned long long polls = 0, limit = 0;
-            if (hdr) { limit = __ldcg(&hdr->wait_limit); if (limit == 0) limit = XCH_DEFAULT_WAIT_POLLS; limit *= 8; }
-            for (;;) {
-                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar + 1) : "memory");
-                if (v != gen) break;
-                if (hdr && ++polls >= limit) { *(volatile unsigned *)&hdr->timed_out = 1u; ok = false; break; }
-            }
+        // release at gpu scope: cumulative over the block's writes (ordered before it by the block barrier)
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" :: "l"(bar) : "memory");
+        unsigned v;
+        unsigned long long polls = 0, limit = 0;
+        if (hdr) { limit = __ldcg(&hdr->wait_limit); if (limit == 0) limit = XCH_DEFAULT_WAIT_POLLS; limit *= 8; }
+        for (;;) {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+            if (v >= target) break;
+            if (hdr && ++polls >= limit) { *(volatile unsigned *)&hdr->timed_out = 1u; ok = false; break; }
         }
-        __threadfence();                                  // acquire side: L1 lines of the previous phase are dropped
     }
     __syncthreads();
     return ok;
@@ -129,7 +145,13 @@ __device__ __forceinline__ void iter_epilogue_local(IterScalars &S, const double
     S.state = st;
 }
 
-template <typename T, int NR, bool SLAB>
+// Tiles are dealt to the group's warps statically (warp w takes tiles w, w + W, ...).  A dynamic deal
+// from one atomic counter was tried to trim the 4-8 us of stragglers at the barrier after each hop on
+// 28^3 x 96 (14 trips for some warps, 13 for others; SMs of unequal speed): 33 k same-address atomics
+// per phase serialise in L2 and the hop went from 62 to 96 us (profiles/README.md, round 2).
+// LRES: the links of both parities and the five vectors fit L2 together (the host decides): the link
+// packets are then loaded with the keep policy and every pass after the first reads them from L2.
+template <typename T, int NR, bool SLAB, bool LRES>
 __global__ void __launch_bounds__(PERSIST_THREADS, PersistTune<T, NR>::BPS)
 cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
 {
@@ -152,6 +174,7 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
     __shared__ double s_sum;
     __shared__ bool s_ok;
     unsigned long long epoch = 0, seq = 0;
+    unsigned bar_target = 0;                        // arrivals that complete the next barrier
     if constexpr (SLAB) { epoch = __ldcg(&hdr->epoch); seq = __ldcg(&hdr->red_seq); }
     if (threadIdx.x == 0) {
         const CgCtrl *c = R.ctrl;
@@ -177,9 +200,7 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
     // release the neighbours' flags for the exchange whose stores the last barrier ordered (block 0, one thread)
     auto raise_flags = [&](unsigned long long e) {
         if (lb == 0 && threadIdx.x == 0) {
-            __threadfence_system();               // cumulative over every block's peer stores (they precede the barrier)
-            asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)R.peer_fwd)->flag_back), "l"(e) : "memory");
-            asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)R.peer_bwd)->flag_fwd), "l"(e) : "memory");
+            raise_halo_flags(R.peer_fwd, R.peer_bwd, e);   // cumulative over every block's peer stores (they precede the barrier)
         }
     };
     // local fixed-order total of this group's partials -> (slab) sum over ranks, the same bits everywhere
@@ -187,11 +208,11 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
         double t = block_total_fixed(part, nb, red);
         if constexpr (SLAB) {
             ++seq;
-            if (threadIdx.x == 0) {
+            if (threadIdx.x < 32) {               // warp 0: lane r talks to rank r
                 if (lb == 0) publish_total(R.peers, R.nranks, R.myrank, seq, t);
                 bool ok;
-                s_sum = gather_total(R.xch, R.nranks, seq, &ok);
-                s_ok = ok;
+                const double tot = gather_total(R.xch, R.nranks, seq, &ok);
+                if (threadIdx.x == 0) { s_sum = tot; s_ok = ok; }
             }
             __syncthreads();
             if (!s_ok) return false;
@@ -204,6 +225,7 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
 
     for (int pass = 0; pass < A.max_iters && S.state == CG_RUN; ++pass) {
         // ---- P0: d = r + beta d (eq. 3.1 after an update) ------------------------------
+        PSTAMP(0);
         {
             const T beta = (T)S.beta;
             V *fwd_back = nullptr, *bwd_fwd = nullptr;
@@ -233,8 +255,10 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
                 }
             }
         }
-        if (!group_barrier(R.bar, nb, hdr)) return;
+        PSTAMP(1);
+        if (!group_barrier(R.bar, bar_target += (unsigned)nb, hdr)) return;
         if constexpr (SLAB) { if (slab_dead(R.xch)) return; ++epoch; raise_flags(epoch); }
+        PSTAMP(2);
 
         // ---- P1: tmp = D_oe d (eq. 2.5 on the odd sites) ------------------------------------
         for (int t = warp_g; t < ntiles; t += nwarps) {
@@ -245,7 +269,7 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
             unsigned neg = 0;
             if (NR != 3) neg = det_sign_mask(g, s);
             C acc[3];
-            hop_site<T, NR, SLAB, false>(acc, d_c, R.links_odd, g, cb, s, neg, R.xch, [=]() { return epoch; });
+            hop_site<T, NR, SLAB, false, LRES>(acc, d_c, R.links_odd, g, cb, s, neg, R.xch, [=]() { return epoch; });
 #pragma unroll
             for (int c = 0; c < 3; ++c) st_keep(tmp_c + (size_t)c * g.Vh_pad + cb, acc[c]);
             if constexpr (SLAB) {
@@ -258,8 +282,10 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
                 }
             }
         }
-        if (!group_barrier(R.bar, nb, hdr)) return;
+        PSTAMP(3);
+        if (!group_barrier(R.bar, bar_target += (unsigned)nb, hdr)) return;
         if constexpr (SLAB) { if (slab_dead(R.xch)) return; ++epoch; raise_flags(epoch); }
+        PSTAMP(4);
 
         // ---- P2: q = m^2 d - D_eo tmp (eq. 2.3), <d,q> in fp64 -------------------------
         double dot = 0.0;
@@ -271,7 +297,7 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
             unsigned neg = 0;
             if (NR != 3) neg = det_sign_mask(g, s);
             C acc[3];
-            hop_site<T, NR, SLAB, false>(acc, tmp_c, R.links_even, g, cb, s, neg, R.xch, [=]() { return epoch; });
+            hop_site<T, NR, SLAB, false, LRES>(acc, tmp_c, R.links_even, g, cb, s, neg, R.xch, [=]() { return epoch; });
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const C o = ld_keep(d_c + (size_t)c * g.Vh_pad + cb);
@@ -286,10 +312,13 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
             const double bs = block_sum(dot, red);
             if (threadIdx.x == 0) partA[lb] = bs;
         }
-        if (!group_barrier(R.bar, nb, hdr)) return;
+        PSTAMP(5);
+        if (!group_barrier(R.bar, bar_target += (unsigned)nb, hdr)) return;
         if constexpr (SLAB) { if (slab_dead(R.xch)) return; }
+        PSTAMP(6);
         double dAd;
         if (!total_over_ranks(partA, &dAd)) return;
+        PSTAMP(7);
 
         // ---- P3: alpha = delta / <d,Ad>; y += alpha d; r -= alpha q; |r|^2 ----
         const double alpha_d = (dAd > 0.0) ? S.delta / dAd : 0.0;
@@ -319,10 +348,13 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
             const double bs = block_sum(s2, red);
             if (threadIdx.x == 0) partB[lb] = bs;
         }
-        if (!group_barrier(R.bar, nb, hdr)) return;
+        PSTAMP(8);
+        if (!group_barrier(R.bar, bar_target += (unsigned)nb, hdr)) return;
         if constexpr (SLAB) { if (slab_dead(R.xch)) return; }
+        PSTAMP(9);
         double dn;
         if (!total_over_ranks(partB, &dn)) return;
+        PSTAMP(10);
         if (threadIdx.x == 0) {
             S.dAd = dAd;
             S.alpha = alpha_d;

@@ -70,9 +70,7 @@ face_push_kernel(const cplx_t<T> *__restrict__ in, const int Vh, const int Vh_pa
     if (threadIdx.x == 0 && atomicAdd(&hdr->ticket, 1u) == gridDim.x - 1) {
         hdr->ticket = 0;
         hdr->epoch = epoch;
-        __threadfence_system();   // cumulativity: every block's stores precede the flags
-        asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)peer_fwd)->flag_back), "l"(epoch) : "memory");
-        asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)peer_bwd)->flag_fwd), "l"(epoch) : "memory");
+        raise_halo_flags(peer_fwd, peer_bwd, epoch);   // cumulative: every block's stores precede the flags
     }
 }
 
@@ -128,37 +126,45 @@ slab_xpay_push_kernel(T *__restrict__ d, const T *__restrict__ r, long n, const 
     if (threadIdx.x == 0 && atomicAdd(&hdr->ticket, 1u) == gridDim.x - 1) {
         hdr->ticket = 0;
         hdr->epoch = epoch;
-        __threadfence_system();
-        asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)peer_fwd)->flag_back), "l"(epoch) : "memory");
-        asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&((XchHeader *)peer_bwd)->flag_fwd), "l"(epoch) : "memory");
+        raise_halo_flags(peer_fwd, peer_bwd, epoch);
     }
 }
 
 // ---- global sums of the slab CG ---------------------------------------------------------
-// One thread: store my local total of reduction seq into every rank's slots, then the flags.
+// Both are called by ALL 32 LANES OF ONE WARP; lane r talks to rank r, so the system-scope round
+// trips to the nranks regions overlap instead of queueing behind one another.
+// Publish: lane r stores my local total of reduction seq into rank r's slot and release-stores
+// seq into my flag there (the release orders the lane's own slot store before it).
+static_assert(MAX_RANKS <= 32, "one lane per rank");
 __device__ __forceinline__ void publish_total(char *const *peers, int nranks, int myrank,
                                               unsigned long long seq, double value)
 {
-    // the release store of the flag orders this thread's slot store before it: no separate fence
-    for (int r = 0; r < nranks; ++r) {
+    const int r = threadIdx.x & 31;
+    if (r < nranks) {
         XchReduce *R = (XchReduce *)(peers[r] + XCH_RED);
         *(volatile double *)&R->slot[seq & 1ull][myrank] = value;
         asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(&R->flag[myrank]), "l"(seq) : "memory");
     }
 }
 
-// Any thread: the sum over ranks of reduction seq, added in rank order (same bits on every rank).
-// *ok = false when a wait gave up (the slab is then marked dead; the sum is not to be used).
+// The sum over ranks of reduction seq, added in rank order (same bits on every rank), returned
+// to every lane.  *ok = false when a wait gave up (the slab is then marked dead; the sum is not to
+// be used).  Lane r acquire-waits for rank r's flag and reads rank r's slot.
 __device__ __forceinline__ double gather_total(char *mine, int nranks, unsigned long long seq, bool *ok)
 {
     const XchReduce *R = (const XchReduce *)(mine + XCH_RED);
-    double t = 0.0;
-    *ok = true;
-    for (int r = 0; r < nranks; ++r) {
-        if (!wait_flag(&R->flag[r], seq, (XchHeader *)mine)) { *ok = false; return 0.0; }
-        t += __ldcg(&R->slot[seq & 1ull][r]);
+    const int r = threadIdx.x & 31;
+    bool good = true;
+    double mine_v = 0.0;
+    if (r < nranks) {
+        good = wait_flag(&R->flag[r], seq, (XchHeader *)mine);
+        mine_v = __ldcg(&R->slot[seq & 1ull][r]);
     }
-    return t;
+    good = __all_sync(0xffffffffu, good);
+    double t = 0.0;
+    for (int k = 0; k < nranks; ++k) t += __shfl_sync(0xffffffffu, mine_v, k);     // rank order
+    *ok = good;
+    return good ? t : 0.0;
 }
 
 // Comm: what a kernel of the slab CG needs to publish / gather (passed by value).  The number of
@@ -171,15 +177,16 @@ struct Comm {
     int nranks, myrank;
 };
 
-// one thread
+// one warp (all 32 lanes)
 __device__ __forceinline__ void publish_next(const Comm &c, double value)
 {
     XchHeader *hdr = (XchHeader *)c.mine;
     const unsigned long long seq = __ldcg(&hdr->red_seq) + 1;
+    __syncwarp();
     publish_total(c.peers, c.nranks, c.myrank, seq, value);
-    hdr->red_seq = seq;
+    if ((threadIdx.x & 31) == 0) hdr->red_seq = seq;
 }
-// any thread of a kernel launched after the publishing one
+// one warp (all 32 lanes) of a kernel launched after the publishing one
 __device__ __forceinline__ double gather_current(const Comm &c, bool *ok)
 {
     return gather_total(c.mine, c.nranks, __ldcg(&((const XchHeader *)c.mine)->red_seq), ok);
@@ -193,7 +200,7 @@ slab_publish_partials_kernel(const double *__restrict__ partials, int n, const C
     if (ctrl->state != CG_RUN || slab_dead(c.mine)) return;
     __shared__ double red[32];
     const double t = block_total_fixed(partials, n, red);
-    if (threadIdx.x == 0) publish_next(c, t);
+    if (threadIdx.x < 32) publish_next(c, t);
 }
 
 // update_kernel for one right-hand side of a slab: <d,Ad> is the all-rank sum of reduction
@@ -211,7 +218,11 @@ slab_update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d
     __shared__ double totals[MAX_RHS];
     __shared__ double s_dAd;
     __shared__ bool s_ok;
-    if (threadIdx.x == 0) s_dAd = gather_current(c, &s_ok);     // every block reads red_seq before the last one bumps it
+    if (threadIdx.x < 32) {                                     // every block reads red_seq before the last one bumps it
+        bool ok;
+        const double t = gather_current(c, &ok);
+        if (threadIdx.x == 0) { s_dAd = t; s_ok = ok; }
+    }
     __syncthreads();
     if (!s_ok) return;            // a peer never published <d,Ad>: leave y, r alone and publish nothing
     const double dAd = s_dAd;
@@ -242,7 +253,7 @@ slab_update_kernel(T *__restrict__ y, T *__restrict__ r, const T *__restrict__ d
     }
     const double bs = block_sum(s, red);
     if (!finish_reduction(bs, partials, &ctrl->ticket[1], red, totals)) return;
-    if (threadIdx.x == 0) publish_next(c, totals[0]);
+    if (threadIdx.x < 32) publish_next(c, totals[0]);
 }
 
 // residual_kernel for one right-hand side of a slab: publishes the local |r|^2 (or |b|^2).
@@ -270,7 +281,7 @@ slab_residual_kernel(double *__restrict__ r, const double *__restrict__ b,
     __shared__ double totals[MAX_RHS];
     const double bs = block_sum(s, red);
     if (!finish_reduction(bs, partials, &ctrl->ticket[2], red, totals)) return;
-    if (threadIdx.x == 0) publish_next(c, totals[0]);
+    if (threadIdx.x < 32) publish_next(c, totals[0]);
 }
 
 // The scalar step that follows a published reduction: gather the all-rank sum and run the same
@@ -279,12 +290,12 @@ enum { SCALAR_ITER = 100 };
 template <int WHAT>
 __global__ void slab_scalar_kernel(CgCtrl *__restrict__ ctrl, const Comm c)
 {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    if (threadIdx.x >= 32 || blockIdx.x != 0) return;            // one warp
     if (WHAT == SCALAR_ITER && ctrl->state != CG_RUN) return;
     if (slab_dead(c.mine)) return;
     bool ok;
     double total = gather_current(c, &ok);
-    if (!ok) return;              // the scalars stay as they were; the host reads STAG_ETIMEOUT from the header
+    if (!ok || threadIdx.x != 0) return;   // on a timeout the scalars stay as they were; the host reads STAG_ETIMEOUT
     if (WHAT == SCALAR_ITER) cg_iteration_epilogue(ctrl, &total);
     else residual_epilogue<WHAT>(ctrl, &total);
 }

@@ -150,9 +150,10 @@ def test_graph_and_plain_launch_paths_agree_bitwise():
     L = stag.Links(cfg.dims, W)
     bd = stag.spinor_pack(b, cfg.dims, 0)
     for mode in (stag.CG_F64, stag.CG_RELIABLE):
-        xa, sa = stag.cg_solve(bd, L, cfg.mass, cfg.tol, cfg.maxiter, mode, graph_chunk=16)
-        xb, sb = stag.cg_solve(bd, L, cfg.mass, cfg.tol, cfg.maxiter, mode, graph_chunk=-1)
-        xc, sc = stag.cg_solve(bd, L, cfg.mass, cfg.tol, cfg.maxiter, mode, graph_chunk=16)
+        # persistent=False: the kernel-per-step path (a lattice this small would otherwise iterate in the persistent kernel)
+        xa, sa = stag.cg_solve(bd, L, cfg.mass, cfg.tol, cfg.maxiter, mode, graph_chunk=16, persistent=False)
+        xb, sb = stag.cg_solve(bd, L, cfg.mass, cfg.tol, cfg.maxiter, mode, graph_chunk=-1, persistent=False)
+        xc, sc = stag.cg_solve(bd, L, cfg.mass, cfg.tol, cfg.maxiter, mode, graph_chunk=16, persistent=False)
         assert sa["iters"] == sb["iters"] == sc["iters"]
         assert torch.equal(xa, xb) and torch.equal(xa, xc)      # fixed-order reductions
 

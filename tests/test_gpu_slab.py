@@ -187,14 +187,15 @@ def test_slab_cg_matches_oracle(nranks, mode):
 
 def test_slab_cg_one_rank_equals_whole_lattice_solver_bitwise():
     """nranks = 1: the global sums have one term, so the slab path must reproduce the one-GPU
-    solver's iterates exactly (same kernels' arithmetic, same reduction order)."""
+    solver's iterates exactly (same kernels' arithmetic, same reduction order) -- kernel-per-step
+    paths on both sides; the persistent kernels sum in another order (tests/test_gpu_persistent.py)."""
     import torch
     cfg = fieldgen.CONFIGS["c1_4^4"]
     W, b = cfg.links(), cfg.source()
     L = stag.Links(cfg.dims, W)
     bd = stag.spinor_pack(b, cfg.dims, 0)
     for mode in (stag.CG_F64, stag.CG_RELIABLE):
-        x1, st1 = stag.cg_solve(bd, L, cfg.mass, cfg.tol, cfg.maxiter, mode)
+        x1, st1 = stag.cg_solve(bd, L, cfg.mass, cfg.tol, cfg.maxiter, mode, persistent=False)
         S = make_slabs(cfg.dims, W, 1)
         xs, sts = slab.cg_solve_in_process(S, [bd], cfg.mass, cfg.tol, cfg.maxiter, mode)
         assert sts[0]["iters"] == st1["iters"] and sts[0]["n_updates"] == st1["n_updates"]
