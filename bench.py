@@ -2,7 +2,7 @@
 """bench.py -- the headline measurement of the staggered mixed-precision CG hot path.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config NAME]
-                    [--only all|hops] [--cpu-full] [--no-cpu-baseline] [--decomp replicas|slabs]
+                    [--only all|hops|mrhs|solve] [--persistent auto|on|off] [--cpu-full] [--no-cpu-baseline] [--decomp replicas|slabs]
 
 One STEP = one full mixed-precision CG solve (mode 3: fp32 iteration on 12-real compressed
 links -- the paper's single-precision kernel also reads compressed links, P:L113 -- with the
@@ -408,6 +408,18 @@ def run_ours(args):
         replicas.finalize()
         return 0
 
+    if args.only == "solve":                     # the timed solve alone: what the in-place ncu captures run
+        if rank == 0:
+            b_dev = stag.spinor_pack(b_np, cfg.dims, stag.PREC_F64)
+            kw = {} if args.persistent == "auto" else {"persistent": args.persistent == "on"}
+            for _ in range(max(1, args.steps)):
+                _, st = stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, args.maxiter or cfg.maxiter, stag.CG_RELIABLE, recon12=True, **kw)
+            print(json.dumps({"only": "solve", "config": {"workload": cfg.name}, "persistent": args.persistent,
+                              "iters": st["iters"], "time_to_solution_s": st["seconds"],
+                              "us_per_iteration": st["seconds"] / max(1, st["iters"]) * 1e6}), flush=True)
+        replicas.finalize()
+        return 0
+
     b_dev = stag.spinor_pack(b_np, cfg.dims, stag.PREC_F64)
     b_host = torch.from_numpy(b_np.view(np.float64).reshape(-1).copy()).pin_memory()
     x_host = torch.zeros_like(b_host).pin_memory()
@@ -465,6 +477,10 @@ def run_ours(args):
         stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, mode, **kw)      # warm: graph instantiated, links derived
         return stag.cg_solve(b_dev, L, cfg.mass, cfg.tol, cfg.maxiter, mode, **kw)[1]
 
+    # the iteration as one persistent kernel per <= 1024 passes against the kernel-per-step CUDA graph
+    # (DESIGN.md section 17); the timed solve above let the library choose by volume
+    st_pk = solve(stag.CG_RELIABLE, recon12=True, persistent=True)
+    st_ks = solve(stag.CG_RELIABLE, recon12=True, persistent=False)
     st64 = solve(stag.CG_F64)
     st18 = solve(stag.CG_RELIABLE)
     st64c = solve(stag.CG_F64, recon12=True)
@@ -518,6 +534,10 @@ def run_ours(args):
                "fp32_share_of_A_applications": st["iters"] / (st["iters"] + st["applies_f64"]),
                "true_resid": st["true_resid"], "time_to_solution_s": st["seconds"],
                "ms_per_iteration": st["seconds"] / max(1, st["iters"]) * 1e3,
+               "iteration_path": "chosen by volume (params.persistent = 0): %s" % (
+                   "persistent kernel" if cfg.vh <= 300000 else "kernel per step, CUDA graph of 32 passes"),
+               "persistent_kernel": brief(st_pk),
+               "kernel_per_step": brief(st_ks),
                "fp64_cg": brief(st64),
                "fp64_cg_12real_links": brief(st64c),
                "mixed_18real_links": brief(st18),
@@ -558,11 +578,16 @@ def run_slabs(args):
     stag.lib()
     cfg = fieldgen.CONFIGS[args.config]
     peak, peak_src = measured_peaks()
-    W = cfg.links()
+    # each rank generates and hands over only its own time slices of the links plus the t-links of
+    # the slice before them (stag_slab_create_local): no rank ever holds the whole gauge field
+    t0, t1 = slab.slab_range(cfg.dims, rank, world)
+    W_loc = cfg.links_slices(t0, t1 - t0)
+    W_back = np.ascontiguousarray(cfg.links_slices(t0 - 1, 1)[3])
     b_np = cfg.source()
-    S = slab.SlabLinks(cfg.dims, W, rank, world)
-    del W
+    S = slab.SlabLinks(cfg.dims, W_loc, rank, world, W_back=W_back)
+    del W_loc, W_back
     S.connect_distributed()
+    replicas.barrier()          # rank skew counts against the slab watchdog: start the first exchange together
     b_loc = np.ascontiguousarray(slab.scatter_spinor(b_np, cfg.dims, rank, world))
     b_dev = stag.spinor_pack(b_loc, S.dims, stag.PREC_F64)
     b_host = torch.from_numpy(b_loc.view(np.float64).reshape(-1).copy()).pin_memory()
@@ -614,6 +639,12 @@ def run_slabs(args):
     e1.record()
     torch.cuda.synchronize(); replicas.barrier()
     hop_us = replicas.max_over_ranks(e0.elapsed_time(e1) / 40 * 1e3, dev)
+    # the same solve on the kernel-per-step slab path (six launches per pass, a CUDA graph per 32 passes)
+    S.cg_solve(b_dev, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True, persistent=False)
+    replicas.barrier()
+    _, st_step = S.cg_solve(b_dev, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True, persistent=False)
+    step_path = {"iters": st_step["iters"], "time_to_solution_s": replicas.max_over_ranks(st_step["seconds"], dev),
+                 "ms_per_iteration": replicas.max_over_ranks(st_step["seconds"], dev) / max(1, st_step["iters"]) * 1e3}
     if rank != 0:
         replicas.finalize()
         return 0
@@ -635,7 +666,9 @@ def run_slabs(args):
                      "algorithmic_bytes_per_launch": hop_bytes, "us_per_launch": hop_us},
         "cpu_baseline": None,
         "cg": {"iters": st["iters"], "n_updates": st["n_updates"], "true_resid": st["true_resid"],
-               "time_to_solution_s": st["seconds"], "ms_per_iteration": st["seconds"] / max(1, st["iters"]) * 1e3},
+               "time_to_solution_s": st["seconds"], "ms_per_iteration": st["seconds"] / max(1, st["iters"]) * 1e3,
+               "iteration_path": "persistent kernel, one cooperative launch per <= 1024 passes (stag_persist.cuh)",
+               "kernel_per_step": step_path},
     }
     print(json.dumps(line), flush=True)
     replicas.finalize()
@@ -652,9 +685,11 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--decomp", choices=["replicas", "slabs"], default="replicas",
                     help="N > 1: independent replicas (weak scaling, default) or one lattice in T-slabs (strong)")
-    ap.add_argument("--only", choices=["all", "hops", "mrhs"], default="all",
-                    help="hops: time the stand-alone hops only; mrhs: only the three-source lockstep solve "
-                         "(the commands the ncu captures under profiles/ run)")
+    ap.add_argument("--only", choices=["all", "hops", "mrhs", "solve"], default="all",
+                    help="hops: time the stand-alone hops only; mrhs: only the three-source lockstep solve; "
+                         "solve: only the mixed solve (the commands the ncu captures under profiles/ run)")
+    ap.add_argument("--persistent", choices=["auto", "on", "off"], default="auto",
+                    help="with --only solve: force the persistent-kernel iteration on or off")
     ap.add_argument("--maxiter", type=int, default=0, help="with --only mrhs: cap the iterations (0 = the config's)")
     ap.add_argument("--hops", default="",
                     help='with --only hops: comma-separated names to run, e.g. "fp32/12,fp32/12 x4,fp32/12 x4 blocked"')

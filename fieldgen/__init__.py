@@ -41,6 +41,9 @@ def _load():
         lib.fg_links.argtypes = [dp, ip, ctypes.c_int, ctypes.c_uint64, ctypes.c_double,
                                  ctypes.c_int, ctypes.c_int]
         lib.fg_links.restype = ctypes.c_int
+        lib.fg_links_slices.argtypes = [dp, ip, ctypes.c_int, ctypes.c_uint64, ctypes.c_double,
+                                        ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]
+        lib.fg_links_slices.restype = ctypes.c_int
         lib.fg_spinor_gaussian.argtypes = [dp, ip, ctypes.c_int, ctypes.c_uint64]
         lib.fg_spinor_gaussian.restype = ctypes.c_int
         lib.fg_spinor_planewave.argtypes = [dp, ip, ctypes.c_int, ip, dp, ctypes.c_int]
@@ -83,6 +86,19 @@ def links(dims, kind: str = "random", seed: int = 0, eps: float = 0.0,
     rc = _load().fg_links(_dp(w), cd, KIND[kind], seed, float(eps), int(fold), int(antiperiodic_t))
     if rc:
         raise RuntimeError("fg_links failed")
+    return w
+
+
+def links_slices(dims, t0: int, nt: int, kind: str = "random", seed: int = 0, eps: float = 0.0,
+                 fold: bool = True, antiperiodic_t: bool = True) -> np.ndarray:
+    """Time slices t0 .. t0+nt-1 (mod X3) of links(dims, ...) without generating the rest:
+    W[mu][p][nt*s3][3][3], equal to links(...)[:, :, t0*s3:(t0+nt)*s3] when the range does not wrap."""
+    cd, d = _dims(dims)
+    s3 = d[0] * d[1] * d[2] // 2
+    w = np.empty((4, 2, int(nt) * s3, 3, 3), dtype=np.complex128)
+    rc = _load().fg_links_slices(_dp(w), cd, KIND[kind], seed, float(eps), int(fold), int(antiperiodic_t), int(t0), int(nt))
+    if rc:
+        raise RuntimeError("fg_links_slices failed")
     return w
 
 
@@ -145,6 +161,9 @@ class Config:
 
     def links(self) -> np.ndarray:
         return links(self.dims, self.kind, LINK_SEED + self.index, self.eps, True, True)
+
+    def links_slices(self, t0: int, nt: int) -> np.ndarray:
+        return links_slices(self.dims, t0, nt, self.kind, LINK_SEED + self.index, self.eps, True, True)
 
     def source(self) -> np.ndarray:
         return spinor_gaussian(self.dims, 0, SOURCE_SEED + self.index)

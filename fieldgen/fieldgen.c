@@ -183,8 +183,45 @@ static inline double phase_sign(const geom_t *g, const int x[4], int mu, int ant
     return sg;
 }
 
-/* kind: 0 = unit links, 1 = random SU(3), 2 = smooth exp(i eps H).
+/* The link W_mu(x) of the site with lexicographic index idx: a pure function of (seed, idx, mu).
+ * kind: 0 = unit links, 1 = random SU(3), 2 = smooth exp(i eps H).
  * fold: multiply by eta*bc (antiperiodic_t selects the time boundary sign). */
+static void link_at(const geom_t *g, long idx, const int x[4], int mu, int kind, uint64_t seed,
+                    double eps, int fold, int antiperiodic_t, double m[18])
+{
+    uint64_t ctr = (uint64_t)idx * 4 + (uint64_t)mu;
+    if (kind == 0) {
+        memset(m, 0, 18 * sizeof(double));
+        m[0] = m[8] = m[16] = 1.0;
+    } else if (kind == 1) {
+        for (int k = 0; k < 18; ++k) m[k] = fg_normal(seed, FG_TAG_LINK, ctr, k);
+        project_su3(m);
+    } else {
+        double gm[18], ih[18];
+        for (int k = 0; k < 18; ++k) gm[k] = fg_normal(seed, FG_TAG_LINK, ctr, k);
+        /* H = (G + G^dag)/2 - tr/3 ; ih = i*eps*H */
+        double h[18];
+        for (int i = 0; i < 3; ++i)
+            for (int j = 0; j < 3; ++j) {
+                h[(3*i+j)*2]   = 0.5 * (gm[(3*i+j)*2]   + gm[(3*j+i)*2]);
+                h[(3*i+j)*2+1] = 0.5 * (gm[(3*i+j)*2+1] - gm[(3*j+i)*2+1]);
+            }
+        double tr = (h[0] + h[8] + h[16]) / 3.0;
+        h[0] -= tr; h[8] -= tr; h[16] -= tr;
+        for (int k = 0; k < 9; ++k) {
+            ih[2*k]   = -eps * h[2*k+1];
+            ih[2*k+1] =  eps * h[2*k];
+        }
+        mat_exp(ih, m);
+        project_su3(m);
+    }
+    if (fold) {
+        double sg = phase_sign(g, x, mu, antiperiodic_t);
+        for (int k = 0; k < 18; ++k) m[k] *= sg;
+    }
+}
+
+/* The whole field W[mu][p][cb][3][3]. */
 int fg_links(double *W, const int dims[4], int kind, uint64_t seed, double eps,
              int fold, int antiperiodic_t)
 {
@@ -198,37 +235,38 @@ int fg_links(double *W, const int dims[4], int kind, uint64_t seed, double eps,
         long cb = idx >> 1;
         for (int mu = 0; mu < 4; ++mu) {
             double m[18];
-            uint64_t ctr = (uint64_t)idx * 4 + (uint64_t)mu;
-            if (kind == 0) {
-                memset(m, 0, sizeof(m));
-                m[0] = m[8] = m[16] = 1.0;
-            } else if (kind == 1) {
-                for (int k = 0; k < 18; ++k) m[k] = fg_normal(seed, FG_TAG_LINK, ctr, k);
-                project_su3(m);
-            } else {
-                double gm[18], ih[18];
-                for (int k = 0; k < 18; ++k) gm[k] = fg_normal(seed, FG_TAG_LINK, ctr, k);
-                /* H = (G + G^dag)/2 - tr/3 ; ih = i*eps*H */
-                double h[18];
-                for (int i = 0; i < 3; ++i)
-                    for (int j = 0; j < 3; ++j) {
-                        h[(3*i+j)*2]   = 0.5 * (gm[(3*i+j)*2]   + gm[(3*j+i)*2]);
-                        h[(3*i+j)*2+1] = 0.5 * (gm[(3*i+j)*2+1] - gm[(3*j+i)*2+1]);
-                    }
-                double tr = (h[0] + h[8] + h[16]) / 3.0;
-                h[0] -= tr; h[8] -= tr; h[16] -= tr;
-                for (int k = 0; k < 9; ++k) {
-                    ih[2*k]   = -eps * h[2*k+1];
-                    ih[2*k+1] =  eps * h[2*k];
-                }
-                mat_exp(ih, m);
-                project_su3(m);
-            }
-            if (fold) {
-                double sg = phase_sign(&g, x, mu, antiperiodic_t);
-                for (int k = 0; k < 18; ++k) m[k] *= sg;
-            }
+            link_at(&g, idx, x, mu, kind, seed, eps, fold, antiperiodic_t, m);
             double *dst = W + (((size_t)mu * 2 + (size_t)p) * (size_t)g.Vh + (size_t)cb) * 18;
+            memcpy(dst, m, sizeof(m));
+        }
+    }
+    return 0;
+}
+
+/* Time slices t0, t0+1, ..., t0+nt-1 (mod X3) of the same field, W[mu][p][cb'][3][3] with
+ * cb' = (slice number j)*s3 + (index inside the slice): what one rank of a T-slab decomposition
+ * needs, generated without the rest of the lattice.  Every value equals the one fg_links writes
+ * for that site (the generator is counter-based). */
+int fg_links_slices(double *W, const int dims[4], int kind, uint64_t seed, double eps,
+                    int fold, int antiperiodic_t, int t0, int nt)
+{
+    geom_t g;
+    if (!W || geom_init(&g, dims) || kind < 0 || kind > 2 || nt < 1 || nt > dims[3]) return -1;
+    const long vslice = g.V / g.X[3];          /* sites per time slice, both parities */
+    const long s3 = vslice / 2;
+#pragma omp parallel for schedule(static)
+    for (long k = 0; k < (long)nt * vslice; ++k) {
+        const int j = (int)(k / vslice);
+        const int t = ((t0 + j) % g.X[3] + g.X[3]) % g.X[3];
+        const long idx = (long)t * vslice + k % vslice;
+        int x[4];
+        site_coords(&g, idx, x);
+        int p = (x[0] + x[1] + x[2] + x[3]) & 1;
+        long cbl = (long)j * s3 + ((idx >> 1) - (long)t * s3);
+        for (int mu = 0; mu < 4; ++mu) {
+            double m[18];
+            link_at(&g, idx, x, mu, kind, seed, eps, fold, antiperiodic_t, m);
+            double *dst = W + (((size_t)mu * 2 + (size_t)p) * (size_t)(nt * s3) + (size_t)cbl) * 18;
             memcpy(dst, m, sizeof(m));
         }
     }

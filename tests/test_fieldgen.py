@@ -1,5 +1,6 @@
 """The seeded input generator: SU(3)-ness, folded phases, reproducibility."""
 import numpy as np
+import pytest
 import scipy.linalg
 
 import fieldgen
@@ -100,3 +101,17 @@ def test_config_table_matches_baseline_json():
     assert c["c1_4^4"].mass == 0.1 and c["c2_8^4"].mass == 0.05
     assert c["c3_16^3x32"].eps == 0.3 and c["c5_48^3x96"].eps == 0.5
     assert c["c4_28^3x96"].mass == 0.0124 and c["c5_48^3x96"].mass == 0.005
+
+
+@pytest.mark.parametrize("kind,eps", [("random", 0.0), ("smooth", 0.3), ("unit", 0.0)])
+def test_time_slices_generated_alone_equal_the_whole_field(kind, eps):
+    """fg_links_slices: what a rank of a T-slab decomposition generates for itself is bit-identical to
+    the same slices of the whole field, including a range that wraps around the time extent (the
+    slice before a slab that starts at t = 0)."""
+    dims = (4, 2, 6, 8)
+    s3 = dims[0] * dims[1] * dims[2] // 2
+    W = fieldgen.links(dims, kind, seed=17, eps=eps)
+    for t0, nt in ((0, 8), (2, 4), (6, 2), (7, 1), (-1, 1)):
+        part = fieldgen.links_slices(dims, t0, nt, kind, seed=17, eps=eps)
+        want = np.concatenate([W[:, :, ((t0 + j) % 8) * s3:((t0 + j) % 8 + 1) * s3] for j in range(nt)], axis=2)
+        assert part.shape == want.shape and np.array_equal(part, want)
