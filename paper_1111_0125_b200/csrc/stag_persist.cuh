@@ -148,7 +148,9 @@ __device__ __forceinline__ void iter_epilogue_local(IterScalars &S, const double
 // Tiles are dealt to the group's warps statically (warp w takes tiles w, w + W, ...).  A dynamic deal
 // from one atomic counter was tried to trim the 4-8 us of stragglers at the barrier after each hop on
 // 28^3 x 96 (14 trips for some warps, 13 for others; SMs of unequal speed): 33 k same-address atomics
-// per phase serialise in L2 and the hop went from 62 to 96 us (profiles/README.md, round 2).
+// per phase serialise in L2 and the hop went from 62 to 96 us; chunks of 1-4 tiles per ticket, drawn one
+// chunk ahead (8 k atomics per phase), left the hop at 66-71 us against 62-67 and cost 28^3 x 12 six
+// microseconds per pass (profiles/README.md, round 2).  The stragglers are not the deal's.
 // LRES: the links of both parities and the five vectors fit L2 together (the host decides): the link
 // packets are then loaded with the keep policy and every pass after the first reads them from L2.
 template <typename T, int NR, bool SLAB, bool LRES>
