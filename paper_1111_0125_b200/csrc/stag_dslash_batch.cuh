@@ -56,6 +56,21 @@ __device__ __forceinline__ void prefetch_l2_bulk_stream(const void *p, unsigned 
 #ifndef STAG_BATCH_MINB
 #define STAG_BATCH_MINB 4
 #endif
+// STAG_BATCH_FFMA2 = 1: the two right-hand sides of a pair go through the packed fp32 FMA of sm_100
+// (fma.rn.f32x2, __ffma2_rn: two IEEE fmas per instruction).  The accumulators of a pair are held as
+// X_i = (Re acc_a, Re acc_b), Y_i = (Im acc_a, Im acc_b), the gathered float4 is split into
+// VX = (Re v_a, Re v_b), VY = (Im v_a, Im v_b), and one complex multiply-add of BOTH right-hand sides is
+//   X = fma2((m.x, m.x), VX, X);  X = fma2((-m.y, -m.y), VY, X);  Y = fma2((m.x, m.x), VY, Y);  Y = fma2((m.y, m.y), VX, Y)
+// -- per component the same four fmas in the same order as cfma, so the result is bit-identical.
+// Four packed instructions instead of eight scalar ones on the FMA pipe, paid for with the moves that
+// build the duplicated matrix entries: SASS of N = 4, 12-real has 576 FFMA2 + 823 MOV where the scalar
+// form has 1248 FFMA (the duplicates are rebuilt per pair: 128 registers do not hold 27 of them across
+// the pairs).  Measured on 28^3 x 96: x2 84.5 us against 80.4, x3 101.6 against 89.7, x4 122.8 against
+// 100.7 -- the hop is bound by issue slots, not by the FMA pipe (47 % busy), and the moves cost more
+// slots than the packing saves.  Off.
+#ifndef STAG_BATCH_FFMA2
+#define STAG_BATCH_FFMA2 0
+#endif
 template <int NR, int N> struct BatchTune {
     static constexpr int MINB = STAG_BATCH_MINB;
     static constexpr int LD = (NR == 3) ? 1 : (STAG_BATCH_LD ? STAG_BATCH_LD : (N == 3 ? 3 : 2));
@@ -164,6 +179,13 @@ dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
 #pragma unroll
             for (int i = 0; i < 3; ++i) acc[k][i] = make_float2(0.f, 0.f);
 
+#if STAG_BATCH_FFMA2
+        float2 AX[(N / 2) ? (N / 2) : 1][3], AY[(N / 2) ? (N / 2) : 1][3];     // packed accumulators of the pairs
+#pragma unroll
+        for (int u = 0; u < N / 2; ++u)
+#pragma unroll
+            for (int i = 0; i < 3; ++i) AX[u][i] = AY[u][i] = make_float2(0.f, 0.f);
+#endif
         Unit vb[2];
         Unit ow[NU];       // the own-site vectors of the epilogue (MODE != HOP_PLAIN)
         gather(vb[0], 0, s.nbr[0]);
@@ -194,6 +216,22 @@ dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
                 if (step + 1 < 8 * NU) gather(vb[(step + 1) & 1], (u + 1) % NU, s.nbr[(step + 1) / NU]);
                 const Unit &v = vb[step & 1];
                 if (PAIRED && 2 * u + 1 < N) {
+#if STAG_BATCH_FFMA2
+                    float2 VX[3], VY[3];
+#pragma unroll
+                    for (int j = 0; j < 3; ++j) { VX[j] = make_float2(v.q[j].x, v.q[j].z); VY[j] = make_float2(v.q[j].y, v.q[j].w); }
+#pragma unroll
+                    for (int i = 0; i < 3; ++i)
+#pragma unroll
+                        for (int j = 0; j < 3; ++j) {
+                            const C mm = m[3 * i + j];
+                            const float2 MX = make_float2(mm.x, mm.x), MY = make_float2(mm.y, mm.y), nMY = make_float2(-mm.y, -mm.y);
+                            AX[u][i] = __ffma2_rn(MX, VX[j], AX[u][i]);
+                            AX[u][i] = __ffma2_rn(nMY, VY[j], AX[u][i]);
+                            AY[u][i] = __ffma2_rn(MX, VY[j], AY[u][i]);
+                            AY[u][i] = __ffma2_rn(MY, VX[j], AY[u][i]);
+                        }
+#else
 #pragma unroll
                     for (int i = 0; i < 3; ++i)
 #pragma unroll
@@ -201,6 +239,7 @@ dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
                             cfma(acc[2 * u][i], m[3 * i + j], make_float2(v.q[j].x, v.q[j].y));
                             cfma(acc[2 * u + 1][i], m[3 * i + j], make_float2(v.q[j].z, v.q[j].w));
                         }
+#endif
                 } else {
                     const int k = PAIRED ? N - 1 : u;
 #pragma unroll
@@ -211,6 +250,17 @@ dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
             }
         }
 
+#if STAG_BATCH_FFMA2
+        if constexpr (PAIRED) {
+#pragma unroll
+            for (int u = 0; u < N / 2; ++u)
+#pragma unroll
+                for (int i = 0; i < 3; ++i) {
+                    acc[2 * u][i] = make_float2(AX[u][i].x, AY[u][i].x);
+                    acc[2 * u + 1][i] = make_float2(AX[u][i].y, AY[u][i].y);
+                }
+        }
+#endif
         if (NR == 1 && cb >= g.Vh) {
             // a rebuilt 8-parameter matrix is unitary, never zero: pad lanes are zeroed here
 #pragma unroll
