@@ -234,3 +234,45 @@ def test_a_dead_slab_takes_its_neighbours_down_and_reset_revives_them():
     assert [s.status() for s in slabs] == [stag.OK, stag.OK]
     for s in slabs:
         s.close()
+
+
+def test_persistent_kernel_of_one_rank_alone_times_out_instead_of_hanging():
+    """Every wait inside the persistent kernel is bounded by the slab's watchdog: with two ranks
+    connected but only rank 0's iterations launched (stag_slab_cg_iter_all on one slab), rank 0's
+    boundary threads wait for faces rank 1 never pushes, give up, the group leaves the kernel and the
+    next control call reports STAG_ETIMEOUT.  Argument errors of the fused launch on the way."""
+    import ctypes
+    dims, mass = (4, 4, 4, 8), 0.1
+    W = fieldgen.links(dims, "random", seed=79)
+    b = fieldgen.spinor_gaussian(dims, 0, seed=80)
+    slabs = make_slabs(dims, W, 2)
+    for s in slabs:
+        s.set_wait_limit(2000)
+    bs = [stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(b, dims, r, 2)), slabs[r].dims, 0) for r in range(2)]
+    import torch
+    xs = [torch.zeros_like(v) for v in bs]
+    for s, x, v in zip(slabs, xs, bs):
+        s.cg_begin(x, v, mass, 1e-10, 100, stag.CG_RELIABLE, recon12=True)
+    one = (ctypes.c_void_p * 1)(slabs[0].handle.value)
+    two = (ctypes.c_void_p * 2)(slabs[0].handle.value, slabs[0].handle.value)
+    assert stag.lib().stag_slab_cg_iter_all(one, 1) == stag.EINVAL          # not yet told to iterate
+    # |b|^2 and the initial residual in lockstep, as cg_solve_in_process does
+    while True:
+        acts = [s.cg_control() for s in slabs]
+        if acts[0] == slab.ACT_ITER:
+            break
+        ph = 0
+        while True:
+            more = [s.cg_step(acts[0], ph) for s in slabs]
+            if not more[0]:
+                break
+            ph += 1
+    assert stag.lib().stag_slab_cg_iter_all(two, 2) == stag.EINVAL          # the same slab twice
+    assert stag.lib().stag_slab_cg_iter_all(one, 0) == stag.EINVAL
+    assert stag.lib().stag_slab_cg_iter_all(one, 1) == stag.OK              # rank 0 alone: nobody answers
+    with pytest.raises(stag.StagError) as e:
+        slabs[0].cg_control()
+    assert e.value.status == stag.ETIMEOUT
+    assert slabs[0].status() == stag.ETIMEOUT and slabs[1].status() == stag.OK
+    for s in slabs:
+        s.close()
