@@ -166,6 +166,10 @@ struct CgCtrl {
     int n_updates;
     int nrhs;
     unsigned ticket[4];      // last-block tickets, one per reducing kernel role
+    // written by the persistent iteration kernel (stag_persist.cuh) when it returns:
+    int have_true;           // 1: the launch ended with a reliable update done IN the kernel, so sum0 is
+                             //    |b - A x|^2 of the current x; 0: passes followed it (or none was done)
+    int n_inkernel;          // reliable updates done in the kernel so far (each one fp64 application of A)
 };
 constexpr int CTRL_SLOT = 2048;   // bytes reserved for CgCtrl in the workspace
 static_assert(sizeof(CgCtrl) <= CTRL_SLOT, "CgCtrl must fit its workspace slot");

@@ -208,6 +208,7 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
     if (persist) {
         if (lo) {
             persist_fill<float>(pa32.rk[0], L, w, S.prec_lo, S.m2, w.y32, w.r32, w.d32, w.q32, w.tmp32);
+            if (mode == STAG_CG_RELIABLE && S.prec_hi == STAG_PREC_F64) persist_fill_update(pa32.rk[0].up, L, w, x, b, S.m2);
             pa32.nlocal = 1; pa32.max_iters = P.persist_chunk;
         } else {
             persist_fill<double>(pa64.rk[0], L, w, S.prec_lo, S.m2, x, w.r64, w.d64, w.q64, w.tmp64);
@@ -254,14 +255,18 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
     int final_state = CG_RUN;
     bool have_true = true;      // ctrl->sum0[k] holds |b_k - A x_k|^2 for the current x
     bool verifying = false;     // mode 0: the last launch was the true-residual check of Q6b
+    bool persist_ran = false;   // the last thing launched was the persistent kernel: it says whether sum0 is current
     for (;;) {
         if ((rc = S.read_ctrl())) return rc;
         const int state = h->state;
+        if (persist_ran) { have_true = h->have_true != 0; persist_ran = false; }
         if (state == CG_RUN) {
             if (verifying) ++n_restarts;
             verifying = false;
             if (persist) {
                 if ((rc = lo ? persist_launch<float>(pa32, S.prec_lo, false, s) : persist_launch<double>(pa64, S.prec_lo, false, s))) return rc;
+                persist_ran = true;
+                continue;
             } else if (gexec) {
                 CU(cudaGraphLaunch(gexec, s));
                 count_launch(graph_nodes);
@@ -327,7 +332,7 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
         st.n_updates = (mode == STAG_CG_DEFECT) ? n_outer : h->n_updates;
         st.n_restarts = n_restarts;
         st.iters_f32 = lo ? h->iters[k] : 0;
-        st.applies_f64 = S.applies_f64;
+        st.applies_f64 = S.applies_f64 + h->n_inkernel;
         st.true_resid = bnorm2[k] > 0.0 ? sqrt(h->sum0[k] / bnorm2[k]) : 0.0;
         st.iter_resid = bnorm2[k] > 0.0 ? sqrt(h->sum1[k] / bnorm2[k]) : 0.0;
         st.seconds = ms * 1e-3;

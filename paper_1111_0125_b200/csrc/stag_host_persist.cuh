@@ -87,6 +87,18 @@ void persist_fill(IterRank<T> &R, const stag_links *L, const Workspace &w, int p
     R.peer_fwd = L->peer_fwd; R.peer_bwd = L->peer_bwd;
     R.peers = L->peers_dev;
     R.nranks = L->nranks; R.myrank = L->rank;
+    memset(&R.up, 0, sizeof(R.up));          // reliable updates are the host's unless persist_fill_update follows
+}
+
+// Mode 3 with the fp64 corrections on 18-real links: the kernel does the reliable + group-wise update
+// itself (x += y, r = b - A x in fp64), so a whole solve is one launch per persist_chunk passes.
+inline void persist_fill_update(IterUpdate &U, const stag_links *L, const Workspace &w, double *x, const double *b, double m2)
+{
+    const size_t per_parity = (size_t)L->ntiles * (8 * link_slots(3)) * TILE;
+    U.x = x; U.b = b; U.tmp = w.tmp64;
+    U.links_even = (const double2 *)L->L[STAG_PREC_F64];
+    U.links_odd = U.links_even + per_parity;
+    U.m2 = m2;
 }
 
 template <typename T, int NR, bool SLAB, bool LRES>

@@ -271,6 +271,7 @@ struct stag_slab_cg {
     bool have_true, verifying;
     int n_restarts, applies_f64, final_state;
     bool persist;                    // stag_slab_cg_run iterates in the persistent kernel (stag_persist.cuh)
+    bool persist_ran;                // the last action was a persistent launch: ctrl->have_true says whether sum0 is current
     double bnorm2;
     int rc_final;
 };
@@ -448,11 +449,13 @@ int slab_iter_all_t(stag_links_t *const *slabs, int n, cudaStream_t s)
         stag_links *L = slabs[i];
         stag_slab_cg *C = L->cg;
         Workspace &w = C->w;
-        if (std::is_same<T, float>::value)
+        if (std::is_same<T, float>::value) {
             persist_fill<T>(A.rk[i], L, w, C->prec_lo, C->m2, (T *)w.y32, (T *)w.r32, (T *)w.d32, (T *)w.q32, (T *)w.tmp32);
-        else
+            if (C->mode == STAG_CG_RELIABLE && C->prec_hi == STAG_PREC_F64) persist_fill_update(A.rk[i].up, L, w, C->x, C->b, C->m2);
+        } else
             persist_fill<T>(A.rk[i], L, w, C->prec_lo, C->m2, (T *)C->x, (T *)w.r64, (T *)w.d64, (T *)w.q64, (T *)w.tmp64);
         ++L->epoch;
+        C->persist_ran = true;
     }
     A.nlocal = n;
     A.max_iters = C0->P.persist_chunk;
@@ -508,6 +511,7 @@ extern "C" int stag_slab_cg_control(stag_links_t *L, int *action_out)
         return STAG_OK;
     }
     const int state = h->state;
+    if (C->persist_ran) { C->have_true = h->have_true != 0; C->persist_ran = false; }
     if (state == CG_RUN) {
         if (C->verifying) ++C->n_restarts;
         C->verifying = false;
@@ -620,7 +624,7 @@ extern "C" int stag_slab_cg_finish(stag_links_t *L, stag_cg_stats_t *stats_out)
     st.n_updates = h->n_updates;
     st.n_restarts = C->n_restarts;
     st.iters_f32 = C->lo ? h->iters[0] : 0;
-    st.applies_f64 = C->applies_f64;
+    st.applies_f64 = C->applies_f64 + h->n_inkernel;
     st.true_resid = C->bnorm2 > 0.0 ? sqrt(h->sum0[0] / C->bnorm2) : 0.0;
     st.iter_resid = C->bnorm2 > 0.0 ? sqrt(h->sum1[0] / C->bnorm2) : 0.0;
     st.seconds = ms * 1e-3;

@@ -16,6 +16,8 @@
 //   --- barrier ---   every block adds the partials in index order   [slab: publish, gather over ranks]
 //   P3  alpha; y += alpha d; r -= alpha q; |r|^2 partials
 //   --- barrier ---   every block adds them, runs the scalar step on its own copy of the scalars
+//   [mode 3, on the trigger of P:L97: x += y, y = 0 | barrier | tmp = D_oe x (fp64) | barrier |
+//    r = b - (m^2 x - D_eo tmp), fp32 copy, |r|^2 | barrier | sum, beta from the corrected residual]
 //
 // Scalars are REPLICATED: every block carries delta, beta, maxr, the counters and the state in shared
 // memory and evolves them from the same sums in the same order, so no block ever reads a scalar
@@ -62,6 +64,16 @@ __device__ __forceinline__ unsigned long long persist_now()
 // How many blocks per SM the launch bounds promise ptxas (registers per thread = 65536 / (256 * BPS)).
 template <typename T, int NR> struct PersistTune { static constexpr int BPS = 512 / PERSIST_THREADS; };
 
+// What the reliable + group-wise update of section 3.2 (step S6) needs when it is done
+// INSIDE the kernel (fp32 iteration, mode 3): links_even == null leaves it to the host as before.
+struct IterUpdate {
+    double *x;                               // the fp64 solution x += y goes into
+    const double *b;                         // the right-hand side (pad lanes read as zero)
+    double *tmp;                             // odd-site scratch of A x in fp64
+    const double2 *links_even, *links_odd;   // fp64, 18-real gathered fields
+    double m2;
+};
+
 template <typename T> struct IterRank {
     T *y, *r, *d, *q, *tmp;                  // flat spinors, 6*Vh_pad reals; y = x itself in mode 0
     const pkt_t<T> *links_even, *links_odd;  // gathered fields of the even / odd OUTPUT sites
@@ -75,6 +87,7 @@ template <typename T> struct IterRank {
     char *xch, *peer_fwd, *peer_bwd;
     char *const *peers;
     int nranks, myrank;
+    IterUpdate up;
 };
 template <typename T> struct IterArgs {
     IterRank<T> rk[MAX_RANKS];
@@ -83,8 +96,8 @@ template <typename T> struct IterArgs {
 };
 
 struct IterScalars {
-    double delta, beta, maxr, tol2b, inner2, eps_in, dAd, alpha, sum1;
-    int state, iter, maxiter, mode, iters, active;
+    double delta, beta, maxr, tol2b, inner2, eps_in, dAd, alpha, sum1, sum0;
+    int state, iter, maxiter, mode, iters, active, n_updates, have_true, n_inkernel;
 };
 
 // Barrier among the nb blocks of one rank group: a monotonic arrival counter, zeroed by the host
@@ -122,6 +135,7 @@ __device__ __forceinline__ void iter_epilogue_local(IterScalars &S, const double
     S.iter = it;
     S.iters += 1;
     S.sum1 = dn;
+    S.have_true = 0;
     bool breakdown = false, trigger = false, conv = false;
     if (!(S.dAd > 0.0) || !(dn == dn)) breakdown = true;
     else if (S.mode == STAG_CG_RELIABLE) {
@@ -153,6 +167,26 @@ __device__ __forceinline__ void iter_epilogue_local(IterScalars &S, const double
 // microseconds per pass (profiles/README.md, round 2).  The stragglers are not the deal's.
 // LRES: the links of both parities and the five vectors fit L2 together (the host decides): the link
 // packets are then loaded with the keep policy and every pass after the first reads them from L2.
+// The scalar step after a reliable update done in the kernel: residual_epilogue<RES_UPDATE>
+// (stag_blas.cuh) restated on IterScalars.  dn = |b - A x|^2 in fp64 (Q9, Q10, Q11).
+__device__ __forceinline__ void update_epilogue_local(IterScalars &S, const double dn)
+{
+    S.sum0 = dn;
+    S.have_true = 1;
+    S.n_updates += 1;
+    S.n_inkernel += 1;
+    const bool bad = !(dn == dn);
+    if (!bad && S.active) {
+        S.maxr = sqrt(dn);                                                 // Q9
+        if (dn <= S.tol2b) S.active = 0;
+        else { S.beta = dn / S.delta; S.delta = dn; }                      // Q10
+    }
+    int st = S.active ? CG_RUN : CG_CONVERGED;
+    if (bad) st = CG_BREAKDOWN;
+    else if (S.active && S.iter >= S.maxiter) st = CG_MAXITER;
+    S.state = st;
+}
+
 template <typename T, int NR, bool SLAB, bool LRES>
 __global__ void __launch_bounds__(PERSIST_THREADS, PersistTune<T, NR>::BPS)
 cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
@@ -185,6 +219,8 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
         S.dAd = __ldcg(&c->dAd[0]); S.alpha = __ldcg(&c->alpha[0]); S.sum1 = __ldcg(&c->sum1[0]);
         S.state = __ldcg(&c->state); S.iter = __ldcg(&c->iter); S.maxiter = __ldcg(&c->maxiter);
         S.mode = __ldcg(&c->mode); S.iters = __ldcg(&c->iters[0]); S.active = __ldcg(&c->active[0]);
+        S.sum0 = __ldcg(&c->sum0[0]); S.n_updates = __ldcg(&c->n_updates);
+        S.have_true = 0; S.n_inkernel = __ldcg(&c->n_inkernel);
         if (!S.active && S.state == CG_RUN) S.state = CG_CONVERGED;
     }
     __syncthreads();
@@ -363,6 +399,93 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
             iter_epilogue_local(S, dn);
         }
         __syncthreads();
+
+        // ---- S6 in the kernel: x += y, y = 0 (group-wise); r = b - A x in fp64, its fp32 copy and
+        // |r|^2 (reliable); beta from the corrected residual with d kept (eq. 3.1, Q10) --------------
+        if constexpr (sizeof(T) == 4) {
+            if (S.state == CG_UPDATE && R.up.links_even != nullptr) {
+                const IterUpdate &U = R.up;
+                using D2 = double2;
+                D2 *x_c = reinterpret_cast<D2 *>(U.x), *t_c = reinterpret_cast<D2 *>(U.tmp);
+                {   // U0: x += y ; y = 0 -- one float4 of y = two complex numbers of x   [slab: the faces of x pushed]
+                    float4 *yv = reinterpret_cast<float4 *>(R.y);
+                    for (long i = tid; i < nv; i += nthreads) {
+                        const float4 yy = ld_pass(yv + i);
+                        D2 a = x_c[2 * i], b2 = x_c[2 * i + 1];
+                        a.x += (double)yy.x; a.y += (double)yy.y; b2.x += (double)yy.z; b2.y += (double)yy.w;
+                        x_c[2 * i] = a; x_c[2 * i + 1] = b2;
+                        st_pass(yv + i, make_float4(0.f, 0.f, 0.f, 0.f));
+                        if constexpr (SLAB) {
+                            const long ci = 2 * i;
+                            const int c = (ci >= 2L * g.Vh_pad) ? 2 : (ci >= g.Vh_pad ? 1 : 0);
+                            const int cb = (int)(ci - (long)c * g.Vh_pad);
+                            if (cb < g.s3) {
+                                D2 *dst = (D2 *)(R.peer_bwd + xch_halo_offset(g.s3, epoch + 1, 1)) + (long)c * g.s3 + cb;
+                                dst[0] = a; dst[1] = b2;
+                            } else if (cb >= g.Vh - g.s3 && cb < g.Vh) {
+                                D2 *dst = (D2 *)(R.peer_fwd + xch_halo_offset(g.s3, epoch + 1, 0)) + (long)c * g.s3 + (cb - (g.Vh - g.s3));
+                                dst[0] = a; dst[1] = b2;
+                            }
+                        }
+                    }
+                }
+                if (!group_barrier(R.bar, bar_target += (unsigned)nb, hdr)) return;
+                if constexpr (SLAB) { if (slab_dead(R.xch)) return; ++epoch; raise_flags(epoch); }
+                // U1: tmp = D_oe x in fp64 on the 18-real links
+                for (int t = warp_g; t < ntiles; t += nwarps) {
+                    int cb = t * TILE + lane;
+                    if constexpr (SLAB) { cb += g.s3; if (cb >= g.Vh_pad) cb -= g.Vh_pad; }
+                    Site s;
+                    decode_site(g, 1, cb < g.Vh ? cb : 0, s);
+                    D2 acc[3];
+                    hop_site<double, 3, SLAB, false, false>(acc, x_c, U.links_odd, g, cb, s, 0u, R.xch, [=]() { return epoch; });
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) t_c[(size_t)c * g.Vh_pad + cb] = acc[c];
+                    if constexpr (SLAB) {
+                        if (cb < g.Vh && (s.x3 == 0 || s.x3 == g.X3 - 1)) {
+                            D2 *dst = (s.x3 == 0)
+                                ? (D2 *)(R.peer_bwd + xch_halo_offset(g.s3, epoch + 1, 1)) + cb
+                                : (D2 *)(R.peer_fwd + xch_halo_offset(g.s3, epoch + 1, 0)) + (cb - (g.Vh - g.s3));
+#pragma unroll
+                            for (int c = 0; c < 3; ++c) dst[(size_t)c * g.s3] = acc[c];
+                        }
+                    }
+                }
+                if (!group_barrier(R.bar, bar_target += (unsigned)nb, hdr)) return;
+                if constexpr (SLAB) { if (slab_dead(R.xch)) return; ++epoch; raise_flags(epoch); }
+                // U2: r = b - (m^2 x - D_eo tmp), its fp32 copy, |r|^2
+                double s3sum = 0.0;
+                const D2 *b_c = reinterpret_cast<const D2 *>(U.b);
+                float2 *r_c = reinterpret_cast<float2 *>(R.r);
+                for (int t = warp_g; t < ntiles; t += nwarps) {
+                    int cb = t * TILE + lane;
+                    if constexpr (SLAB) { cb += g.s3; if (cb >= g.Vh_pad) cb -= g.Vh_pad; }
+                    Site s;
+                    decode_site(g, 0, cb < g.Vh ? cb : 0, s);
+                    D2 acc[3];
+                    hop_site<double, 3, SLAB, false, false>(acc, t_c, U.links_even, g, cb, s, 0u, R.xch, [=]() { return epoch; });
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        const D2 o = x_c[(size_t)c * g.Vh_pad + cb];
+                        D2 bb = make_double2(0.0, 0.0);
+                        if (cb < g.Vh) bb = b_c[(size_t)c * g.Vh_pad + cb];       // b's pad lanes count as zero
+                        const double vx = bb.x - fma(U.m2, o.x, -acc[c].x), vy = bb.y - fma(U.m2, o.y, -acc[c].y);
+                        r_c[(size_t)c * g.Vh_pad + cb] = make_float2((float)vx, (float)vy);
+                        s3sum += vx * vx + vy * vy;
+                    }
+                }
+                {
+                    const double bs = block_sum(s3sum, red);
+                    if (threadIdx.x == 0) partA[lb] = bs;
+                }
+                if (!group_barrier(R.bar, bar_target += (unsigned)nb, hdr)) return;
+                if constexpr (SLAB) { if (slab_dead(R.xch)) return; }
+                double rn2;
+                if (!total_over_ranks(partA, &rn2)) return;
+                if (threadIdx.x == 0) update_epilogue_local(S, rn2);
+                __syncthreads();
+            }
+        }
     }
 
     if (lb == 0 && threadIdx.x == 0) {
@@ -370,6 +493,7 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
         c->delta[0] = S.delta; c->beta[0] = S.beta; c->maxr[0] = S.maxr;
         c->dAd[0] = S.dAd; c->alpha[0] = S.alpha; c->sum1[0] = S.sum1;
         c->iter = S.iter; c->iters[0] = S.iters; c->active[0] = S.active;
+        c->sum0[0] = S.sum0; c->n_updates = S.n_updates; c->have_true = S.have_true; c->n_inkernel = S.n_inkernel;
         c->state = S.state;
         if constexpr (SLAB) { hdr->epoch = epoch; hdr->red_seq = seq; }
     }
