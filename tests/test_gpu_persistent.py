@@ -91,3 +91,32 @@ def test_persistent_is_bit_reproducible_and_independent_of_the_chunk():
     for x, st in runs[1:]:
         assert st["iters"] == runs[0][1]["iters"] and bool((x == runs[0][0]).all())
     L.close()
+
+
+def test_mixed_solve_is_one_launch_with_the_reliable_updates_inside_the_kernel():
+    """Mode 3, fp64 corrections on 18-real links: the trigger of P:L97 is served inside the persistent
+    kernel (x += y, r = b - A x in fp64, beta from the corrected residual), so after the initial
+    residual the whole solve is ONE launch -- counted -- and still meets every bar."""
+    dims, mass, tol = (8, 8, 8, 8), 0.05, 1e-10
+    W = fieldgen.links(dims, "random", seed=87)
+    b = fieldgen.spinor_gaussian(dims, 0, seed=88)
+    x_ref, _, _, _, rc = oracle.cg(b, W, dims, mass, 1e-12, 50000)
+    assert rc == 0
+    L = stag.Links(dims, W)
+    bd = stag.spinor_pack(b, dims, 0)
+    stag.cg_solve(bd, L, mass, tol, 20000, stag.CG_RELIABLE, recon12=True, persistent=True)     # derive the link forms
+    stag.reset_launch_count()
+    x, st = stag.cg_solve(bd, L, mass, tol, 20000, stag.CG_RELIABLE, recon12=True, persistent=True, persist_chunk=100000)
+    launches = stag.launch_count()
+    assert st["status"] == stag.OK and st["true_resid"] <= tol
+    assert st["n_updates"] >= 3 and st["applies_f64"] == st["n_updates"] + 1      # the initial residual + one per update
+    assert launches <= 6, launches        # |b|^2, two hops and the residual of r0, the persistent kernel: no launch per update
+    xs = stag.spinor_unpack(x, dims, 0)
+    assert rel_err(xs, x_ref) <= 1e-8
+    assert _true_resid(xs, b, W, dims, mass) <= tol * (1 + 1e-3)
+    # with 12-real fp64 corrections the update stays on the host: more launches, same solution within the bars
+    stag.reset_launch_count()
+    x2, st2 = stag.cg_solve(bd, L, mass, tol, 20000, stag.CG_RELIABLE, recon12=True, recon12_f64=True, persistent=True)
+    assert stag.launch_count() > launches and st2["status"] == stag.OK
+    assert rel_err(stag.spinor_unpack(x2, dims, 0), x_ref) <= 1e-8
+    L.close()
