@@ -645,6 +645,11 @@ def run_slabs(args):
     _, st_step = S.cg_solve(b_dev, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True, persistent=False)
     step_path = {"iters": st_step["iters"], "time_to_solution_s": replicas.max_over_ranks(st_step["seconds"], dev),
                  "ms_per_iteration": replicas.max_over_ranks(st_step["seconds"], dev) / max(1, st_step["iters"]) * 1e3}
+    S.cg_solve(b_dev, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True, persistent=True)
+    replicas.barrier()
+    _, st_pers = S.cg_solve(b_dev, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True, persistent=True)
+    pers_path = {"iters": st_pers["iters"], "time_to_solution_s": replicas.max_over_ranks(st_pers["seconds"], dev),
+                 "ms_per_iteration": replicas.max_over_ranks(st_pers["seconds"], dev) / max(1, st_pers["iters"]) * 1e3}
     if rank != 0:
         replicas.finalize()
         return 0
@@ -667,8 +672,10 @@ def run_slabs(args):
         "cpu_baseline": None,
         "cg": {"iters": st["iters"], "n_updates": st["n_updates"], "true_resid": st["true_resid"],
                "time_to_solution_s": st["seconds"], "ms_per_iteration": st["seconds"] / max(1, st["iters"]) * 1e3,
-               "iteration_path": "persistent kernel, one cooperative launch per <= 1024 passes (stag_persist.cuh)",
-               "kernel_per_step": step_path},
+               "iteration_path": "chosen by volume (params.persistent = 0): %s" % (
+                   "persistent kernel, one cooperative launch per <= 1024 passes" if cfg.vh // world <= 800000
+                   else "kernel per step, CUDA graph of 32 passes"),
+               "persistent_kernel": pers_path, "kernel_per_step": step_path},
     }
     print(json.dumps(line), flush=True)
     replicas.finalize()

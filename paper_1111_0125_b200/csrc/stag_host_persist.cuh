@@ -12,9 +12,11 @@ static_assert(sizeof(CgCtrl) <= PERSIST_BAR_OFF && PERSIST_BAR_OFF + sizeof(unsi
 
 // persistent = 0 picks the persistent kernel for whole lattices of at most this many sites per parity
 // (28^3 x 24 = 263 424: 47.8 us per pass against 50.4 on the kernel-per-step path; at 28^3 x 48 the
-// two are level and beyond it the stand-alone hops win, profiles/README.md round 2), and always for
-// T-slabs, whose kernel-per-step pass has six launches.
+// two are level and beyond it the stand-alone hops win, profiles/README.md round 2).  T-slabs, whose
+// kernel-per-step pass has six launches, gain up to a larger volume: 28^3 x 48 (526 848 sites) 101.0 us
+// per pass against 107.5, 28^3 x 96 199.0-200.2 against 193.9-197.7.
 constexpr int PERSIST_AUTO_MAX_VH = 300000;
+constexpr int PERSIST_AUTO_MAX_VH_SLAB = 800000;
 
 inline bool persist_prec_ok(int prec)     // the 8-parameter forms stay on the kernel-per-step path
 {
@@ -45,7 +47,7 @@ int persist_capacity()
 // that stream from HBM, so on one GPU it pays for small volumes only.
 inline bool persist_by_volume(const Geom &g, bool is_slab)
 {
-    return is_slab || g.Vh <= PERSIST_AUTO_MAX_VH;
+    return g.Vh <= (is_slab ? PERSIST_AUTO_MAX_VH_SLAB : PERSIST_AUTO_MAX_VH);
 }
 
 // Bytes of links + vectors up to which the persistent kernel keeps the links in L2: 5/8 of the
