@@ -9,7 +9,7 @@
 // RANK GROUP instead of a kernel boundary:
 //
 //   P0  d = r + beta d                      [slab: the faces of d stored into the neighbours' halos]
-//   --- barrier ---                         [slab: block 0 release-stores the neighbours' flags]
+//   --- barrier ---                         [slab: block 0 fences at system scope, sets the neighbours' flags]
 //   P1  tmp = D_oe d                        [slab: boundary slices last, halo after an acquire-wait;
 //   --- barrier ---                          the faces of tmp pushed, flags as above]
 //   P2  q = m^2 d - D_eo tmp, <d,q> partials

@@ -7,8 +7,8 @@
 // memory mapped into this process with CUDA IPC or, for slabs that share a process, used directly)
 // by the kernel that PRODUCES that spinor -- slab_xpay_push_kernel for the direction d, the
 // boundary-slice threads of hop 1 for its output (stag_dslash.cuh) -- or, stand-alone, by
-// face_push_kernel; a system-scope release store of the exchange's number into each neighbour's
-// flag follows.  The consuming hop (dslash_kernel<..., HALO = true>) waits on
+// face_push_kernel; the exchange's number is then stored into each neighbour's flag behind one
+// system-scope fence (raise_halo_flags, stag_dslash.cuh).  The consuming hop (dslash_kernel<..., HALO = true>) waits on
 // its own two flags only in the threads of the first and last time slice, which it visits last.
 //
 // The slab CG's global sums go through the same region: a rank stores its local total into slot
@@ -24,7 +24,7 @@
 // Ordering of a push: every storing block's thread 0, after the block barrier, fences at gpu scope and
 // takes a ticket; the ticket's last holder has thereby observed all of them, fences at SYSTEM scope
 // (cumulative over everything that happens-before it, i.e. every block's peer stores) and only then
-// release-stores the flags.  One system-scope fence per launch instead of one per storing block:
+// stores the flags (raise_halo_flags: fence.acq_rel.sys, then two relaxed system-scope stores).  One system-scope fence per launch instead of one per storing block:
 // those sat at the tail of the kernel and cost ~8 us.
 // Double buffering by epoch parity is enough: a rank cannot start exchange e+2 before both its
 // neighbours have finished consuming exchange e (its own hop e+1 waits for their push e+1, which
