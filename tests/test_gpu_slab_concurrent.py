@@ -197,6 +197,46 @@ def test_all_ranks_in_one_cooperative_launch(dims, nranks, mass, mode):
         s.close()
 
 
+@pytest.mark.slow
+@pytest.mark.parametrize("nranks", [4, 8])
+def test_full_size_lattice_split_over_concurrent_ranks_against_the_oracle_record(nranks):
+    """BASELINE configs[3] (28^3 x 96) split along time over 4 and 8 ranks that run CONCURRENTLY in
+    one cooperative launch -- 263 KB faces, thousands of boundary threads waiting on flags, in-kernel
+    reliable updates with fp64 exchanges -- each slab built from its OWN time slices of the links
+    (fieldgen.links_slices: no rank sees the whole field).  The gathered solution against the oracle's
+    stored solve to 1e-12 (tests/golden/refsol_c4_283x96.npz): sampled sites and the whole-field sketch
+    at north_star's 1e-8."""
+    from tests import refsol
+    cfg = fieldgen.CONFIGS["c4_28^3x96"]
+    rec = refsol.load(cfg.name)
+    b = cfg.source()
+    slabs = []
+    for r in range(nranks):
+        t0, t1 = slab.slab_range(cfg.dims, r, nranks)
+        Wl = cfg.links_slices(t0, t1 - t0)
+        Wb = np.ascontiguousarray(cfg.links_slices(t0 - 1, 1)[3])
+        slabs.append(slab.SlabLinks(cfg.dims, Wl, r, nranks, W_back=Wb))
+        del Wl, Wb
+    slab.connect_in_process(slabs)
+    for s in slabs:
+        s.set_wait_limit(WAIT_LIMIT)
+    bs = [stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(b, cfg.dims, r, nranks)), slabs[r].dims, 0)
+          for r in range(nranks)]
+    xs, sts = slab.cg_solve_in_process(slabs, bs, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, fused=True, recon12=True)
+    assert all(st["status"] == stag.OK and st["true_resid"] <= cfg.tol for st in sts), sts
+    for st in sts[1:]:
+        assert (st["iters"], st["true_resid"], st["n_updates"]) == (sts[0]["iters"], sts[0]["true_resid"], sts[0]["n_updates"])
+    x = slab.gather_spinor([stag.spinor_unpack(xs[r], slabs[r].dims, 0) for r in range(nranks)], cfg.dims)
+    sc = refsol.score(x, rec, cfg)
+    print("%d ranks: %d iterations, %d updates, errors vs oracle %r, waits that spun %r"
+          % (nranks, sts[0]["iters"], sts[0]["n_updates"], sc, [s.wait_stats()[0] for s in slabs]))
+    assert sc["l2_sketch"] <= 1e-8 and sc["l2_sites"] <= 1e-8 and sc["max_site"] <= 1e-8 and sc["norm"] <= 1e-8
+    assert sum(s.wait_stats()[0] for s in slabs) > 0
+    assert all(s.status() == stag.OK for s in slabs)
+    for s in slabs:
+        s.close()
+
+
 def test_a_dead_slab_takes_its_neighbours_down_and_reset_revives_them():
     """Rank 0 hops after an exchange rank 1 never joined: its watchdog fires.  From then on rank 0
     publishes nothing, so rank 1 -- whose first exchange still completes, rank 0's push preceded its
