@@ -198,16 +198,16 @@ def test_all_ranks_in_one_cooperative_launch(dims, nranks, mass, mode):
 
 
 @pytest.mark.slow
-@pytest.mark.parametrize("nranks", [4, 8])
-def test_full_size_lattice_split_over_concurrent_ranks_against_the_oracle_record(nranks):
-    """BASELINE configs[3] (28^3 x 96) split along time over 4 and 8 ranks that run CONCURRENTLY in
+@pytest.mark.parametrize("name,nranks", [("c4_28^3x96", 4), ("c4_28^3x96", 8), ("c5_48^3x96", 8)])
+def test_full_size_lattice_split_over_concurrent_ranks_against_the_oracle_record(name, nranks):
+    """BASELINE configs[3] and [4] (28^3 x 96; 48^3 x 96) split along time over ranks that run CONCURRENTLY in
     one cooperative launch -- 263 KB faces, thousands of boundary threads waiting on flags, in-kernel
     reliable updates with fp64 exchanges -- each slab built from its OWN time slices of the links
     (fieldgen.links_slices: no rank sees the whole field).  The gathered solution against the oracle's
-    stored solve to 1e-12 (tests/golden/refsol_c4_283x96.npz): sampled sites and the whole-field sketch
-    at north_star's 1e-8."""
+    stored solve to 1e-12 (tests/golden/refsol_*.npz): sampled sites and the whole-field sketch at
+    north_star's 1e-8."""
     from tests import refsol
-    cfg = fieldgen.CONFIGS["c4_28^3x96"]
+    cfg = fieldgen.CONFIGS[name]
     rec = refsol.load(cfg.name)
     b = cfg.source()
     slabs = []
@@ -228,8 +228,8 @@ def test_full_size_lattice_split_over_concurrent_ranks_against_the_oracle_record
         assert (st["iters"], st["true_resid"], st["n_updates"]) == (sts[0]["iters"], sts[0]["true_resid"], sts[0]["n_updates"])
     x = slab.gather_spinor([stag.spinor_unpack(xs[r], slabs[r].dims, 0) for r in range(nranks)], cfg.dims)
     sc = refsol.score(x, rec, cfg)
-    print("%d ranks: %d iterations, %d updates, errors vs oracle %r, waits that spun %r"
-          % (nranks, sts[0]["iters"], sts[0]["n_updates"], sc, [s.wait_stats()[0] for s in slabs]))
+    print("%s in %d ranks: %d iterations, %d updates, errors vs oracle %r, waits that spun %r"
+          % (name, nranks, sts[0]["iters"], sts[0]["n_updates"], sc, [s.wait_stats()[0] for s in slabs]))
     assert sc["l2_sketch"] <= 1e-8 and sc["l2_sites"] <= 1e-8 and sc["max_site"] <= 1e-8 and sc["norm"] <= 1e-8
     assert sum(s.wait_stats()[0] for s in slabs) > 0
     assert all(s.status() == stag.OK for s in slabs)
