@@ -329,8 +329,10 @@ typedef struct stag_cg_params {
     int    recon8;        /* 1: the iteration's Dslash uses 8-parameter links (overrides recon12) */
     int    persistent;    /* the iteration as ONE persistent cooperative kernel per chunk of passes
                              (grid barriers instead of four kernel boundaries per pass; one
-                             right-hand side, 18- or 12-real links): 1 = yes, -1 = no, 0 = the
-                             library decides by lattice volume         */
+                             right-hand side, 18- or 12-real links; in mode 3 with 18-real fp64
+                             corrections the reliable updates run inside the kernel too, so a
+                             solve is one launch after the initial residual): 1 = yes, -1 = no,
+                             0 = the library decides by lattice volume */
     int    persist_chunk; /* passes per persistent launch between host checks (default 1024) */
 } stag_cg_params_t;
 
