@@ -41,28 +41,38 @@ def _worker(rank, world, port, q):
         os.environ.update({"MASTER_ADDR": "127.0.0.1", "MASTER_PORT": str(port)})
         torch.cuda.set_device(rank)
         dist.init_process_group("nccl", rank=rank, world_size=world)
-        W = fieldgen.links(DIMS, "random", seed=11)
+        W = fieldgen.links(DIMS, "random", seed=11)                # for the oracle; the slab sees only its own slices
         b = fieldgen.spinor_gaussian(DIMS, 0, seed=12)
-        S = slab.SlabLinks(DIMS, W, rank, world)
+        t0, t1 = slab.slab_range(DIMS, rank, world)
+        S = slab.SlabLinks(DIMS, fieldgen.links_slices(DIMS, t0, t1 - t0, "random", seed=11), rank, world,
+                           W_back=np.ascontiguousarray(fieldgen.links_slices(DIMS, t0 - 1, 1, "random", seed=11)[3]))
         S.connect_distributed()
         S.set_wait_limit(1 << 22)
 
         from tests.parity import rel_err as rel      # L2 AND worst-site bound (tests/parity.py)
 
+        # all the CPU work first (the oracle's solve takes a different time on every rank), then a barrier
+        # before every first exchange: rank skew counts against the slab watchdog (include/stag.h)
         ref = slab.scatter_spinor(oracle.dslash(b, W, DIMS, 1), DIMS, rank, world)
+        x_ref, _, _, _, _ = oracle.cg(b, W, DIMS, MASS, 1e-12, 50000)
         for prec, tol in ((0, 1e-13), (3, 2e-6)):
             v = stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(b, DIMS, rank, world)), S.dims, prec)
+            torch.cuda.synchronize()
+            dist.barrier()
             for rep in range(20):                      # back to back, no host synchronisation
                 o = S.dslash(v, 1, prec)
             assert rel(stag.spinor_unpack(o, S.dims, prec), ref) <= tol
-        x_ref, _, _, _, _ = oracle.cg(b, W, DIMS, MASS, 1e-12, 50000)
         out = {}
-        for mode in (stag.CG_F64, stag.CG_RELIABLE):
+        for mode, persistent in ((stag.CG_F64, False), (stag.CG_RELIABLE, False), (stag.CG_F64, True), (stag.CG_RELIABLE, True)):
             bd = stag.spinor_pack(np.ascontiguousarray(slab.scatter_spinor(b, DIMS, rank, world)), S.dims, 0)
-            x, st = S.cg_solve(bd, MASS, TOL, 20000, mode)        # stag_slab_cg_run: graph replays, real waits
+            torch.cuda.synchronize()
+            dist.barrier()
+            # stag_slab_cg_run: graph replays of the kernel-per-step pass, or the persistent kernel with the
+            # reliable updates inside; real waits on the other GPUs either way
+            x, st = S.cg_solve(bd, MASS, TOL, 20000, mode, persistent=persistent)
             assert st["status"] == stag.OK and st["true_resid"] <= TOL, st
             assert rel(stag.spinor_unpack(x, S.dims, 0), slab.scatter_spinor(x_ref, DIMS, rank, world)) <= 1e-8
-            out[mode] = (st["iters"], st["true_resid"], st["n_updates"])
+            out[(mode, persistent)] = (st["iters"], st["true_resid"], st["n_updates"])
         assert S.status() == stag.OK
         torch.cuda.synchronize()
         dist.barrier()
