@@ -208,7 +208,7 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
     if (persist) {
         if (lo) {
             persist_fill<float>(pa32.rk[0], L, w, S.prec_lo, S.m2, w.y32, w.r32, w.d32, w.q32, w.tmp32);
-            if (mode == STAG_CG_RELIABLE && S.prec_hi == STAG_PREC_F64) persist_fill_update(pa32.rk[0].up, L, w, x, b, S.m2);
+            if ((mode == STAG_CG_RELIABLE || mode == STAG_CG_DEFECT) && S.prec_hi == STAG_PREC_F64) persist_fill_update(pa32.rk[0].up, L, w, x, b, S.m2);
             pa32.nlocal = 1; pa32.max_iters = P.persist_chunk;
         } else {
             persist_fill<double>(pa64.rk[0], L, w, S.prec_lo, S.m2, x, w.r64, w.d64, w.q64, w.tmp64);
@@ -329,7 +329,7 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
     for (int k = 0; k < nrhs; ++k) {
         stag_cg_stats_t st = zero;
         st.iters = h->iters[k];
-        st.n_updates = (mode == STAG_CG_DEFECT) ? n_outer : h->n_updates;
+        st.n_updates = (mode == STAG_CG_DEFECT) ? n_outer + h->n_inkernel : h->n_updates;
         st.n_restarts = n_restarts;
         st.iters_f32 = lo ? h->iters[k] : 0;
         st.applies_f64 = S.applies_f64 + h->n_inkernel;

@@ -187,6 +187,27 @@ __device__ __forceinline__ void update_epilogue_local(IterScalars &S, const doub
     S.state = st;
 }
 
+// The scalar step after an outer step of Fig. 2 (mode 2) done in the kernel: residual_epilogue<RES_INIT>
+// restated on IterScalars -- a fresh inner CG from the fp64 residual (beta = 0 makes the next P0 d = r).
+__device__ __forceinline__ void outer_epilogue_local(IterScalars &S, const double dn)
+{
+    S.sum0 = dn;
+    S.have_true = 1;
+    S.n_inkernel += 1;
+    const bool bad = !(dn == dn);
+    if (!bad) {
+        S.delta = dn;
+        S.beta = 0.0;
+        S.maxr = sqrt(dn);
+        S.inner2 = fmax(S.eps_in * S.eps_in * dn, S.tol2b);               // Fig. 2, Q8
+        S.active = dn > S.tol2b;
+    }
+    int st = S.active ? CG_RUN : CG_CONVERGED;
+    if (bad) st = CG_BREAKDOWN;
+    else if (S.active && S.iter >= S.maxiter) st = CG_MAXITER;
+    S.state = st;
+}
+
 template <typename T, int NR, bool SLAB, bool LRES>
 __global__ void __launch_bounds__(PERSIST_THREADS, PersistTune<T, NR>::BPS)
 cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
@@ -401,9 +422,11 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
         __syncthreads();
 
         // ---- S6 in the kernel: x += y, y = 0 (group-wise); r = b - A x in fp64, its fp32 copy and
-        // |r|^2 (reliable); beta from the corrected residual with d kept (eq. 3.1, Q10) --------------
+        // |r|^2 (reliable); beta from the corrected residual with d kept (eq. 3.1, Q10).  The same
+        // three phases serve the outer step of Fig. 2 (mode 2), which restarts from d = r ---------
         if constexpr (sizeof(T) == 4) {
-            if (S.state == CG_UPDATE && R.up.links_even != nullptr) {
+            const bool outer = S.mode == STAG_CG_DEFECT && S.state == CG_CONVERGED;      // Fig. 2: the inner CG met its target
+            if ((S.state == CG_UPDATE || outer) && R.up.links_even != nullptr) {
                 const IterUpdate &U = R.up;
                 using D2 = double2;
                 D2 *x_c = reinterpret_cast<D2 *>(U.x), *t_c = reinterpret_cast<D2 *>(U.tmp);
@@ -482,7 +505,10 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
                 if constexpr (SLAB) { if (slab_dead(R.xch)) return; }
                 double rn2;
                 if (!total_over_ranks(partA, &rn2)) return;
-                if (threadIdx.x == 0) update_epilogue_local(S, rn2);
+                if (threadIdx.x == 0) {
+                    if (outer) outer_epilogue_local(S, rn2);
+                    else update_epilogue_local(S, rn2);
+                }
                 __syncthreads();
             }
         }
@@ -490,7 +516,7 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
 
     if (lb == 0 && threadIdx.x == 0) {
         CgCtrl *c = R.ctrl;
-        c->delta[0] = S.delta; c->beta[0] = S.beta; c->maxr[0] = S.maxr;
+        c->delta[0] = S.delta; c->beta[0] = S.beta; c->maxr[0] = S.maxr; c->inner2[0] = S.inner2;
         c->dAd[0] = S.dAd; c->alpha[0] = S.alpha; c->sum1[0] = S.sum1;
         c->iter = S.iter; c->iters[0] = S.iters; c->active[0] = S.active;
         c->sum0[0] = S.sum0; c->n_updates = S.n_updates; c->have_true = S.have_true; c->n_inkernel = S.n_inkernel;

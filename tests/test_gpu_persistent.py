@@ -114,6 +114,12 @@ def test_mixed_solve_is_one_launch_with_the_reliable_updates_inside_the_kernel()
     xs = stag.spinor_unpack(x, dims, 0)
     assert rel_err(xs, x_ref) <= 1e-8
     assert _true_resid(xs, b, W, dims, mass) <= tol * (1 + 1e-3)
+    # Fig. 2's outer steps (mode 2) run inside the kernel the same way
+    stag.reset_launch_count()
+    xd, std = stag.cg_solve(bd, L, mass, tol, 20000, stag.CG_DEFECT, recon12=True, persistent=True, persist_chunk=100000)
+    assert stag.launch_count() <= 6 and std["status"] == stag.OK and std["n_updates"] >= 2
+    assert std["applies_f64"] == std["n_updates"] + 1
+    assert rel_err(stag.spinor_unpack(xd, dims, 0), x_ref) <= 1e-8
     # with 12-real fp64 corrections the update stays on the host: more launches, same solution within the bars
     stag.reset_launch_count()
     x2, st2 = stag.cg_solve(bd, L, mass, tol, 20000, stag.CG_RELIABLE, recon12=True, recon12_f64=True, persistent=True)
