@@ -203,6 +203,43 @@ int stag_dslash(void *out, const void *in, const stag_links_t *links, int parity
 int stag_apply_A(void *out_even, const void *in_even, const stag_links_t *links, double mass,
                  int prec);
 
+/* The same operator for callers that cannot allocate device memory.
+ *
+ * stag_apply_A needs somewhere to keep D_oe in_even between its two hops: the workspace, which
+ * either you own (stag_set_workspace) or the handle cudaMallocs on first use.  That rules it out
+ * for a program that gave all device memory to its own pool at start-up (a cudaMalloc from inside
+ * a library then fails), for code running where cudaMalloc / cudaFree are banned because they
+ * stall every stream on the device, and for a caller that holds nothing but the spinors it was
+ * handed and cannot keep a workspace of ours alive.  This entry point is for them: the
+ * intermediate lives in an array that is part of the library image, STAG_NOALLOC_SCRATCH_BYTES
+ * (8 MiB) of it on every device that loads libstag.so, held until the process exits whether or
+ * not this function is ever called.  The call itself issues two kernel launches and nothing
+ * else: no cudaMalloc, no cudaFree, no workspace, no library routine that allocates.
+ *
+ * Arguments, layouts, result (eq. 2.3: out_even = mass^2 in_even - D_eo D_oe in_even, bit for bit
+ * what stag_apply_A writes) and stream as stag_apply_A with one right-hand side; you still
+ * supply in_even and out_even (device, device layout of `prec`, not aliased).  Limits:
+ *   - size: 3 * Vh_pad complex numbers of `prec` must fit the array, i.e. Vh_pad <= 174 762
+ *     sites per parity in fp64 (16^3 x 32, 16^3 x 64 fit; 28^3 x 96 does not) and <= 349 525 in
+ *     fp32.  A larger lattice gets STAG_EINVAL and stag_strerror names both sizes; nothing is
+ *     launched.
+ *   - links: the gathered links of `prec` must exist already, because building them allocates.
+ *     STAG_PREC_F64 always exists; any other form is built by the first stag_dslash /
+ *     stag_apply_A / solve that uses it, so make one such call during set-up.  Otherwise
+ *     STAG_EINVAL (the text says so).
+ *   - first call on each device: looks up the array's device address (cudaGetSymbolAddress,
+ *     with that device current) and remembers it.  It is host-side bookkeeping that may load the
+ *     library's device code; make that first call during set-up, before any stream capture is
+ *     begun.
+ *   - sharing: there is ONE array per device and every call uses it.  Calls issued on one
+ *     stream are ordered and safe.  Two calls that can overlap on the GPU (different streams,
+ *     or different host threads on different streams) race on it and both results are garbage;
+ *     the library does not detect this.  The array keeps whatever the last call left in it;
+ *     no call depends on that, since the first hop overwrites every element the second reads. */
+#define STAG_NOALLOC_SCRATCH_BYTES (8u << 20)
+int stag_apply_A_noalloc(void *out_even, const void *in_even, const stag_links_t *links, double mass,
+                         int prec);
+
 /* ---- several right-hand sides sharing one pass over the links ------------------------
  *
  * The hop is bandwidth-bound on the gauge field, and the production use of the

@@ -108,6 +108,7 @@ SIGNATURES = {
     "stag_spinor_unpack": (ctypes.c_int, [_vp, _vp, _ip, ctypes.c_int]),
     "stag_dslash": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, _ip, ctypes.c_int]),
     "stag_apply_A": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_int]),
+    "stag_apply_A_noalloc": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_int]),
     "stag_cg_solve": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                      ctypes.c_int, _ip, _dp]),
     "stag_cg_solve_ex": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
@@ -349,6 +350,23 @@ def apply_A(v_even, links: Links, mass: float, prec, out=None):
         out = empty_spinor(links.dims, prec)
     _check(lib().stag_apply_A(ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(v_even.data_ptr()),
                               links.handle, float(mass), int(prec)))
+    return out
+
+
+NOALLOC_SCRATCH_BYTES = 8 << 20
+
+
+def apply_A_noalloc(v_even, out, links: Links, mass: float, prec):
+    """stag_apply_A_noalloc: out = mass^2 v_even - D_eo D_oe v_even written into the spinor `out`
+    YOU pass (this wrapper creates no tensor), with the odd-site intermediate in the library's
+    built-in 8 MiB device array instead of a workspace.  For callers that may not allocate device
+    memory (all of it belongs to their own pool, or cudaMalloc is banned where they run).
+    Raises StagError(EINVAL) when the lattice is too large for the array or the links of `prec`
+    have not been built by an earlier ordinary call.  Calls on different streams must not overlap:
+    they share the one array."""
+    use_current_stream()
+    _check(lib().stag_apply_A_noalloc(ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(v_even.data_ptr()),
+                                      links.handle, float(mass), int(prec)))
     return out
 
 

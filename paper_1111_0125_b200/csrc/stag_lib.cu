@@ -204,9 +204,10 @@ struct stag_links {
     stag_links() { for (auto &r : L_ready) r.store(0, std::memory_order_relaxed); }
 };
 
-// The rest of the translation unit, in five sections (they see everything above):
+// The rest of the translation unit, in six sections (they see everything above):
 #include "stag_host_ws.cuh"      // the CG workspace: layout, lease; C ABI: stag_cg_workspace_bytes, stag_set_workspace
 #include "stag_host_links.cuh"   // S0 kernels, hop launchers; C ABI: state, links, spinors, operator
 #include "stag_host_persist.cuh" // launching the persistent iteration kernel (stag_persist.cuh)
 #include "stag_host_cg.cuh"      // one-GPU CG drivers; C ABI: stag_cg_solve*, stag_solve_M
 #include "stag_host_slab.cuh"    // T-slabs: wiring, push / hop, CG over slabs; C ABI: stag_slab_*
+#include "stag_host_noalloc.cuh" // A with its intermediate in a static device array; C ABI: stag_apply_A_noalloc
