@@ -673,7 +673,7 @@ def run_slabs(args):
         "cg": {"iters": st["iters"], "n_updates": st["n_updates"], "true_resid": st["true_resid"],
                "time_to_solution_s": st["seconds"], "ms_per_iteration": st["seconds"] / max(1, st["iters"]) * 1e3,
                "iteration_path": "chosen by volume (params.persistent = 0): %s" % (
-                   "persistent kernel, one cooperative launch per <= 1024 passes" if cfg.vh // world <= 800000
+                   "persistent kernel, one cooperative launch per <= 1024 passes" if world == 1 and cfg.vh <= 800000
                    else "kernel per step, CUDA graph of 32 passes"),
                "persistent_kernel": pers_path, "kernel_per_step": step_path},
     }

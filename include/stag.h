@@ -369,7 +369,9 @@ typedef struct stag_cg_params {
                              right-hand side, 18- or 12-real links; in mode 3 with 18-real fp64
                              corrections the reliable updates run inside the kernel too, so a
                              solve is one launch after the initial residual): 1 = yes, -1 = no,
-                             0 = the library decides by lattice volume */
+                             0 = the library decides by lattice volume;
+                             for a lattice split over more than one T-slab 0 means "no": across
+                             GPUs this kernel is opt-in until it has been run and timed there  */
     int    persist_chunk; /* passes per persistent launch between host checks (default 1024) */
 } stag_cg_params_t;
 
@@ -467,8 +469,8 @@ int stag_slab_cg_finish(stag_links_t *slab, stag_cg_stats_t *stats_out);
 /* One STAG_SLAB_ACT_ITER (up to persist_chunk passes of the loop) of the n slabs given, in ONE
  * cooperative launch of the persistent iteration kernel: each slab's blocks form a rank group with
  * its own barrier, and the groups talk only through the exchange regions.  n = 1: what a process of
- * a one-process-per-GPU run launches for its own slab (stag_slab_cg_run does, with
- * params->persistent = 1).  n = nranks with all slabs on the calling thread's device: the
+ * a one-process-per-GPU run launches for its own slab (stag_slab_cg_run does when
+ * params->persistent = 1, or when it is 0 and the slab is the whole lattice, nranks = 1).  n = nranks with all slabs on the calling thread's device: the
  * single-GPU emulation of the multi-GPU run -- the ranks' kernels run concurrently and really wait
  * for each other, which separate launches on one device cannot promise.  Replaces the phases of
  * that action in the stepped loop; every slab must have been told STAG_SLAB_ACT_ITER by

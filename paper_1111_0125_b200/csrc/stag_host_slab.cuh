@@ -428,8 +428,13 @@ extern "C" int stag_slab_cg_begin(stag_links_t *L, void *x_even, const void *b_e
     h->eps_in = C->P.eps_in;
     h->nrhs = 1;
     CU(cudaMemcpyAsync(C->w.ctrl, h, sizeof(CgCtrl), cudaMemcpyHostToDevice, t_stream));
+    // persistent = 0 (the library decides) takes the persistent kernel only for a lattice held by ONE
+    // slab.  Across several GPUs its peer stores, system-scope flags and replicated scalars have never
+    // executed on hardware and its volume threshold was measured with all ranks on one device (same
+    // L2, no NVLink): until tests/test_gpu_slab_multi.py and a timing have run on >= 2 GPUs it is
+    // opt-in there (persistent = 1) and the default is the kernel-per-step graph.
     C->persist = persist_prec_ok(C->prec_lo) &&
-                 (C->P.persistent > 0 || (C->P.persistent == 0 && persist_by_volume(L->g, true)));
+                 (C->P.persistent > 0 || (C->P.persistent == 0 && L->nranks == 1 && persist_by_volume(L->g, true)));
     CU(cudaEventRecord(L->own.ev0, t_stream));
     C->stage = 0;
     return STAG_OK;

@@ -123,10 +123,12 @@ def test_hops_back_to_back_from_one_thread_per_slab(dims, nranks):
 
 @pytest.mark.parametrize("dims,nranks,mass", [((4, 4, 4, 8), 2, 0.1), ((4, 4, 4, 16), 4, 0.1), ((8, 8, 8, 16), 2, 0.05)])
 @pytest.mark.parametrize("mode", [stag.CG_F64, stag.CG_RELIABLE])
-def test_slab_cg_run_from_one_thread_per_slab(dims, nranks, mass, mode):
+@pytest.mark.parametrize("persistent", [None, True])
+def test_slab_cg_run_from_one_thread_per_slab(dims, nranks, mass, mode, persistent):
     """stag_slab_cg_run -- the call of a one-process-per-GPU run: CUDA-graph replays of whole chunks of
-    iterations, the in-kernel pushes of hop 1 and of the direction update, global sums through the
-    exchange regions -- issued concurrently by every rank's own thread.  Solution against the oracle's
+    iterations (persistent=None: with more than one rank the library's own choice), or the persistent
+    kernel (opt-in across ranks), the in-kernel pushes of hop 1 and of the direction update, global sums
+    through the exchange regions -- issued concurrently by every rank's own thread.  Solution against the oracle's
     solve (1e-8), true residual with the oracle's A, identical scalars on every rank."""
     tol = 1e-10
     W = fieldgen.links(dims, "random", seed=73)
@@ -141,7 +143,7 @@ def test_slab_cg_run_from_one_thread_per_slab(dims, nranks, mass, mode):
 
     def body(r):
         time.sleep(0.02 * r)                     # rank skew: the first global sum is certain to wait for the last rank
-        return slabs[r].cg_solve(bs[r], mass, tol, 20000, mode, recon12=True, chunk=8)
+        return slabs[r].cg_solve(bs[r], mass, tol, 20000, mode, recon12=True, chunk=8, persistent=persistent)
 
     res = run_ranks(nranks, body)
     sts = [st for _, st in res]
