@@ -369,10 +369,13 @@ typedef struct stag_cg_params {
                              right-hand side, 18- or 12-real links; in mode 3 with 18-real fp64
                              corrections the reliable updates run inside the kernel too, so a
                              solve is one launch after the initial residual): 1 = yes, -1 = no,
-                             0 = the library decides by lattice volume;
+                             0 = the library decides by lattice volume
+                             and falls back to the kernel-per-step path if the device refuses
+                             the cooperative launch (1 reports that as STAG_ECUDA instead);
                              for a lattice split over more than one T-slab 0 means "no": across
                              GPUs this kernel is opt-in until it has been run and timed there  */
-    int    persist_chunk; /* passes per persistent launch between host checks (default 1024) */
+    int    persist_chunk; /* passes per persistent launch between host checks (default 1024;
+                             values above 65536 are taken as 65536)                            */
 } stag_cg_params_t;
 
 typedef struct stag_cg_stats {

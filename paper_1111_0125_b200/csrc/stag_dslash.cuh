@@ -212,8 +212,11 @@ __device__ __forceinline__ bool slab_dead(const char *xch)
 // false inside the persistent kernel, where another phase of the same launch wrote it.
 // LRES: the gauge field is small enough to stay in L2 next to the vectors (persistent kernel on
 // small lattices): its packets are then loaded with the keep policy instead of streamed through.
+// Returns false when a halo wait of this site gave up (HALO only; the slab is then marked dead): acc
+// was computed from a halo that never arrived, and the caller must not store it into a peer's buffers
+// (wait_flag's contract: a timed-out slab publishes nothing).  Always true otherwise.
 template <typename T, int NR, bool HALO, bool NC = true, bool LRES = false, typename EpochFn>
-__device__ __forceinline__ void hop_site(cplx_t<T> (&acc)[3], const cplx_t<T> *__restrict__ in,
+__device__ __forceinline__ bool hop_site(cplx_t<T> (&acc)[3], const cplx_t<T> *__restrict__ in,
                                          const pkt_t<T> *__restrict__ links, const Geom &g, const int cb,
                                          const Site &s, const unsigned neg, char *xch, EpochFn epoch)
 {
@@ -234,19 +237,20 @@ __device__ __forceinline__ void hop_site(cplx_t<T> (&acc)[3], const cplx_t<T> *_
             if constexpr (NC) v1[d][c] = ld_keep_nc(in + (size_t)c * g.Vh_pad + s.nbr[d]);
             else v1[d][c] = ld_keep(in + (size_t)c * g.Vh_pad + s.nbr[d]);
         }
+    bool fresh = true;
     if constexpr (HALO) {
         XchHeader *hdr = (XchHeader *)xch;
         if (s.x3 == g.X3 - 1) {
             const unsigned long long e = epoch();
             const C *fwd = (const C *)(xch + xch_halo_offset(g.s3, e, 1));
-            wait_flag(&hdr->flag_fwd, e, hdr);
+            fresh = wait_flag(&hdr->flag_fwd, e, hdr);
 #pragma unroll
             for (int c = 0; c < 3; ++c) v1[3][c] = __ldcg(fwd + (size_t)c * g.s3 + s.nbr[3]);
         }
         if (s.x3 == 0) {
             const unsigned long long e = epoch();
             const C *back = (const C *)(xch + xch_halo_offset(g.s3, e, 0));
-            wait_flag(&hdr->flag_back, e, hdr);
+            fresh = wait_flag(&hdr->flag_back, e, hdr) && fresh;
 #pragma unroll
             for (int c = 0; c < 3; ++c)
                 v1[7][c] = __ldcg(back + (size_t)c * g.s3 + (s.nbr[7] - (g.X3 - 1) * g.s3));
@@ -276,6 +280,7 @@ __device__ __forceinline__ void hop_site(cplx_t<T> (&acc)[3], const cplx_t<T> *_
                 for (int j = 0; j < 3; ++j) cfma(acc[i], m[3 * i + j], v1[d][j]);
         }
     }
+    return fresh;
 }
 
 // T: float or double.  NR: storage of each link (3 = 18-real, 2 = 12-real rows 0,1, 1 = 8-parameter).
@@ -348,8 +353,9 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
         if (NR != 3) neg = det_sign_mask(g, s);
 
         C acc[N][3];
+        bool fresh = true;      // false: a halo wait of this site timed out, its result is not pushed to a peer
         if constexpr (N == 1) {
-            hop_site<T, NR, HALO, true>(acc[0], in, links, g, cb, s, neg, halo.xch,
+            fresh = hop_site<T, NR, HALO, true>(acc[0], in, links, g, cb, s, neg, halo.xch,
                                   [&]() { return __ldcg(&((const XchHeader *)halo.xch)->epoch); });
         } else {
             // several right-hand sides: the neighbours of one group of directions at a time (register budget)
@@ -450,7 +456,7 @@ dslash_kernel(cplx_t<T> *__restrict__ out, const cplx_t<T> *__restrict__ in,
 #pragma unroll
                 for (int c = 0; c < 3; ++c) st_keep(out + k * rs + (size_t)c * g.Vh_pad + cb, acc[k][c]);
                 if constexpr (HALO) {
-                    if (pushing && cb < g.Vh && (s.x3 == 0 || s.x3 == g.X3 - 1)) {
+                    if (pushing && fresh && cb < g.Vh && (s.x3 == 0 || s.x3 == g.X3 - 1)) {
                         // first slice -> the backward neighbour's "fwd" halo, last slice -> the
                         // forward neighbour's "back" halo, buffers of exchange e_in + 1.  Only the
                         // boundary threads read the count, and only their blocks take the ticket

@@ -116,6 +116,7 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
     if (!(P.eps_in > 0.0)) P.eps_in = (mode == STAG_CG_DEFECT) ? 1e-2 : 0.1;
     if (P.graph_chunk == 0) P.graph_chunk = 32;
     if (P.persist_chunk <= 0) P.persist_chunk = 1024;
+    if (P.persist_chunk > PERSIST_MAX_CHUNK) P.persist_chunk = PERSIST_MAX_CHUNK;
 
     Solver S;
     S.L = L;
@@ -201,8 +202,8 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
     // workspace: everything else the nodes bake in (vector addresses, control block) is a
     // function of the workspace's base address and those.
     // Or, for one right-hand side, as one persistent kernel per chunk (stag_persist.cuh).
-    const bool persist = nrhs == 1 && persist_prec_ok(S.prec_lo) &&
-                         (P.persistent > 0 || (P.persistent == 0 && persist_by_volume(L->g, false)));
+    bool persist = nrhs == 1 && persist_prec_ok(S.prec_lo) &&
+                   (P.persistent > 0 || (P.persistent == 0 && persist_by_volume(L->g, false)));
     IterArgs<float> pa32;
     IterArgs<double> pa64;
     if (persist) {
@@ -218,7 +219,9 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
     const int chunk = P.graph_chunk;
     cudaGraphExec_t gexec = nullptr;
     unsigned long long graph_nodes = 0;
-    if (chunk > 0 && !persist) {
+    // (a lambda: the persistent path needs the graph only if its launch is refused, see the loop)
+    auto acquire_graph = [&]() -> int {
+        if (chunk <= 0 || gexec) return STAG_OK;
         const void *xkey = (mode == STAG_CG_F64) ? (const void *)x : nullptr;
         GraphSlot *slot = nullptr, *victim = &ws->graphs[0];
         for (GraphSlot &gs : ws->graphs) {
@@ -249,13 +252,16 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
         slot->stamp = ++ws->stamp;
         gexec = slot->exec;
         graph_nodes = slot->nodes;
-    }
+        return STAG_OK;
+    };
+    if (!persist && (rc = acquire_graph())) return rc;
 
     int n_restarts = 0, n_outer = 0;
     int final_state = CG_RUN;
     bool have_true = true;      // ctrl->sum0[k] holds |b_k - A x_k|^2 for the current x
     bool verifying = false;     // mode 0: the last launch was the true-residual check of Q6b
     bool persist_ran = false;   // the last thing launched was the persistent kernel: it says whether sum0 is current
+    bool persist_any = false;   // a persistent launch has been accepted in this solve
     for (;;) {
         if ((rc = S.read_ctrl())) return rc;
         const int state = h->state;
@@ -264,10 +270,22 @@ int cg_solve_device(double *x, const double *b, const stag_links *L, WsHost *ws,
             if (verifying) ++n_restarts;
             verifying = false;
             if (persist) {
-                if ((rc = lo ? persist_launch<float>(pa32, S.prec_lo, false, s) : persist_launch<double>(pa64, S.prec_lo, false, s))) return rc;
-                persist_ran = true;
-                continue;
-            } else if (gexec) {
+                rc = lo ? persist_launch<float>(pa32, S.prec_lo, false, s) : persist_launch<double>(pa64, S.prec_lo, false, s);
+                if (rc == STAG_OK) {
+                    persist_ran = persist_any = true;
+                    continue;
+                }
+                // The library chose this path itself (persistent = 0) and the device refuses the
+                // cooperative launch (an MPS thread limit, MIG, a green context, no cooperative
+                // launch at all) before any pass has run: nothing was changed, so take the
+                // kernel-per-step path these lattices ran on before.  An explicit persistent = 1
+                // keeps the hard error.
+                if (P.persistent != 0 || persist_any) return rc;
+                (void)cudaGetLastError();
+                persist = false;
+                if ((rc = acquire_graph())) return rc;
+            }
+            if (gexec) {
                 CU(cudaGraphLaunch(gexec, s));
                 count_launch(graph_nodes);
             } else {

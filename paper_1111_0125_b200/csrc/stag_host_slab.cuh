@@ -390,6 +390,7 @@ extern "C" int stag_slab_cg_begin(stag_links_t *L, void *x_even, const void *b_e
     if (!(C->P.eps_in > 0.0)) C->P.eps_in = 0.1;
     if (C->P.graph_chunk <= 0) C->P.graph_chunk = 32;    // iterations between host checks (plain launches)
     if (C->P.persist_chunk <= 0) C->P.persist_chunk = 1024;
+    if (C->P.persist_chunk > PERSIST_MAX_CHUNK) C->P.persist_chunk = PERSIST_MAX_CHUNK;
     C->x = (double *)x_even;
     C->b = (const double *)b_even;
     C->mass = mass;

@@ -328,11 +328,11 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
             unsigned neg = 0;
             if (NR != 3) neg = det_sign_mask(g, s);
             C acc[3];
-            hop_site<T, NR, SLAB, false, LRES>(acc, d_c, R.links_odd, g, cb, s, neg, R.xch, [=]() { return epoch; });
+            const bool fresh = hop_site<T, NR, SLAB, false, LRES>(acc, d_c, R.links_odd, g, cb, s, neg, R.xch, [=]() { return epoch; });
 #pragma unroll
             for (int c = 0; c < 3; ++c) st_keep(tmp_c + (size_t)c * g.Vh_pad + cb, acc[c]);
             if constexpr (SLAB) {
-                if (cb < g.Vh && (s.x3 == 0 || s.x3 == g.X3 - 1)) {
+                if (fresh && cb < g.Vh && (s.x3 == 0 || s.x3 == g.X3 - 1)) {      // a timed-out wait publishes nothing
                     C *dst = (s.x3 == 0)
                         ? (C *)(R.peer_bwd + xch_halo_offset(g.s3, epoch + 1, 1)) + cb
                         : (C *)(R.peer_fwd + xch_halo_offset(g.s3, epoch + 1, 0)) + (cb - (g.Vh - g.s3));
@@ -461,11 +461,11 @@ cg_iter_persistent_kernel(const __grid_constant__ IterArgs<T> A)
                     Site s;
                     decode_site(g, 1, cb < g.Vh ? cb : 0, s);
                     D2 acc[3];
-                    hop_site<double, 3, SLAB, false, false>(acc, x_c, U.links_odd, g, cb, s, 0u, R.xch, [=]() { return epoch; });
+                    const bool fresh = hop_site<double, 3, SLAB, false, false>(acc, x_c, U.links_odd, g, cb, s, 0u, R.xch, [=]() { return epoch; });
 #pragma unroll
                     for (int c = 0; c < 3; ++c) t_c[(size_t)c * g.Vh_pad + cb] = acc[c];
                     if constexpr (SLAB) {
-                        if (cb < g.Vh && (s.x3 == 0 || s.x3 == g.X3 - 1)) {
+                        if (fresh && cb < g.Vh && (s.x3 == 0 || s.x3 == g.X3 - 1)) {
                             D2 *dst = (s.x3 == 0)
                                 ? (D2 *)(R.peer_bwd + xch_halo_offset(g.s3, epoch + 1, 1)) + cb
                                 : (D2 *)(R.peer_fwd + xch_halo_offset(g.s3, epoch + 1, 0)) + (cb - (g.Vh - g.s3));

@@ -278,6 +278,13 @@ def test_a_dead_slab_takes_its_neighbours_down_and_reset_revives_them():
         s.close()
 
 
+class _RawDeviceBytes:
+    """n bytes of device memory at ptr, for torch.as_tensor (CUDA array interface)."""
+
+    def __init__(self, ptr, n):
+        self.__cuda_array_interface__ = {"shape": (int(n),), "typestr": "|u1", "data": (int(ptr), False), "version": 2}
+
+
 def test_persistent_kernel_of_one_rank_alone_times_out_instead_of_hanging():
     """Every wait inside the persistent kernel is bounded by the slab's watchdog: with two ranks
     connected but only rank 0's iterations launched (stag_slab_cg_iter_all on one slab), rank 0's
@@ -311,10 +318,23 @@ def test_persistent_kernel_of_one_rank_alone_times_out_instead_of_hanging():
             ph += 1
     assert stag.lib().stag_slab_cg_iter_all(two, 2) == stag.EINVAL          # the same slab twice
     assert stag.lib().stag_slab_cg_iter_all(one, 0) == stag.EINVAL
+    # rank 1's halo buffers before: [epoch parity][direction], 3 colours x s3 sites x 16 bytes each (stag_common.cuh)
+    ptr, nbytes = slabs[1].exchange_region()
+    s3 = dims[0] * dims[1] * dims[2] // 2
+    halo = 4 * 3 * s3 * 16
+    region = torch.as_tensor(_RawDeviceBytes(ptr, nbytes), device="cuda")
+    torch.cuda.synchronize()
+    before = region[nbytes - halo:].clone().cpu().numpy().reshape(2, -1)
     assert stag.lib().stag_slab_cg_iter_all(one, 1) == stag.OK              # rank 0 alone: nobody answers
     with pytest.raises(stag.StagError) as e:
         slabs[0].cg_control()
     assert e.value.status == stag.ETIMEOUT
     assert slabs[0].status() == stag.ETIMEOUT and slabs[1].status() == stag.OK
+    # "A timed-out slab publishes nothing": the faces of d that rank 0 pushed BEFORE it waited (phase P0,
+    # next exchange) are in one parity's buffers; the other parity's would have received the hop results
+    # of the boundary threads whose wait gave up, computed from a halo that never came -- untouched.
+    after = region[nbytes - halo:].clone().cpu().numpy().reshape(2, -1)
+    changed = [bool((before[k] != after[k]).any()) for k in range(2)]
+    assert changed.count(True) == 1, changed
     for s in slabs:
         s.close()
