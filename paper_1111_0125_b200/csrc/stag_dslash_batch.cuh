@@ -27,53 +27,13 @@ namespace stag {
 // Sweep on 28^3 x 96, 12-real links, us per hop for N = 2 / 3 / 4 (profiles/README.md, round 2):
 //   LD 1: 80.0 / 94.5 / 103.6    LD 2: 80.2 / 94.3 / 102.7    LD 3: 80.4 / 90.4 / 104.3
 //   3 blocks per SM (LD 2): 80.2 / 98.7 / 110.9               5 blocks per SM (LD 1): 78.1 / 94.4 / 112.8
-#ifndef STAG_BATCH_LD
-#define STAG_BATCH_LD 0      // 0: per-N default below
-#endif
-// Experiments kept compilable (all measured SLOWER, profiles/README.md round 2; defaults are off):
-// STAG_BATCH_PF  pull link tiles towards L2 ahead of the demand loads, holding no register:
-//                1 = prefetch.global.L2 of the warp's own tile, 2 = own tile in the first wave plus the
-//                tile one wave of resident blocks ahead, 3 / 4 = the same as 2 / 1 with one
-//                cp.async.bulk.prefetch.L2 per warp marked evict-first.  N = 4, 12-real: 102.7 us without,
-//                110.1 / 118.4 / 116.6 / 108.5 us with.
-// STAG_BATCH_EXP diagnostics that break the result on purpose: 1 = no stores (94.2 us), 2 = every
-//                gather at the thread's own site (94.5 us), 3 = constant links, i.e. no link traffic
-//                at all (62.0 us: the arithmetic and the spinor traffic alone take as long as streaming
-//                the 405 MB of links does).
-#ifndef STAG_BATCH_PF
-#define STAG_BATCH_PF 0
-#endif
-__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
-// one thread: bring [p, p + bytes) towards L2, marked evict-first (bytes a multiple of 16)
-__device__ __forceinline__ void prefetch_l2_bulk_stream(const void *p, unsigned bytes)
-{
-    asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;"
-                 :: "l"(p), "r"(bytes), "l"(policy_evict_first()) : "memory");
-}
-#ifndef STAG_BATCH_EXP
-#define STAG_BATCH_EXP 0
-#endif
-#ifndef STAG_BATCH_MINB
-#define STAG_BATCH_MINB 4
-#endif
-// STAG_BATCH_FFMA2 = 1: the two right-hand sides of a pair go through the packed fp32 FMA of sm_100
-// (fma.rn.f32x2, __ffma2_rn: two IEEE fmas per instruction).  The accumulators of a pair are held as
-// X_i = (Re acc_a, Re acc_b), Y_i = (Im acc_a, Im acc_b), the gathered float4 is split into
-// VX = (Re v_a, Re v_b), VY = (Im v_a, Im v_b), and one complex multiply-add of BOTH right-hand sides is
-//   X = fma2((m.x, m.x), VX, X);  X = fma2((-m.y, -m.y), VY, X);  Y = fma2((m.x, m.x), VY, Y);  Y = fma2((m.y, m.y), VX, Y)
-// -- per component the same four fmas in the same order as cfma, so the result is bit-identical.
-// Four packed instructions instead of eight scalar ones on the FMA pipe, paid for with the moves that
-// build the duplicated matrix entries: SASS of N = 4, 12-real has 576 FFMA2 + 823 MOV where the scalar
-// form has 1248 FFMA (the duplicates are rebuilt per pair: 128 registers do not hold 27 of them across
-// the pairs).  Measured on 28^3 x 96: x2 84.5 us against 80.4, x3 101.6 against 89.7, x4 122.8 against
-// 100.7 -- the hop is bound by issue slots, not by the FMA pipe (47 % busy), and the moves cost more
-// slots than the packing saves.  Off.
-#ifndef STAG_BATCH_FFMA2
-#define STAG_BATCH_FFMA2 0
-#endif
+// Measured slower and no longer in the tree (numbers in profiles/README.md, round 2): prefetching link
+// tiles towards L2 ahead of the demand loads (prefetch.global.L2 or cp.async.bulk.prefetch.L2), the
+// packed fp32 FMA (fma.rn.f32x2) for the two right-hand sides of a pair, and a shared-memory ring of
+// link half-tiles filled by cp.async.bulk.
 template <int NR, int N> struct BatchTune {
-    static constexpr int MINB = STAG_BATCH_MINB;
-    static constexpr int LD = (NR == 3) ? 1 : (STAG_BATCH_LD ? STAG_BATCH_LD : (N == 3 ? 3 : 2));
+    static constexpr int MINB = 4;
+    static constexpr int LD = (NR == 3) ? 1 : (N == 3 ? 3 : 2);
 };
 
 // NR, MODE, N, PAIRED as in dslash_kernel; float only; no halo.
@@ -82,7 +42,7 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, BatchTune<NR, N>::MINB)
 dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
                     const float4 *__restrict__ links, const Geom g, const int p, const float a, const float cD,
                     const float2 *__restrict__ own, double *__restrict__ partials,
-                    const CgCtrl *__restrict__ ctrl, const int pf_ahead)
+                    const CgCtrl *__restrict__ ctrl)
 {
     static_assert(N >= 2 && N <= 4, "batch hop: 2..4 right-hand sides per pass");
     using C = float2;
@@ -101,45 +61,13 @@ dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
     for (int k = 0; k < N; ++k) dot[k] = 0.0;
 
     if (cb < g.Vh_pad) {
-#if STAG_BATCH_PF > 0
-        {   // pull the warp's link tile(s) towards L2 without holding a register: one 128-byte line per lane and trip
-            constexpr int TILE_BYTES = PPS * TILE * 16;
-            const int lane = threadIdx.x & 31;
-#if STAG_BATCH_PF == 3
-            const int tile = cb >> 5, ntiles = g.Vh_pad >> 5;
-            if (lane == 0) {
-                if (tile < pf_ahead) prefetch_l2_bulk_stream(links + (size_t)tile * (size_t)(PPS * TILE), TILE_BYTES);
-                if (tile + pf_ahead < ntiles) prefetch_l2_bulk_stream(links + (size_t)(tile + pf_ahead) * (size_t)(PPS * TILE), TILE_BYTES);
-            }
-#elif STAG_BATCH_PF == 4
-            if (lane == 0) prefetch_l2_bulk_stream(links + (size_t)(cb >> 5) * (size_t)(PPS * TILE), TILE_BYTES);
-#elif STAG_BATCH_PF == 1
-            const char *t0 = (const char *)(links + (size_t)(cb >> 5) * (size_t)(PPS * TILE));
-            for (int off = lane * 128; off < TILE_BYTES; off += 32 * 128) prefetch_l2(t0 + off);
-#else
-            const int tile = cb >> 5, ntiles = g.Vh_pad >> 5;
-            if (tile < pf_ahead) {
-                const char *t0 = (const char *)(links + (size_t)tile * (size_t)(PPS * TILE));
-                for (int off = lane * 128; off < TILE_BYTES; off += 32 * 128) prefetch_l2(t0 + off);
-            }
-            if (tile + pf_ahead < ntiles) {
-                const char *t1 = (const char *)(links + (size_t)(tile + pf_ahead) * (size_t)(PPS * TILE));
-                for (int off = lane * 128; off < TILE_BYTES; off += 32 * 128) prefetch_l2(t1 + off);
-            }
-#endif
-        }
-#endif
         const float4 *L = links + (size_t)(cb >> 5) * (size_t)(PPS * TILE) + (cb & 31);
         // packets first_d .. first_d + PPD - 1 hold direction d's numbers K*d .. K*d + K - 1
         auto load_links = [&](float4 (&pk)[PPD], const int d) {
             const int first = (K * d) >> 1, last = (K * d + K - 1) >> 1;
 #pragma unroll
             for (int i = 0; i < PPD; ++i)
-#if STAG_BATCH_EXP == 3
-                if (first + i <= last) pk[i] = make_float4(0.1f * d, 0.2f, 0.3f + i, 0.4f);
-#else
                 if (first + i <= last) pk[i] = ld_stream(L + (first + i) * TILE);
-#endif
         };
         float4 lk[NLB][PPD];
 #pragma unroll
@@ -166,12 +94,7 @@ dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
                 }
             }
         };
-        auto gather = [&](Unit &v, const int u, int nb) {
-#if STAG_BATCH_EXP == 2
-            nb = cb;
-#endif
-            gather_from(in, v, u, nb);
-        };
+        auto gather = [&](Unit &v, const int u, int nb) { gather_from(in, v, u, nb); };
 
         C acc[N][3];
 #pragma unroll
@@ -179,13 +102,6 @@ dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
 #pragma unroll
             for (int i = 0; i < 3; ++i) acc[k][i] = make_float2(0.f, 0.f);
 
-#if STAG_BATCH_FFMA2
-        float2 AX[(N / 2) ? (N / 2) : 1][3], AY[(N / 2) ? (N / 2) : 1][3];     // packed accumulators of the pairs
-#pragma unroll
-        for (int u = 0; u < N / 2; ++u)
-#pragma unroll
-            for (int i = 0; i < 3; ++i) AX[u][i] = AY[u][i] = make_float2(0.f, 0.f);
-#endif
         Unit vb[2];
         Unit ow[NU];       // the own-site vectors of the epilogue (MODE != HOP_PLAIN)
         gather(vb[0], 0, s.nbr[0]);
@@ -216,22 +132,6 @@ dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
                 if (step + 1 < 8 * NU) gather(vb[(step + 1) & 1], (u + 1) % NU, s.nbr[(step + 1) / NU]);
                 const Unit &v = vb[step & 1];
                 if (PAIRED && 2 * u + 1 < N) {
-#if STAG_BATCH_FFMA2
-                    float2 VX[3], VY[3];
-#pragma unroll
-                    for (int j = 0; j < 3; ++j) { VX[j] = make_float2(v.q[j].x, v.q[j].z); VY[j] = make_float2(v.q[j].y, v.q[j].w); }
-#pragma unroll
-                    for (int i = 0; i < 3; ++i)
-#pragma unroll
-                        for (int j = 0; j < 3; ++j) {
-                            const C mm = m[3 * i + j];
-                            const float2 MX = make_float2(mm.x, mm.x), MY = make_float2(mm.y, mm.y), nMY = make_float2(-mm.y, -mm.y);
-                            AX[u][i] = __ffma2_rn(MX, VX[j], AX[u][i]);
-                            AX[u][i] = __ffma2_rn(nMY, VY[j], AX[u][i]);
-                            AY[u][i] = __ffma2_rn(MX, VY[j], AY[u][i]);
-                            AY[u][i] = __ffma2_rn(MY, VX[j], AY[u][i]);
-                        }
-#else
 #pragma unroll
                     for (int i = 0; i < 3; ++i)
 #pragma unroll
@@ -239,7 +139,6 @@ dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
                             cfma(acc[2 * u][i], m[3 * i + j], make_float2(v.q[j].x, v.q[j].y));
                             cfma(acc[2 * u + 1][i], m[3 * i + j], make_float2(v.q[j].z, v.q[j].w));
                         }
-#endif
                 } else {
                     const int k = PAIRED ? N - 1 : u;
 #pragma unroll
@@ -250,17 +149,6 @@ dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
             }
         }
 
-#if STAG_BATCH_FFMA2
-        if constexpr (PAIRED) {
-#pragma unroll
-            for (int u = 0; u < N / 2; ++u)
-#pragma unroll
-                for (int i = 0; i < 3; ++i) {
-                    acc[2 * u][i] = make_float2(AX[u][i].x, AY[u][i].x);
-                    acc[2 * u + 1][i] = make_float2(AX[u][i].y, AY[u][i].y);
-                }
-        }
-#endif
         if (NR == 1 && cb >= g.Vh) {
             // a rebuilt 8-parameter matrix is unitary, never zero: pad lanes are zeroed here
 #pragma unroll
@@ -277,9 +165,6 @@ dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
                 for (int c = 0; c < 3; ++c) {
                     float4 *po = (float4 *)(out + 2 * j * rs) + (size_t)c * g.Vh_pad + cb;
                     if (MODE == HOP_PLAIN) {
-#if STAG_BATCH_EXP == 1
-                        if (acc[2 * j][c].x == 1.2345e-30f)
-#endif
                         st_keep(po, make_float4(acc[2 * j][c].x, acc[2 * j][c].y, acc[2 * j + 1][c].x, acc[2 * j + 1][c].y));
                     } else {
                         const float4 o = ow[j].q[c];
@@ -289,13 +174,8 @@ dslash_batch_kernel(float2 *__restrict__ out, const float2 *__restrict__ in,
                         r.z = fma(a, o.z, -sc * acc[2 * j + 1][c].x); r.w = fma(a, o.w, -sc * acc[2 * j + 1][c].y);
                         st_keep(po, r);
                         if (MODE == HOP_XPAY_DOT) {
-#if STAG_BATCH_EXP == 5
-                            dot[2 * j] += (double)(o.x * r.x + o.y * r.y);
-                            dot[2 * j + 1] += (double)(o.z * r.z + o.w * r.w);
-#else
                             dot[2 * j] += (double)o.x * (double)r.x + (double)o.y * (double)r.y;
                             dot[2 * j + 1] += (double)o.z * (double)r.z + (double)o.w * (double)r.w;
-#endif
                         }
                     }
                 }

@@ -316,9 +316,7 @@ template <int NR, int MODE, int N, bool PAIRED>
 int launch_batch_mode(const float4 *field, unsigned grid, float2 *out, const float2 *in, const Geom &g, int parity,
                       double a, double cD, const float2 *own, double *partials, const CgCtrl *ctrl, cudaStream_t s)
 {
-    // tiles (warps) of one wave of resident blocks: how far ahead a warp prefetches link tiles into L2
-    const int pf_ahead = (blas_full_grid() / 4) * BatchTune<NR, N>::MINB * (DSLASH_BLOCK / TILE);
-    dslash_batch_kernel<NR, MODE, N, PAIRED><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (float)a, (float)cD, own, partials, ctrl, pf_ahead);
+    dslash_batch_kernel<NR, MODE, N, PAIRED><<<grid, DSLASH_BLOCK, 0, s>>>(out, in, field, g, parity, (float)a, (float)cD, own, partials, ctrl);
     count_launch();
     KCHECK();
     return STAG_OK;
@@ -331,24 +329,6 @@ int launch_batch_n(const stag_links *L, int prec, int hop, float2 *out, const fl
     const Geom &g = L->g;
     const float4 *field = (const float4 *)L->L[prec] + (size_t)parity * L->ntiles * (8 * link_slots(NR) / 2) * TILE;
     const unsigned grid = (unsigned)((g.Vh_pad + DSLASH_BLOCK - 1) / DSLASH_BLOCK);
-    if constexpr (NR == 2 && PAIRED) {
-        // EXPERIMENT (stag_dslash_ring.cuh): STAG_BATCH_RING=1 sends the plain paired hop through the shared-memory ring
-        static const bool ring = getenv("STAG_BATCH_RING") && atoi(getenv("STAG_BATCH_RING")) > 0;
-        if (ring && hop == HOP_PLAIN) {
-            static std::atomic<int> ready{0};
-            if (!ready.load()) {
-                CU(cudaFuncSetAttribute(dslash_batch_ring_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, RING_SMEM));
-                ready.store(1);
-            }
-            unsigned rg = (unsigned)blas_full_grid();                      // 148 x 4 persistent blocks
-            const unsigned need = (unsigned)((L->ntiles + RING_WARPS - 1) / RING_WARPS);
-            if (rg > need) rg = need;
-            dslash_batch_ring_kernel<N><<<rg, DSLASH_BLOCK, RING_SMEM, s>>>(out, in, field, g, parity);
-            count_launch();
-            KCHECK();
-            return STAG_OK;
-        }
-    }
     switch (hop) {
     case HOP_PLAIN:    return launch_batch_mode<NR, HOP_PLAIN, N, PAIRED>(field, grid, out, in, g, parity, a, cD, own, partials, ctrl, s);
     case HOP_XPAY:     return launch_batch_mode<NR, HOP_XPAY, N, PAIRED>(field, grid, out, in, g, parity, a, cD, own, partials, ctrl, s);

@@ -18,26 +18,35 @@ static_assert(sizeof(CgCtrl) <= PERSIST_BAR_OFF && PERSIST_BAR_OFF + sizeof(unsi
 constexpr int PERSIST_AUTO_MAX_VH = 300000;
 constexpr int PERSIST_AUTO_MAX_VH_SLAB = 800000;
 
+// Most passes one persistent launch carries (params.persist_chunk is clamped to it).  The group
+// barrier compares a 32-bit arrival counter, reset at every launch, with a target that grows by the
+// group's block count at each of the <= 7 barriers of a pass: 65 536 passes x 7 x 296 blocks = 1.4e8,
+// far from wrapping -- an unchecked user value of a few million passes would wrap it and leave the
+// cooperative grid spinning for ever (the whole-lattice path has no watchdog).
+constexpr int PERSIST_MAX_CHUNK = 65536;
+
 inline bool persist_prec_ok(int prec)     // the 8-parameter forms stay on the kernel-per-step path
 {
     return prec == STAG_PREC_F64 || prec == STAG_PREC_F32 || prec == STAG_PREC_F64_R12 || prec == STAG_PREC_F32_R12;
 }
 
 // Blocks of the persistent kernel that can be resident at once on this device (the cooperative
-// launch refuses more).  One query per instantiation.
+// launch refuses more).  One query per instantiation and device.
 template <typename T, int NR, bool SLAB, bool LRES>
 int persist_capacity()
 {
-    static std::atomic<int> cap{0};
-    int c = cap.load(std::memory_order_relaxed);
+    constexpr int MAX_DEV = 64;                  // cached per device ordinal; beyond that, asked every time
+    static std::atomic<int> cap[MAX_DEV];        // zero-initialised
+    int dev = 0, sms = 0, per = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -1;
+    const bool cached = dev >= 0 && dev < MAX_DEV;
+    int c = cached ? cap[dev].load(std::memory_order_relaxed) : 0;
     if (c == 0) {
-        int dev = 0, sms = 0, per = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, cg_iter_persistent_kernel<T, NR, SLAB, LRES>, PERSIST_THREADS, 0) != cudaSuccess)
             return -1;
         c = sms * per;
-        cap.store(c, std::memory_order_relaxed);
+        if (cached) cap[dev].store(c, std::memory_order_relaxed);
     }
     return c;
 }
@@ -59,8 +68,7 @@ inline size_t persist_l2_budget()
     if (b == 0) {
         int dev = 0, l2 = 0;
         if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev) != cudaSuccess) l2 = 0;
-        if (const char *e = getenv("STAG_PERSIST_L2_BUDGET_MB")) b = (size_t)atol(e) << 20;     // measurement knob
-        else b = (size_t)l2 / 8 * 5;
+        b = (size_t)l2 / 8 * 5;
         if (b == 0) b = 1;
         budget.store(b, std::memory_order_relaxed);
     }
@@ -107,7 +115,12 @@ template <typename T, int NR, bool SLAB, bool LRES>
 int persist_launch_t(IterArgs<T> &A, cudaStream_t s)
 {
     const int cap = persist_capacity<T, NR, SLAB, LRES>();
-    if (cap < A.nlocal) return STAG_ECUDA;
+    if (cap < A.nlocal) {
+        snprintf(t_errbuf, sizeof(t_errbuf), "persistent kernel: %d rank group(s) but only %d block(s) can be resident on this device", A.nlocal, cap);
+        t_errbuf_status = STAG_ECUDA;
+        (void)cudaGetLastError();
+        return STAG_ECUDA;
+    }
     // split the resident blocks evenly among the rank groups, no group larger than its volume needs
     const int share = cap / A.nlocal;
     int grid = 0;

@@ -13,7 +13,6 @@
 #include "stag_common.cuh"
 #include "stag_dslash.cuh"
 #include "stag_dslash_batch.cuh"
-#include "stag_dslash_ring.cuh"
 #include "stag_slab.cuh"
 #include "stag_persist.cuh"
 
