@@ -249,7 +249,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_tot / max(1, args.steps) * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": workload_config(cfg, args.gpus, sample=sample),
+        "data": "synthetic", "config": workload_config(cfg, args.gpus),      # the repo arm's dict exactly; the sample is in cpu_baseline
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                          "threads": cores, "nproc": os.cpu_count(), "affinity": host_threads(),
                          "cpu_model": cpu_model(), "compile_flags": " ".join(flags)},
@@ -260,8 +260,15 @@ def run_reference(args):
     return 0
 
 
+def link_kind(cfg):
+    """The config's gauge field in words (fieldgen.CONFIGS; BASELINE.json configs)."""
+    if cfg.kind == "smooth":
+        return "smooth SU(3) links U = exp(i eps H), eps = %g" % cfg.eps
+    return {"random": "random SU(3) links", "unit": "unit links (free field)"}.get(cfg.kind, cfg.kind + " links")
+
+
 def workload_config(cfg, n_gpus, **extra):
-    c = {"workload": "%s staggered mixed-precision CG solve (mode 3, fp32 iteration on 12-real links, fp64 updates on 18-real links), random SU(3) links with eta and antiperiodic-t folded in, Gaussian even-site source, m=%g, tol=%g" % (cfg.name, cfg.mass, cfg.tol),
+    c = {"workload": "%s staggered mixed-precision CG solve (mode 3, fp32 iteration on 12-real links, fp64 updates on 18-real links), %s with eta and antiperiodic-t folded in, Gaussian even-site source, m=%g, tol=%g" % (cfg.name, link_kind(cfg), cfg.mass, cfg.tol),
          "dims": list(cfg.dims), "even_sites": cfg.vh, "mass": cfg.mass, "tol": cfg.tol,
          "maxiter": cfg.maxiter, "parallelism": "replicas x%d (no collective)" % n_gpus,
          "flop_convention": "1224 flop / even site / iteration = 2 x 576 (P:L62) + 72",
@@ -345,6 +352,49 @@ def hop_timings(stag, torch, fieldgen, cfg, L, select=None):
                for p, n in ((stag.PREC_F32_R12, 3), (stag.PREC_F32_R12, 4), (stag.PREC_F32, 4))
                if want("%s x%d blocked" % (stag.PREC_NAMES[p], n))}
     return dsl, batch, blocked
+
+
+def propagator_timings(stag, torch, cfg, L, peak):
+    """The production call (eq. 2.2): stag_solve_M, the
+    staggered propagator (D + m) psi = h, for the three colour point sources of one site (nrhs = 3)
+    and of four sites (nrhs = 12: three chunks of four, the links re-read once per chunk).  The whole
+    call is timed (CUDA events on the stream the library launches on): b_e = m h_e - D_eo h_o, the
+    lockstep mixed-precision solve, psi_o = (h_o - D_oe psi_e) / m.  byte floor per source and pass:
+    2 hops x 384 B of 12-real links shared by the chunk + 14 vector passes x 24 B."""
+    n = stag.spinor_bytes(cfg.dims, stag.PREC_F64) // 8          # reals per device spinor
+    vh_pad = n // 6
+    out = {}
+    for nsites in (1, 4):
+        nrhs = 3 * nsites
+        he = torch.zeros((nrhs, n), dtype=torch.float64, device="cuda")
+        ho = torch.zeros_like(he)
+        for j in range(nsites):
+            cb = (12345 + 77777 * j) % cfg.vh                    # odd-parity checkerboard index of the source site
+            for c in range(3):
+                ho[3 * j + c, (c * vh_pad + cb) * 2] = 1.0       # Re of colour c at that site (device layout v[c][cb])
+        stag.solve_M(he, ho, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True)      # warm-up: graphs, workspace
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        pe, po, sts = stag.solve_M(he, ho, L, cfg.mass, cfg.tol, cfg.maxiter, stag.CG_RELIABLE, recon12=True)
+        e1.record()
+        torch.cuda.synchronize()
+        sec = e0.elapsed_time(e1) * 1e-3
+        iters = [t["iters"] for t in sts]
+        chunk = min(nrhs, 4)
+        floor_bytes = (2 * 384.0 / chunk + 14 * 24.0) * cfg.vh
+        us = sec / max(1, max(iters)) / nrhs * 1e6
+        out["nrhs_%d" % nrhs] = {
+            "sources": "%d site(s) x 3 colours, point sources on odd sites" % nsites,
+            "status": [t["status"] for t in sts], "iters": iters, "true_resid_max": max(t["true_resid"] for t in sts),
+            "time_to_solution_s": sec, "cg_seconds": sts[0]["seconds"],
+            "gflops": sum(iters) * FLOP_PER_SITE_ITER * cfg.vh / sec * 1e-9,
+            "us_per_iteration_per_source": us,
+            "byte_floor_us_per_iteration_per_source": floor_bytes / peak * 1e-3,
+            "frac_of_byte_floor": floor_bytes / peak * 1e-3 / us,
+            "links_passes_per_hop": (nrhs + 3) // 4}
+        del he, ho, pe, po
+    return out
 
 
 def roofline_block(dsl, cfg, peak, peak_src):
@@ -510,6 +560,7 @@ def run_ours(args):
             "layout": "fp32 batches paired (include/stag.h batch layouts), fp64 blocked"}
     del b3, x3
     stag.set_workspace(None)
+    propagator = propagator_timings(stag, torch, cfg, L, peak)
 
     cpu, cpu_others = None, None
     if world == 1 and not args.no_cpu_baseline:
@@ -549,6 +600,7 @@ def run_ours(args):
                "speedup_mixed_vs_fp64": st64["seconds"] / st["seconds"]},
         "dslash": dsl,
         "mrhs": mrhs,
+        "propagator": propagator,
         "setup_s0_seconds": setup_s,
         "workspace": "caller-owned (stag_set_workspace), %d bytes" % ws.numel(),
         "paper_context": "GTX480: 145 GFLOPS SP / 55 DP per GPU pure-GPU CG (P:L131), 1.04 / 2.77 ms per Dirac op on a quarter lattice (Table 1)",

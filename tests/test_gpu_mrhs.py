@@ -189,34 +189,56 @@ def test_mrhs_argument_errors():
 
 @pytest.mark.slow
 def test_mrhs_full_size_hop_matches_oracle():
-    """bench configuration: three right-hand sides through the fp32/12 and fp64/18 batch hops,
-    every output site against the oracle."""
+    """bench configuration: three right-hand sides through the fp32/12 and fp64/18 batch hops in the
+    blocked layout, then 2, 3 and 4 right-hand sides through the PAIRED layout -- the instantiations
+    dslash_batch_kernel<.., PAIRED = true> that bench.py's `mrhs.dslash` rows time and the fp32
+    iteration of stag_cg_solve_mrhs runs on -- every output site against the oracle (eq. 2.5),
+    relative L2 error and worst component (tests/parity.py)."""
+    import torch
     cfg = fieldgen.CONFIGS["c4_28^3x96"]
     W = cfg.links()
     L = stag.Links(cfg.dims, W)
-    chis = [fieldgen.spinor_gaussian(cfg.dims, 0, seed=100 + k) for k in range(3)]
+    chis = [fieldgen.spinor_gaussian(cfg.dims, 0, seed=100 + k) for k in range(4)]
     refs = [oracle.dslash(c, W, cfg.dims, 1) for c in chis]
     for prec in (stag.PREC_F32_R12, stag.PREC_F32, stag.PREC_F64):
-        outs = stag.dslash_mrhs(stag.spinor_pack_mrhs(chis, cfg.dims, prec), L, 1, prec)
+        outs = stag.dslash_mrhs(stag.spinor_pack_mrhs(chis[:3], cfg.dims, prec), L, 1, prec)
         for k, o in enumerate(stag.spinor_unpack_mrhs(outs, cfg.dims, prec)):
             assert rel_l2(o, refs[k]) <= TOL[prec]
+    for prec in (stag.PREC_F32_R12, stag.PREC_F32):
+        for n in (2, 3, 4):
+            pv = stag.batch_convert(stag.spinor_pack_mrhs(chis[:n], cfg.dims, prec), cfg.dims, prec, stag.BATCH_PAIRED)
+            po = torch.full_like(pv, float("nan"))
+            stag.dslash_mrhs(pv, L, 1, prec, out=po, layout=stag.BATCH_PAIRED)
+            outs = stag.batch_convert(po, cfg.dims, prec, stag.BATCH_BLOCKED)
+            for k, o in enumerate(stag.spinor_unpack_mrhs(outs, cfg.dims, prec)):
+                assert rel_l2(o, refs[k]) <= TOL[prec], (prec, n, k)
+    L.close()
 
 
 @pytest.mark.slow
 def test_batched_solve_and_propagator_full_size_with_oracle_operators():
     """bench configuration (28^3 x 96): three sources in lockstep (mode 3, 12-real fp32 links), each
-    solution checked through the ORACLE's A; then the propagator wrapper for a point source in the
-    three colours, checked through the oracle's M = D + m on the whole lattice."""
+    solution checked through the ORACLE's A; right-hand side 0 is the config's own source, so its
+    solution is also held to north_star's "within 1e-8 relative of the oracle solve" (eq. 2.1-2.3,
+    P:L27-37) against the oracle's stored solve (tests/golden/refsol_c4_283x96.npz, tests/refsol.py);
+    then the propagator wrapper for a point source in the three colours, checked through the oracle's
+    M = D + m on the whole lattice."""
+    from tests import refsol
     cfg = fieldgen.CONFIGS["c4_28^3x96"]
+    rec = refsol.load(cfg.name)
     W = cfg.links()
     L = stag.Links(cfg.dims, W)
-    bs = [fieldgen.spinor_gaussian(cfg.dims, 0, seed=500 + k) for k in range(3)]
+    bs = [cfg.source()] + [fieldgen.spinor_gaussian(cfg.dims, 0, seed=500 + k) for k in (1, 2)]
     xs, sts = stag.cg_solve_mrhs(stag.spinor_pack_mrhs(bs, cfg.dims, 0), L, cfg.mass, cfg.tol, cfg.maxiter,
                                  stag.CG_RELIABLE, recon12=True)
     for k, x in enumerate(stag.spinor_unpack_mrhs(xs, cfg.dims, 0)):
         assert sts[k]["status"] == stag.OK and sts[k]["true_resid"] <= cfg.tol
         res = np.linalg.norm((bs[k] - oracle.apply_A(x, W, cfg.dims, cfg.mass)).ravel()) / np.linalg.norm(bs[k].ravel())
         assert res <= cfg.tol * (1 + 1e-3), (k, res)
+        if k == 0:
+            s = refsol.score(x, rec, cfg)
+            print("batched solve, right-hand side 0 vs the oracle's solve: %r" % (s,))
+            assert s["l2_sketch"] <= 1e-8 and s["l2_sites"] <= 1e-8 and s["max_site"] <= 1e-8 and s["norm"] <= 1e-8
     del xs
     hs = []
     for c in range(3):
